@@ -1,0 +1,143 @@
+/* rfim_pt.h -- C ABI of librfimpt.so: B200-native (sm_100a) Exchange Monte Carlo (parallel
+ * tempering) for the 3D Random Field Ising Model, after arxiv 1508.06268.
+ *
+ * Conventions
+ *  - Every pointer argument is HOST memory owned by the caller unless it says "device".
+ *    The library owns the handle and all device memory behind it.
+ *  - Device memory comes from the allocator hook (rfim_pt_set_allocator; default cudaMalloc);
+ *    kernels are enqueued on the handle's stream (rfim_pt_set_stream; default stream 0).
+ *  - rfim_pt_sweep / rfim_pt_adapt_temperatures's trial enqueue work and return without
+ *    synchronising where they can; every getter synchronises the handle's stream first.
+ *  - Return value: 0 (RFIM_OK) or a negative code; rfim_pt_last_error gives a message.
+ *    No exception crosses this boundary.  One host thread per handle at a time.
+ *  - Lattice: L even, >= 2; site i = x + L*(y + L*z), x fastest; spins are int8 +1/-1 at the
+ *    boundary (stored 1 byte or 1 bit per spin on the device).
+ *  - R is the slot capacity; n (<= R) temperatures are active.  A "slot" is a stored lattice
+ *    (lattices never move); a "rank" is a position in the ascending
+ *    temperature list.  Arrays "by rank" have n entries per realisation.
+ *  - A batch handle holds D independent disorder realisations ("members"), member d being
+ *    exactly a single handle created with seeds[d].  Calls without a member argument act on
+ *    all members; array outputs are then laid out [d][rank].
+ *  - The exact arithmetic (random-number keying, thresholds, exchange rule, adaptation rule)
+ *    is DESIGN.md section 3.
+ */
+#ifndef RFIM_PT_H
+#define RFIM_PT_H
+
+#include <stddef.h>
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+typedef struct rfim_pt rfim_pt;
+
+enum { RFIM_OK = 0, RFIM_EINVAL = -1, RFIM_ESTATE = -2, RFIM_ENOMEM = -3, RFIM_ECUDA = -4 };
+enum { RFIM_FIELD_BIMODAL = 0, RFIM_FIELD_GAUSSIAN = 1 };
+
+/* ---- the calls north_star names --------------------------------------------------------- */
+
+/* PAPER.md:65-69 (section 3.1 steps 2-3): one random field H shared by all replicas
+ * (bimodal h_i = +-1, or Gaussian N(0,1) on a 2^-20 grid), R random spin configurations.
+ * H = -J sum_<ij> s_i s_j - h sum_i h_i s_i (Eq. 1).  Temperatures must be set
+ * before sweeping.  EINVAL: odd or < 2 L, R < 1, bad field_kind, non-finite J or h. */
+int rfim_pt_create(rfim_pt** out, int L, int R, double J, double h, int field_kind, uint64_t seed);
+
+/* D realisations x R replicas in one handle (BASELINE.json config 5; "[..] average
+ * over different disorder realizations").  seeds: D values. */
+int rfim_pt_create_batch(rfim_pt** out, int L, int R, double J, double h, int field_kind,
+                         int D, const uint64_t* seeds);
+
+int rfim_pt_destroy(rfim_pt* h);
+
+/* PAPER.md:67 (step 1) + step 3's X_i <- beta_i: T[0..n) strictly ascending, > 0, 1 <= n <= R.
+ * Rank t is given to slot t (identity permutation); acceptance tables are rebuilt on the host in
+ * binary64 (S3); exchange statistics and the time series are reset; spins, the global
+ * sweep counter and the global exchange-step counter are kept.  Applies to every member. */
+int rfim_pt_set_temperatures(rfim_pt* h, const double* T, int n);
+
+/* PAPER.md:70 (step 4): n_sweeps checkerboard Metropolis sweeps (colour (x+y+z) mod 2 = 0, then 1;
+ * PAPER.md:101 Eq. 3) of every active replica; whenever the global sweep counter becomes a
+ * multiple of exchange_every (> 0) an exchange step runs: per-replica energy reduction
+ * (PAPER.md:220), one time-series row, then the even or odd adjacent pairs are swapped with
+ * probability min(1, e^Delta) (Eq. 2) by permuting temperatures
+ * (PAPER.md:131-137).  exchange_every = 0: never exchange.  Asynchronous.
+ * EINVAL: negative arguments; ESTATE: temperatures not set. */
+int rfim_pt_sweep(rfim_pt* h, int64_t n_sweeps, int exchange_every);
+
+/* PAPER.md:147-153 (section 4): reset statistics, run one trial of trial_sweeps sweeps, then
+ * insert midpoint temperatures where the exchange rate is lowest (growing n while n < R, else the
+ * fixed-count insert-and-prune rule of DESIGN.md S8).  Synchronises.
+ * ESTATE: temperatures not set, or a pair saw no exchange attempt in the trial. */
+int rfim_pt_adapt_temperatures(rfim_pt* h, int64_t trial_sweeps);
+
+/* By rank: E[t] = H of the replica now at rank t (Eq. 1), M[t] = (1/N) sum_i s_i (PAPER.md:251,
+ * Eq. 11 before |.|), exchange_rate[t] = accepted/attempted swaps of pair (t,t+1) since the last
+ * reset (-1 if none attempted).  Sizes D*n, D*n, D*(n-1); any pointer may be NULL.  Synchronises. */
+int rfim_pt_observables(rfim_pt* h, double* E, double* M, double* exchange_rate);
+
+/* Spins (+1/-1, L^3 bytes, x fastest) of the replica at temperature rank temp_rank of member 0. */
+int rfim_pt_get_spins(rfim_pt* h, int temp_rank, int8_t* out);
+
+/* ---- plumbing ------------------------------------------------------------------------------ */
+
+/* cuda_stream: a cudaStream_t (e.g. torch.cuda.current_stream().cuda_stream); NULL = default. */
+int rfim_pt_set_stream(rfim_pt* h, void* cuda_stream);
+int rfim_pt_synchronize(rfim_pt* h);
+/* Process-wide device allocator used by handles created afterwards.  alloc returns a device
+ * pointer or NULL; both NULL restores cudaMalloc/cudaFree. */
+typedef void* (*rfim_pt_alloc_fn)(size_t bytes);
+typedef void (*rfim_pt_free_fn)(void* device_ptr);
+int rfim_pt_set_allocator(rfim_pt_alloc_fn alloc, rfim_pt_free_fn release);
+const char* rfim_pt_last_error(rfim_pt* h);
+/* 8 = one byte per spin (default), 1 = bit-packed.  Converts the stored lattices in place. */
+int rfim_pt_set_packing(rfim_pt* h, int bits);
+/* which sweep implementation runs: 0 = automatic (default), others are listed in DESIGN.md. */
+int rfim_pt_set_kernel_variant(rfim_pt* h, int variant);
+/* exchange period used by adapt's trial (default 10) and insertions per trial
+ * (default 4, Fig. 6; the paper recommends 1-5). */
+int rfim_pt_set_adapt_params(rfim_pt* h, int exchange_every, int insertions);
+
+/* ---- extensions used by tests and the benchmark (state must be observable to be compared) -- */
+
+int rfim_pt_get_info(rfim_pt* h, int* L, int* R, int* n, int* D, int* field_kind);
+int rfim_pt_get_spins_member(rfim_pt* h, int d, int temp_rank, int8_t* out);
+int rfim_pt_get_spins_slot(rfim_pt* h, int d, int slot, int8_t* out);
+int rfim_pt_set_spins_slot(rfim_pt* h, int d, int slot, const int8_t* in);
+/* all D*R slots at once, [d][slot][L^3]; the host buffers of the end-to-end benchmark */
+int rfim_pt_get_spins_all(rfim_pt* h, int8_t* out);
+int rfim_pt_set_spins_all(rfim_pt* h, const int8_t* in);
+/* field of member d in natural site order: bimodal +-1, Gaussian g_i in units of 2^-20 */
+int rfim_pt_get_field(rfim_pt* h, int d, int32_t* out);
+int rfim_pt_set_field(rfim_pt* h, int d, const int32_t* in);
+int rfim_pt_get_permutation(rfim_pt* h, int d, int32_t* t2r);
+int rfim_pt_set_permutation(rfim_pt* h, int d, const int32_t* t2r);
+int rfim_pt_get_temperatures(rfim_pt* h, int d, double* T, int* n);
+int rfim_pt_get_counters(rfim_pt* h, uint64_t* sweep_index, uint64_t* exchange_step);
+int rfim_pt_set_counters(rfim_pt* h, uint64_t sweep_index, uint64_t exchange_step);
+/* integer energy terms by rank: Eb = sum_bonds s_i s_j, Ef = sum h_i s_i (or sum g_i s_i), Msum */
+int rfim_pt_get_energy_terms(rfim_pt* h, int d, int64_t* Eb, int64_t* Ef, int64_t* Msum);
+/* one row [rank] per exchange step since the last reset */
+int64_t rfim_pt_timeseries_steps(rfim_pt* h);
+int rfim_pt_get_timeseries(rfim_pt* h, int d, int64_t* Eb, int64_t* Ef, int64_t* Msum);
+int rfim_pt_get_exchange_counts(rfim_pt* h, int d, uint64_t* attempted, uint64_t* accepted);
+/* device acceptance table entry as the 33-bit threshold of DESIGN.md S3 (bimodal only) */
+int rfim_pt_get_bimodal_threshold(rfim_pt* h, int d, int rank, int k, int b, uint64_t* thr);
+/* diag[0] kernels launched so far, [1] Gaussian attempts decided by the exact binary64 path,
+ * [2] decisions within 1e-5 of a binary64 threshold (device and host exp could disagree there;
+ * expected 0), [3] exchange decisions taken with a random number */
+int rfim_pt_get_diagnostics(rfim_pt* h, uint64_t diag[4]);
+
+/* ---- roofline microbenchmarks (bench.py measures both bounds in the same run) ------------- */
+
+/* Philox4x32-10 only: calls_per_thread calls per thread, outputs folded; *ms = device time of one
+ * launch (CUDA events), *attempts = 4 * calls issued. */
+int rfim_pt_bench_philox(void* cuda_stream, int calls_per_thread, double* ms, double* attempts);
+/* streaming int8 read-modify-write over bytes bytes of device memory (> L2 for an HBM figure). */
+int rfim_pt_bench_stream(void* cuda_stream, size_t bytes, double* ms, double* bytes_moved);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* RFIM_PT_H */

@@ -10,7 +10,8 @@ import os
 
 import numpy as np
 
-from .build import LIB, build
+from .build import LIB
+from .build import build as _build_oracle
 
 _lib = None
 
@@ -26,7 +27,7 @@ _u64p = ctypes.POINTER(ctypes.c_uint64)
 def lib():
     global _lib
     if _lib is None:
-        build()
+        _build_oracle()
         L = ctypes.CDLL(LIB)
         sig = {
             "oracle_philox4x32_10": (None, [ctypes.c_uint32] * 6 + [_u32p]),

@@ -1,0 +1,311 @@
+"""Thin ctypes binding over librfimpt.so (include/rfim_pt.h): argument marshalling only.
+
+Every step of the hot path runs in the library's CUDA kernels.  PyTorch is used for the device
+allocator (installed as the library's allocator hook) and for the current stream.  There is no CPU
+fallback: if the library is missing or no CUDA device is present the calls raise.
+"""
+import ctypes
+import os
+
+import numpy as np
+
+_HERE = os.path.dirname(os.path.abspath(__file__))
+_LIB_PATH = os.path.join(_HERE, "librfimpt.so")
+_lib = None
+_alloc_refs = {}
+
+BIMODAL, GAUSSIAN = 0, 1
+OK, EINVAL, ESTATE, ENOMEM, ECUDA = 0, -1, -2, -3, -4
+
+_vp = ctypes.c_void_p
+_dp = ctypes.POINTER(ctypes.c_double)
+_ip = ctypes.POINTER(ctypes.c_int)
+_i8p = ctypes.POINTER(ctypes.c_int8)
+_i32p = ctypes.POINTER(ctypes.c_int32)
+_i64p = ctypes.POINTER(ctypes.c_int64)
+_u64p = ctypes.POINTER(ctypes.c_uint64)
+_ALLOC_FN = ctypes.CFUNCTYPE(ctypes.c_void_p, ctypes.c_size_t)
+_FREE_FN = ctypes.CFUNCTYPE(None, ctypes.c_void_p)
+
+# every symbol include/rfim_pt.h declares: name -> (restype, argtypes)
+SIGNATURES = {
+    "rfim_pt_create": (ctypes.c_int, [ctypes.POINTER(_vp), ctypes.c_int, ctypes.c_int, ctypes.c_double, ctypes.c_double,
+                                      ctypes.c_int, ctypes.c_uint64]),
+    "rfim_pt_create_batch": (ctypes.c_int, [ctypes.POINTER(_vp), ctypes.c_int, ctypes.c_int, ctypes.c_double,
+                                            ctypes.c_double, ctypes.c_int, ctypes.c_int, _u64p]),
+    "rfim_pt_destroy": (ctypes.c_int, [_vp]),
+    "rfim_pt_set_temperatures": (ctypes.c_int, [_vp, _dp, ctypes.c_int]),
+    "rfim_pt_sweep": (ctypes.c_int, [_vp, ctypes.c_int64, ctypes.c_int]),
+    "rfim_pt_adapt_temperatures": (ctypes.c_int, [_vp, ctypes.c_int64]),
+    "rfim_pt_observables": (ctypes.c_int, [_vp, _dp, _dp, _dp]),
+    "rfim_pt_get_spins": (ctypes.c_int, [_vp, ctypes.c_int, _i8p]),
+    "rfim_pt_set_stream": (ctypes.c_int, [_vp, _vp]),
+    "rfim_pt_synchronize": (ctypes.c_int, [_vp]),
+    "rfim_pt_set_allocator": (ctypes.c_int, [_ALLOC_FN, _FREE_FN]),
+    "rfim_pt_last_error": (ctypes.c_char_p, [_vp]),
+    "rfim_pt_set_packing": (ctypes.c_int, [_vp, ctypes.c_int]),
+    "rfim_pt_set_kernel_variant": (ctypes.c_int, [_vp, ctypes.c_int]),
+    "rfim_pt_set_adapt_params": (ctypes.c_int, [_vp, ctypes.c_int, ctypes.c_int]),
+    "rfim_pt_get_info": (ctypes.c_int, [_vp, _ip, _ip, _ip, _ip, _ip]),
+    "rfim_pt_get_spins_member": (ctypes.c_int, [_vp, ctypes.c_int, ctypes.c_int, _i8p]),
+    "rfim_pt_get_spins_slot": (ctypes.c_int, [_vp, ctypes.c_int, ctypes.c_int, _i8p]),
+    "rfim_pt_set_spins_slot": (ctypes.c_int, [_vp, ctypes.c_int, ctypes.c_int, _i8p]),
+    "rfim_pt_get_spins_all": (ctypes.c_int, [_vp, _i8p]),
+    "rfim_pt_set_spins_all": (ctypes.c_int, [_vp, _i8p]),
+    "rfim_pt_get_field": (ctypes.c_int, [_vp, ctypes.c_int, _i32p]),
+    "rfim_pt_set_field": (ctypes.c_int, [_vp, ctypes.c_int, _i32p]),
+    "rfim_pt_get_permutation": (ctypes.c_int, [_vp, ctypes.c_int, _i32p]),
+    "rfim_pt_set_permutation": (ctypes.c_int, [_vp, ctypes.c_int, _i32p]),
+    "rfim_pt_get_temperatures": (ctypes.c_int, [_vp, ctypes.c_int, _dp, _ip]),
+    "rfim_pt_get_counters": (ctypes.c_int, [_vp, _u64p, _u64p]),
+    "rfim_pt_set_counters": (ctypes.c_int, [_vp, ctypes.c_uint64, ctypes.c_uint64]),
+    "rfim_pt_get_energy_terms": (ctypes.c_int, [_vp, ctypes.c_int, _i64p, _i64p, _i64p]),
+    "rfim_pt_timeseries_steps": (ctypes.c_int64, [_vp]),
+    "rfim_pt_get_timeseries": (ctypes.c_int, [_vp, ctypes.c_int, _i64p, _i64p, _i64p]),
+    "rfim_pt_get_exchange_counts": (ctypes.c_int, [_vp, ctypes.c_int, _u64p, _u64p]),
+    "rfim_pt_get_bimodal_threshold": (ctypes.c_int, [_vp, ctypes.c_int, ctypes.c_int, ctypes.c_int, ctypes.c_int, _u64p]),
+    "rfim_pt_get_diagnostics": (ctypes.c_int, [_vp, _u64p]),
+    "rfim_pt_bench_philox": (ctypes.c_int, [_vp, ctypes.c_int, _dp, _dp]),
+    "rfim_pt_bench_stream": (ctypes.c_int, [_vp, ctypes.c_size_t, _dp, _dp]),
+}
+
+
+class RfimPtError(RuntimeError):
+    def __init__(self, code, msg):
+        super().__init__(f"librfimpt error {code}: {msg}")
+        self.code = code
+
+
+def load():
+    """dlopen the library and type every entry point (no GPU needed for this)."""
+    global _lib
+    if _lib is None:
+        if not os.path.exists(_LIB_PATH):
+            raise RuntimeError(f"{_LIB_PATH} is missing: run `python -m paper_1508_06268_b200.build` "
+                               "(the CUDA extension is the product; there is no fallback)")
+        L = ctypes.CDLL(_LIB_PATH)
+        for name, (res, args) in SIGNATURES.items():
+            fn = getattr(L, name)
+            fn.restype = res
+            fn.argtypes = args
+        _lib = L
+    return _lib
+
+
+def use_torch_allocator():
+    """Route the library's device allocations through PyTorch's CUDA caching allocator."""
+    import torch
+    lib = load()
+
+    def _alloc(nbytes):
+        try:
+            return torch.cuda.caching_allocator_alloc(int(nbytes))
+        except Exception:
+            return None
+
+    def _free(ptr):
+        if ptr:
+            torch.cuda.caching_allocator_delete(ptr)
+
+    a, f = _ALLOC_FN(_alloc), _FREE_FN(_free)
+    _alloc_refs["alloc"], _alloc_refs["free"] = a, f          # keep the thunks alive
+    rc = lib.rfim_pt_set_allocator(a, f)
+    if rc:
+        raise RfimPtError(rc, "rfim_pt_set_allocator")
+
+
+def _p(a, t):
+    return a.ctypes.data_as(t)
+
+
+class RfimPT:
+    """Handle on D realisations x R replica slots of an L^3 lattice (see include/rfim_pt.h)."""
+
+    def __init__(self, L, R, J, h, field_kind, seed=None, seeds=None, torch_allocator=True, torch_stream=True):
+        lib = load()
+        if torch_allocator:
+            import torch
+            if not torch.cuda.is_available():
+                raise RuntimeError("no CUDA device: librfimpt has no CPU fallback")
+            torch.cuda.init()
+            use_torch_allocator()
+        self._h = _vp()
+        if seeds is None:
+            rc = lib.rfim_pt_create(ctypes.byref(self._h), L, R, J, h, field_kind, int(seed))
+            self.D = 1
+        else:
+            s = np.ascontiguousarray(seeds, dtype=np.uint64)
+            rc = lib.rfim_pt_create_batch(ctypes.byref(self._h), L, R, J, h, field_kind, len(s), _p(s, _u64p))
+            self.D = len(s)
+        if rc:
+            raise RfimPtError(rc, "rfim_pt_create failed (bad argument, no CUDA device, or out of memory)")
+        self.L, self.R, self.J, self.h, self.kind = L, R, J, h, field_kind
+        self.N = L ** 3
+        self._torch_stream = torch_stream
+        if torch_stream:
+            self.use_current_torch_stream()
+
+    # -- plumbing ---------------------------------------------------------------------------
+    def _ck(self, rc):
+        if rc:
+            raise RfimPtError(rc, load().rfim_pt_last_error(self._h).decode())
+
+    def use_current_torch_stream(self):
+        import torch
+        self._ck(load().rfim_pt_set_stream(self._h, _vp(torch.cuda.current_stream().cuda_stream)))
+
+    def set_stream(self, cuda_stream_ptr):
+        self._ck(load().rfim_pt_set_stream(self._h, _vp(cuda_stream_ptr)))
+
+    def synchronize(self):
+        self._ck(load().rfim_pt_synchronize(self._h))
+
+    def close(self):
+        if getattr(self, "_h", None):
+            load().rfim_pt_destroy(self._h)
+            self._h = _vp()
+
+    def __del__(self):
+        try:
+            self.close()
+        except Exception:
+            pass
+
+    @property
+    def n(self):
+        n = ctypes.c_int()
+        self._ck(load().rfim_pt_get_info(self._h, None, None, ctypes.byref(n), None, None))
+        return n.value
+
+    # -- the calls north_star names ---------------------------------------------------------------
+    def set_temperatures(self, T):
+        T = np.ascontiguousarray(T, dtype=np.float64)
+        self._ck(load().rfim_pt_set_temperatures(self._h, _p(T, _dp), len(T)))
+
+    def sweep(self, n_sweeps, exchange_every):
+        self._ck(load().rfim_pt_sweep(self._h, int(n_sweeps), int(exchange_every)))
+
+    def adapt_temperatures(self, trial_sweeps):
+        self._ck(load().rfim_pt_adapt_temperatures(self._h, int(trial_sweeps)))
+
+    def observables(self):
+        n, D = self.n, self.D
+        E = np.zeros((D, n)); M = np.zeros((D, n)); rate = np.zeros((D, max(n - 1, 0)))
+        self._ck(load().rfim_pt_observables(self._h, _p(E, _dp), _p(M, _dp), _p(rate, _dp)))
+        if D == 1:
+            return E[0], M[0], rate[0]
+        return E, M, rate
+
+    def get_spins(self, temp_rank, d=0):
+        out = np.zeros(self.N, dtype=np.int8)
+        self._ck(load().rfim_pt_get_spins_member(self._h, d, temp_rank, _p(out, _i8p)))
+        return out
+
+    # -- extensions ------------------------------------------------------------------------------
+    def set_packing(self, bits):
+        self._ck(load().rfim_pt_set_packing(self._h, bits))
+
+    def set_kernel_variant(self, variant):
+        self._ck(load().rfim_pt_set_kernel_variant(self._h, variant))
+
+    def set_adapt_params(self, exchange_every, insertions):
+        self._ck(load().rfim_pt_set_adapt_params(self._h, exchange_every, insertions))
+
+    def get_spins_slot(self, slot, d=0):
+        out = np.zeros(self.N, dtype=np.int8)
+        self._ck(load().rfim_pt_get_spins_slot(self._h, d, slot, _p(out, _i8p)))
+        return out
+
+    def set_spins_slot(self, slot, s, d=0):
+        s = np.ascontiguousarray(s, dtype=np.int8)
+        assert s.size == self.N
+        self._ck(load().rfim_pt_set_spins_slot(self._h, d, slot, _p(s, _i8p)))
+
+    def get_spins_all(self, out=None):
+        if out is None:
+            out = np.zeros((self.D, self.R, self.N), dtype=np.int8)
+        self._ck(load().rfim_pt_get_spins_all(self._h, _p(out, _i8p)))
+        return out
+
+    def set_spins_all(self, s):
+        assert s.dtype == np.int8 and s.size == self.D * self.R * self.N and s.flags.c_contiguous
+        self._ck(load().rfim_pt_set_spins_all(self._h, _p(s, _i8p)))
+
+    def get_field(self, d=0):
+        out = np.zeros(self.N, dtype=np.int32)
+        self._ck(load().rfim_pt_get_field(self._h, d, _p(out, _i32p)))
+        return out
+
+    def set_field(self, f, d=0):
+        f = np.ascontiguousarray(f, dtype=np.int32)
+        assert f.size == self.N
+        self._ck(load().rfim_pt_set_field(self._h, d, _p(f, _i32p)))
+
+    def get_permutation(self, d=0):
+        out = np.zeros(self.n, dtype=np.int32)
+        self._ck(load().rfim_pt_get_permutation(self._h, d, _p(out, _i32p)))
+        return out
+
+    def set_permutation(self, t2r, d=0):
+        t2r = np.ascontiguousarray(t2r, dtype=np.int32)
+        assert t2r.size == self.n
+        self._ck(load().rfim_pt_set_permutation(self._h, d, _p(t2r, _i32p)))
+
+    def get_temperatures(self, d=0):
+        out = np.zeros(self.n)
+        self._ck(load().rfim_pt_get_temperatures(self._h, d, _p(out, _dp), None))
+        return out
+
+    def get_counters(self):
+        a, b = ctypes.c_uint64(), ctypes.c_uint64()
+        self._ck(load().rfim_pt_get_counters(self._h, ctypes.byref(a), ctypes.byref(b)))
+        return a.value, b.value
+
+    def set_counters(self, sweep_index, exchange_step):
+        self._ck(load().rfim_pt_set_counters(self._h, sweep_index, exchange_step))
+
+    def get_energy_terms(self, d=0):
+        n = self.n
+        Eb = np.zeros(n, dtype=np.int64); Ef = np.zeros(n, dtype=np.int64); Ms = np.zeros(n, dtype=np.int64)
+        self._ck(load().rfim_pt_get_energy_terms(self._h, d, _p(Eb, _i64p), _p(Ef, _i64p), _p(Ms, _i64p)))
+        return Eb, Ef, Ms
+
+    def get_timeseries(self, d=0):
+        steps = int(load().rfim_pt_timeseries_steps(self._h))
+        n = self.n
+        Eb = np.zeros((steps, n), dtype=np.int64); Ef = np.zeros_like(Eb); Ms = np.zeros_like(Eb)
+        if steps:
+            self._ck(load().rfim_pt_get_timeseries(self._h, d, _p(Eb, _i64p), _p(Ef, _i64p), _p(Ms, _i64p)))
+        return Eb, Ef, Ms
+
+    def get_exchange_counts(self, d=0):
+        n = self.n
+        att = np.zeros(max(n - 1, 0), dtype=np.uint64); acc = np.zeros_like(att)
+        self._ck(load().rfim_pt_get_exchange_counts(self._h, d, _p(att, _u64p), _p(acc, _u64p)))
+        return att, acc
+
+    def bimodal_threshold(self, rank, k, b, d=0):
+        thr = ctypes.c_uint64()
+        self._ck(load().rfim_pt_get_bimodal_threshold(self._h, d, rank, k, b, ctypes.byref(thr)))
+        return thr.value
+
+    def diagnostics(self):
+        d = (ctypes.c_uint64 * 4)()
+        self._ck(load().rfim_pt_get_diagnostics(self._h, d))
+        return {"launches": int(d[0]), "exact_path": int(d[1]), "ulp_ambiguous": int(d[2]), "exchange_draws": int(d[3])}
+
+
+def bench_philox(calls_per_thread=2000, stream=None):
+    ms, att = ctypes.c_double(), ctypes.c_double()
+    rc = load().rfim_pt_bench_philox(_vp(stream or 0), calls_per_thread, ctypes.byref(ms), ctypes.byref(att))
+    if rc:
+        raise RfimPtError(rc, "rfim_pt_bench_philox")
+    return ms.value, att.value
+
+
+def bench_stream(nbytes, stream=None):
+    ms, moved = ctypes.c_double(), ctypes.c_double()
+    rc = load().rfim_pt_bench_stream(_vp(stream or 0), nbytes, ctypes.byref(ms), ctypes.byref(moved))
+    if rc:
+        raise RfimPtError(rc, "rfim_pt_bench_stream")
+    return ms.value, moved.value

@@ -1,0 +1,920 @@
+// rfim_pt.cu -- host side of librfimpt.so: the C ABI of include/rfim_pt.h.
+// Handle, device buffers, acceptance tables (binary64 on the host, S3), kernel launch
+// sequencing for sweep / reduce / exchange, the adaptation rule (S8), getters.
+// No part of this file includes, links or calls anything under oracle/.
+#include <cuda_runtime.h>
+
+#include <algorithm>
+#include <cmath>
+#include <cstdint>
+#include <cstdio>
+#include <cstring>
+#include <string>
+#include <vector>
+
+#include "../../include/rfim_pt.h"
+#include "kernels_ref.cuh"
+#include "philox.cuh"
+#include "view.h"
+
+using namespace rfim;
+
+namespace {
+
+rfim_pt_alloc_fn g_alloc = nullptr;
+rfim_pt_free_fn g_free = nullptr;
+
+constexpr double kTwo32 = 4294967296.0;
+constexpr double kFieldScale = 1048576.0;   // 2^20
+constexpr int32_t kFieldClamp = 8 * 1048576;
+
+}  // namespace
+
+struct rfim_pt {
+    int L = 0, R = 0, n = 0, D = 1, kind = 0;
+    long long N = 0, Nh = 0;
+    double J = 0, h = 0;
+    std::vector<uint64_t> seeds;
+    cudaStream_t stream = nullptr;
+    bool have_T = false;
+    std::vector<int32_t> field_nat;   // [D][N] natural order: +-1 or g_i
+    std::vector<double> amax;         // [D] max |hs * g_i|
+    std::vector<double> T;            // [D][R] by rank
+    View v{};
+    std::vector<void*> owned;         // every device allocation, released in destroy
+    int8_t* stage = nullptr;          // device staging for spin import/export
+    size_t stage_bytes = 0;
+    uint64_t sweep_g = 0, xstep = 0;
+    long long series_steps = 0, series_cap = 0;
+    int adapt_k = 10, adapt_a = 4;
+    int packing = 8, variant = 0;
+    uint64_t launches = 0;
+    std::string err;
+};
+
+namespace {
+
+int fail(rfim_pt* h, int code, const std::string& msg) {
+    if (h) h->err = msg;
+    return code;
+}
+
+#define CU(call)                                                                                   \
+    do {                                                                                           \
+        cudaError_t e_ = (call);                                                                   \
+        if (e_ != cudaSuccess)                                                                     \
+            return fail(h, RFIM_ECUDA, std::string(#call) + ": " + cudaGetErrorString(e_));        \
+    } while (0)
+
+void* dev_alloc(size_t bytes) {
+    if (bytes == 0) bytes = 16;
+    if (g_alloc) return g_alloc(bytes);
+    void* p = nullptr;
+    if (cudaMalloc(&p, bytes) != cudaSuccess) return nullptr;
+    return p;
+}
+void dev_free(void* p) {
+    if (!p) return;
+    if (g_free) g_free(p); else cudaFree(p);
+}
+
+template <class Tp>
+int alloc_into(rfim_pt* h, Tp** out, size_t count) {
+    void* p = dev_alloc(count * sizeof(Tp));
+    if (!p) return fail(h, RFIM_ENOMEM, "device allocation failed");
+    h->owned.push_back(p);
+    *out = reinterpret_cast<Tp*>(p);
+    return RFIM_OK;
+}
+void release(rfim_pt* h, void* p) {
+    auto it = std::find(h->owned.begin(), h->owned.end(), p);
+    if (it != h->owned.end()) h->owned.erase(it);
+    dev_free(p);
+}
+
+inline long long layout_index(const rfim_pt* h, int x, int y, int z, int* colour) {
+    *colour = (x + y + z) & 1;
+    return (long long)(x >> 1) + (long long)(h->L / 2) * (y + (long long)h->L * z);
+}
+
+dim3 grid_for(long long work, int ny, int threads = 256) {
+    long long bx = (work + threads - 1) / threads;
+    if (bx < 1) bx = 1;
+    if (bx > 4096) bx = 4096;
+    return dim3((unsigned)bx, (unsigned)ny, 1);
+}
+
+// ---- field ---------------------------------------------------------------------------------
+void generate_field_host(rfim_pt* h, int d) {
+    const uint32_t k0 = (uint32_t)(h->seeds[d] & 0xFFFFFFFFull), k1 = (uint32_t)(h->seeds[d] >> 32);
+    int32_t* f = h->field_nat.data() + (long long)d * h->N;
+    for (long long i = 0; i < h->N; ++i) {
+        const Words4 w = philox4x32_10(k0, k1, (uint32_t)i, 0u, 0u, kDomField);
+        if (h->kind == RFIM_FIELD_BIMODAL) {
+            f[i] = (w.w0 >> 31) ? 1 : -1;
+        } else {
+            const double u1 = ((double)w.w0 + 1.0) / kTwo32;
+            const double u2 = (double)w.w1 / kTwo32;
+            const double radius = std::sqrt(-2.0 * std::log(u1));
+            const double z = radius * std::cos((2.0 * M_PI) * u2);
+            long long q = std::llrint(z * kFieldScale);
+            q = std::min<long long>(std::max<long long>(q, -kFieldClamp), kFieldClamp);
+            f[i] = (int32_t)q;
+        }
+    }
+}
+
+int upload_field(rfim_pt* h, int d) {
+    const int L = h->L;
+    const int32_t* f = h->field_nat.data() + (long long)d * h->N;
+    const double hs = h->v.hs;
+    if (h->kind == RFIM_FIELD_BIMODAL) {
+        std::vector<uint8_t> fb(h->N);
+        for (int z = 0; z < L; ++z) for (int y = 0; y < L; ++y) for (int x = 0; x < L; ++x) {
+            int c; const long long j = layout_index(h, x, y, z, &c);
+            fb[(long long)c * h->Nh + j] = f[x + (long long)L * (y + (long long)L * z)] > 0 ? 0x10 : 0x00;
+        }
+        CU(cudaMemcpyAsync(const_cast<uint8_t*>(h->v.fieldb) + (long long)d * h->N, fb.data(), h->N, cudaMemcpyHostToDevice, h->stream));
+        CU(cudaStreamSynchronize(h->stream));
+        h->amax[d] = std::fabs(hs);
+    } else {
+        std::vector<float> fa(h->N);
+        std::vector<int32_t> fg(h->N);
+        double amax = 0.0;
+        for (int z = 0; z < L; ++z) for (int y = 0; y < L; ++y) for (int x = 0; x < L; ++x) {
+            int c; const long long j = layout_index(h, x, y, z, &c);
+            const int32_t g = f[x + (long long)L * (y + (long long)L * z)];
+            const double a = hs * (double)g;
+            fa[(long long)c * h->Nh + j] = (float)a;
+            fg[(long long)c * h->Nh + j] = g;
+            amax = std::max(amax, std::fabs(a));
+        }
+        CU(cudaMemcpyAsync(const_cast<float*>(h->v.fielda) + (long long)d * h->N, fa.data(), h->N * sizeof(float), cudaMemcpyHostToDevice, h->stream));
+        CU(cudaMemcpyAsync(const_cast<int32_t*>(h->v.fieldg) + (long long)d * h->N, fg.data(), h->N * sizeof(int32_t), cudaMemcpyHostToDevice, h->stream));
+        CU(cudaStreamSynchronize(h->stream));
+        h->amax[d] = amax;
+    }
+    return RFIM_OK;
+}
+
+// ---- acceptance tables (S3), binary64 on the host -----------------------------------
+uint64_t threshold33(double x) {
+    const double p = std::exp(-x);
+    if (p >= 1.0) return (uint64_t)1 << 32;
+    return (uint64_t)std::floor(p * kTwo32);
+}
+
+int upload_tables(rfim_pt* h) {
+    const int R = h->R, n = h->n, D = h->D;
+    std::vector<double> beta((size_t)D * R, 0.0);
+    for (int d = 0; d < D; ++d)
+        for (int t = 0; t < n; ++t) beta[(size_t)d * R + t] = 1.0 / h->T[(size_t)d * R + t];
+    CU(cudaMemcpyAsync(const_cast<double*>(h->v.beta), beta.data(), beta.size() * sizeof(double), cudaMemcpyHostToDevice, h->stream));
+    if (h->kind == RFIM_FIELD_BIMODAL) {
+        std::vector<uint32_t> etab((size_t)D * R * 32, 0u), never((size_t)D * R, 0u);
+        for (int d = 0; d < D; ++d)
+            for (int t = 0; t < n; ++t) {
+                const double b = beta[(size_t)d * R + t];
+                uint32_t nv = 0;
+                for (int idx = 0; idx < 32; ++idx) {
+                    const int n1 = idx & 7, s = (idx >> 3) & 1, hb = (idx >> 4) & 1;
+                    if (n1 == 7) { nv |= 1u << idx; continue; }              // unreachable neighbour count
+                    const int k = s ? n1 : 6 - n1;                            // k = (s*n + 6)/2
+                    const int bb = (s == hb) ? 1 : 0;                         // b = (s*h_i + 1)/2
+                    const double dE = 2.0 * (h->J * (double)(2 * k - 6) + h->h * (double)(2 * bb - 1));
+                    const uint64_t thr = threshold33(dE * b);
+                    if (thr == 0) nv |= 1u << idx;
+                    etab[((size_t)d * R + t) * 32 + idx] = (uint32_t)(thr - 1);
+                }
+                never[(size_t)d * R + t] = nv;
+            }
+        CU(cudaMemcpyAsync(const_cast<uint32_t*>(h->v.etab), etab.data(), etab.size() * 4, cudaMemcpyHostToDevice, h->stream));
+        CU(cudaMemcpyAsync(const_cast<uint32_t*>(h->v.never), never.data(), never.size() * 4, cudaMemcpyHostToDevice, h->stream));
+    } else {
+        std::vector<GaussEntry> gtab((size_t)D * R * 16);
+        std::vector<float> band((size_t)D * R, 0.f);
+        for (int d = 0; d < D; ++d)
+            for (int t = 0; t < n; ++t) {
+                const double b = beta[(size_t)d * R + t];
+                const double c = -2.0 * b * M_LOG2E;              // log2 P = c * sigma * (J n + a) ; +32 for the 2^32 scale
+                for (int idx = 0; idx < 16; ++idx) {
+                    const int n1 = idx & 7, s = (idx >> 3) & 1;
+                    const double sigma = s ? 1.0 : -1.0;
+                    GaussEntry e;
+                    e.x = (float)(c * sigma * h->J * (double)(2 * n1 - 6) + 32.0);
+                    e.y = (float)(c * sigma);
+                    gtab[((size_t)d * R + t) * 16 + idx] = e;
+                }
+                // guard band: bound on |P~ - P| over the float path, in units of u
+                const double aY = h->amax[d] * std::fabs(c);
+                const double Xmax = std::fabs(c) * std::fabs(h->J) * 6.0 + 32.0;
+                const double arg_err = std::ldexp(3.0 * aY + 2.0 * Xmax, -24);
+                const double eta = M_LN2 * arg_err + std::ldexp(1.0, -21) + std::ldexp(1.0, -23);
+                const double bd = 1.5 * eta * kTwo32 + 512.0;
+                band[(size_t)d * R + t] = (float)std::min(bd, 3.0e38);
+            }
+        CU(cudaMemcpyAsync(const_cast<GaussEntry*>(h->v.gtab), gtab.data(), gtab.size() * sizeof(GaussEntry), cudaMemcpyHostToDevice, h->stream));
+        CU(cudaMemcpyAsync(const_cast<float*>(h->v.band), band.data(), band.size() * 4, cudaMemcpyHostToDevice, h->stream));
+    }
+    CU(cudaStreamSynchronize(h->stream));   // host vectors go out of scope
+    return RFIM_OK;
+}
+
+int reset_statistics(rfim_pt* h) {
+    const size_t DR = (size_t)h->D * h->R;
+    CU(cudaMemsetAsync(h->v.att, 0, DR * 8, h->stream));
+    CU(cudaMemsetAsync(h->v.accn, 0, DR * 8, h->stream));
+    CU(cudaMemsetAsync(h->v.acc, 0, DR * 3 * 8, h->stream));
+    h->series_steps = 0;
+    return RFIM_OK;
+}
+
+int upload_permutation(rfim_pt* h, const std::vector<int32_t>& t2r) {   // [D][R], -1 beyond n
+    std::vector<int32_t> r2t((size_t)h->D * h->R, -1);
+    for (int d = 0; d < h->D; ++d)
+        for (int t = 0; t < h->n; ++t) r2t[(size_t)d * h->R + t2r[(size_t)d * h->R + t]] = t;
+    CU(cudaMemcpyAsync(h->v.t2r, t2r.data(), t2r.size() * 4, cudaMemcpyHostToDevice, h->stream));
+    CU(cudaMemcpyAsync(h->v.r2t, r2t.data(), r2t.size() * 4, cudaMemcpyHostToDevice, h->stream));
+    CU(cudaStreamSynchronize(h->stream));
+    return RFIM_OK;
+}
+
+int ensure_series(rfim_pt* h, long long rows) {
+    if (rows <= h->series_cap) return RFIM_OK;
+    long long cap = std::max<long long>(rows, h->series_cap * 2);
+    cap = std::max<long long>(cap, 64);
+    const size_t row_elems = (size_t)h->D * h->R * 3;
+    long long* p = nullptr;
+    int rc = alloc_into(h, &p, (size_t)cap * row_elems);
+    if (rc) return rc;
+    if (h->v.series && h->series_steps > 0)
+        CU(cudaMemcpyAsync(p, h->v.series, (size_t)h->series_steps * row_elems * 8, cudaMemcpyDeviceToDevice, h->stream));
+    if (h->v.series) { CU(cudaStreamSynchronize(h->stream)); release(h, h->v.series); }
+    h->v.series = p;
+    h->series_cap = cap;
+    return RFIM_OK;
+}
+
+int ensure_stage(rfim_pt* h, size_t bytes) {
+    if (bytes <= h->stage_bytes) return RFIM_OK;
+    if (h->stage) { CU(cudaStreamSynchronize(h->stream)); release(h, h->stage); h->stage = nullptr; h->stage_bytes = 0; }
+    int rc = alloc_into(h, &h->stage, bytes);
+    if (rc) return rc;
+    h->stage_bytes = bytes;
+    return RFIM_OK;
+}
+
+// ---- launches ------------------------------------------------------------------------------
+int launch_sweep(rfim_pt* h) {
+    const int ny = h->D * h->n;
+    const uint32_t g32 = (uint32_t)h->sweep_g;
+    const bool word = (h->variant == 2) || (h->variant == 0 && h->v.W > 0);
+    if (h->variant == 2 && h->v.W == 0) return fail(h, RFIM_EINVAL, "word kernel needs L % 8 == 0");
+    for (int colour = 0; colour < 2; ++colour) {
+        if (word) k_sweep_word<<<grid_for(h->Nh / 4, ny), 256, 0, h->stream>>>(h->v, colour, g32);
+        else k_sweep_site<<<grid_for(h->Nh, ny), 256, 0, h->stream>>>(h->v, colour, g32);
+        h->launches += 1;
+    }
+    CU(cudaGetLastError());
+    return RFIM_OK;
+}
+
+int launch_reduce(rfim_pt* h) {
+    k_reduce_site<<<grid_for(h->Nh, h->D * h->n), 256, 0, h->stream>>>(h->v);
+    h->launches += 1;
+    CU(cudaGetLastError());
+    return RFIM_OK;
+}
+
+int launch_exchange(rfim_pt* h) {
+    int threads = 32;
+    while (threads < h->n && threads < 1024) threads *= 2;
+    k_exchange<<<h->D, threads, 0, h->stream>>>(h->v, (uint32_t)h->xstep, h->series_steps, 1);
+    h->launches += 1;
+    CU(cudaGetLastError());
+    return RFIM_OK;
+}
+
+int do_sweeps(rfim_pt* h, int64_t n_sweeps, int k) {
+    if (!h->have_T) return fail(h, RFIM_ESTATE, "temperatures not set");
+    if (n_sweeps < 0 || k < 0) return fail(h, RFIM_EINVAL, "negative argument");
+    if (k > 0) {
+        h->adapt_k = k;
+        const long long steps = (long long)((h->sweep_g + (uint64_t)n_sweeps) / (uint64_t)k - h->sweep_g / (uint64_t)k);
+        int rc = ensure_series(h, h->series_steps + steps);
+        if (rc) return rc;
+    }
+    for (int64_t it = 0; it < n_sweeps; ++it) {
+        int rc = launch_sweep(h);
+        if (rc) return rc;
+        h->sweep_g += 1;
+        if (k > 0 && (h->sweep_g % (uint64_t)k) == 0) {
+            if ((rc = launch_reduce(h))) return rc;
+            if ((rc = launch_exchange(h))) return rc;
+            h->series_steps += 1;
+            h->xstep += 1;
+        }
+    }
+    return RFIM_OK;
+}
+
+// current integer terms of every active replica, by rank: out [D][n][3]; also returns t2r [D][R]
+int measure_now(rfim_pt* h, std::vector<long long>& terms, std::vector<int32_t>& t2r) {
+    const size_t DR = (size_t)h->D * h->R;
+    CU(cudaMemsetAsync(h->v.acc, 0, DR * 3 * 8, h->stream));
+    int rc = launch_reduce(h);
+    if (rc) return rc;
+    std::vector<long long> acc(DR * 3);
+    t2r.assign(DR, -1);
+    CU(cudaMemcpyAsync(acc.data(), h->v.acc, DR * 3 * 8, cudaMemcpyDeviceToHost, h->stream));
+    CU(cudaMemcpyAsync(t2r.data(), h->v.t2r, DR * 4, cudaMemcpyDeviceToHost, h->stream));
+    CU(cudaMemsetAsync(h->v.acc, 0, DR * 3 * 8, h->stream));
+    CU(cudaStreamSynchronize(h->stream));
+    terms.assign((size_t)h->D * h->n * 3, 0);
+    for (int d = 0; d < h->D; ++d)
+        for (int t = 0; t < h->n; ++t) {
+            const int slot = t2r[(size_t)d * h->R + t];
+            for (int q = 0; q < 3; ++q) terms[((size_t)d * h->n + t) * 3 + q] = acc[((size_t)d * h->R + slot) * 3 + q];
+        }
+    return RFIM_OK;
+}
+
+int check_member(rfim_pt* h, int d) {
+    if (!h) return RFIM_EINVAL;
+    if (d < 0 || d >= h->D) return fail(h, RFIM_EINVAL, "member index out of range");
+    return RFIM_OK;
+}
+
+int create_impl(rfim_pt** out, int L, int R, double J, double hh, int kind, int D, const uint64_t* seeds) {
+    if (!out) return RFIM_EINVAL;
+    *out = nullptr;
+    if (L < 2 || (L & 1) || L > 1024 || R < 1 || R > 4096 || D < 1 || D > 4096 || !seeds) return RFIM_EINVAL;
+    if (kind != RFIM_FIELD_BIMODAL && kind != RFIM_FIELD_GAUSSIAN) return RFIM_EINVAL;
+    if (!std::isfinite(J) || !std::isfinite(hh)) return RFIM_EINVAL;
+    int ndev = 0;
+    if (cudaGetDeviceCount(&ndev) != cudaSuccess || ndev < 1) return RFIM_ECUDA;   // no CPU fallback
+    rfim_pt* h = new rfim_pt();
+    h->L = L; h->R = R; h->D = D; h->kind = kind; h->J = J; h->h = hh;
+    h->N = (long long)L * L * L; h->Nh = h->N / 2;
+    h->seeds.assign(seeds, seeds + D);
+    h->field_nat.assign((size_t)D * h->N, 0);
+    h->amax.assign(D, 0.0);
+    h->T.assign((size_t)D * R, 0.0);
+    View& v = h->v;
+    v.L = L; v.Lh = L / 2; v.R = R; v.n = 0; v.D = D; v.kind = kind;
+    v.W = (L % 8 == 0) ? L / 8 : 0;
+    v.N = h->N; v.Nh = h->Nh;
+    v.J = J; v.hs = (kind == RFIM_FIELD_BIMODAL) ? hh : hh / kFieldScale;
+    const size_t DR = (size_t)D * R;
+    int rc = RFIM_OK;
+    auto A = [&](int r) { if (rc == RFIM_OK) rc = r; };
+    A(alloc_into(h, &v.spins, DR * (size_t)h->N));
+    if (kind == RFIM_FIELD_BIMODAL) {
+        A(alloc_into(h, const_cast<uint8_t**>(&v.fieldb), (size_t)D * h->N));
+        A(alloc_into(h, const_cast<uint32_t**>(&v.etab), DR * 32));
+        A(alloc_into(h, const_cast<uint32_t**>(&v.never), DR));
+    } else {
+        A(alloc_into(h, const_cast<float**>(&v.fielda), (size_t)D * h->N));
+        A(alloc_into(h, const_cast<int32_t**>(&v.fieldg), (size_t)D * h->N));
+        A(alloc_into(h, const_cast<GaussEntry**>(&v.gtab), DR * 16));
+        A(alloc_into(h, const_cast<float**>(&v.band), DR));
+    }
+    A(alloc_into(h, const_cast<double**>(&v.beta), DR));
+    A(alloc_into(h, &v.t2r, DR));
+    A(alloc_into(h, &v.r2t, DR));
+    A(alloc_into(h, const_cast<uint32_t**>(&v.keys), (size_t)D * 2));
+    A(alloc_into(h, &v.acc, DR * 3));
+    A(alloc_into(h, &v.ework, DR));
+    A(alloc_into(h, &v.att, DR));
+    A(alloc_into(h, &v.accn, DR));
+    A(alloc_into(h, &v.diag, 4));
+    if (rc != RFIM_OK) { rfim_pt_destroy(h); return rc; }
+    auto body = [&]() -> int {
+        std::vector<uint32_t> keys((size_t)D * 2);
+        for (int d = 0; d < D; ++d) { keys[2 * d] = (uint32_t)(seeds[d] & 0xFFFFFFFFull); keys[2 * d + 1] = (uint32_t)(seeds[d] >> 32); }
+        CU(cudaMemcpyAsync(const_cast<uint32_t*>(v.keys), keys.data(), keys.size() * 4, cudaMemcpyHostToDevice, h->stream));
+        CU(cudaMemsetAsync(v.diag, 0, 32, h->stream));
+        CU(cudaMemsetAsync(v.t2r, 0xFF, DR * 4, h->stream));
+        CU(cudaMemsetAsync(v.r2t, 0xFF, DR * 4, h->stream));
+        CU(cudaStreamSynchronize(h->stream));
+        int r2 = reset_statistics(h);
+        if (r2) return r2;
+        for (int d = 0; d < D; ++d) {
+            generate_field_host(h, d);
+            if ((r2 = upload_field(h, d))) return r2;
+        }
+        k_init_spins<<<grid_for(h->N, D * R), 256, 0, h->stream>>>(v);
+        h->launches += 1;
+        CU(cudaGetLastError());
+        CU(cudaStreamSynchronize(h->stream));
+        return RFIM_OK;
+    };
+    rc = body();
+    if (rc != RFIM_OK) { rfim_pt_destroy(h); return rc; }
+    *out = h;
+    return RFIM_OK;
+}
+
+// DESIGN.md S8: given the trial's rates, produce the new ladder for one member.
+// Returns new temperatures, for each new rank the old rank it keeps the slot of (-1 = new replica),
+// and for new replicas the old rank whose spins they copy.
+struct AdaptPlan {
+    std::vector<double> T;
+    std::vector<int> keep_of;     // per new rank: old rank whose slot is kept, or -1
+    std::vector<int> copy_of;     // per new rank: old rank copied (only where keep_of == -1)
+};
+
+AdaptPlan plan_adaptation(const std::vector<double>& T, const std::vector<double>& rate, int n, int R, int a_req) {
+    AdaptPlan p;
+    std::vector<int> order(n - 1);
+    for (int t = 0; t < n - 1; ++t) order[t] = t;
+    std::stable_sort(order.begin(), order.end(), [&](int x, int y) { return rate[x] < rate[y]; });
+    std::vector<char> split(std::max(n - 1, 0), 0), removed(n, 0);
+    if (n < R) {
+        const int a = std::min(std::min(a_req, R - n), n - 1);
+        for (int q = 0; q < a; ++q) split[order[q]] = 1;
+    } else {
+        const int a = std::min(a_req, n - 1);
+        std::vector<char> inS(std::max(n - 1, 0), 0);
+        for (int q = 0; q < a; ++q) inS[order[q]] = 1;
+        const double rho = a > 0 ? rate[order[a - 1]] : 0.0;
+        auto merged = [&](int u) { const double r1 = rate[u - 1], r2 = rate[u]; return (r1 * r2) * std::min(r1, r2); };
+        std::vector<int> cand;
+        for (int u = 1; u <= n - 2; ++u)
+            if (!inS[u - 1] && !inS[u] && merged(u) > rho) cand.push_back(u);
+        std::stable_sort(cand.begin(), cand.end(), [&](int x, int y) {
+            if (merged(x) != merged(y)) return merged(x) > merged(y);
+            return x > y;
+        });
+        int n_removed = 0;
+        for (int u : cand) {
+            if (n_removed == a) break;
+            if (removed[u - 1] || removed[u + 1]) continue;
+            removed[u] = 1;
+            n_removed += 1;
+        }
+        for (int q = 0; q < n_removed; ++q) split[order[q]] = 1;
+    }
+    for (int t = 0; t < n; ++t) {
+        if (!removed[t]) { p.T.push_back(T[t]); p.keep_of.push_back(t); p.copy_of.push_back(-1); }
+        if (t < n - 1 && split[t]) { p.T.push_back((T[t] + T[t + 1]) / 2.0); p.keep_of.push_back(-1); p.copy_of.push_back(t); }
+    }
+    return p;
+}
+
+}  // namespace
+
+// =================================================================================================
+extern "C" {
+
+int rfim_pt_set_allocator(rfim_pt_alloc_fn alloc, rfim_pt_free_fn release_fn) {
+    if ((alloc == nullptr) != (release_fn == nullptr)) return RFIM_EINVAL;
+    g_alloc = alloc; g_free = release_fn;
+    return RFIM_OK;
+}
+
+int rfim_pt_create(rfim_pt** out, int L, int R, double J, double hh, int field_kind, uint64_t seed) {
+    return create_impl(out, L, R, J, hh, field_kind, 1, &seed);
+}
+
+int rfim_pt_create_batch(rfim_pt** out, int L, int R, double J, double hh, int field_kind, int D, const uint64_t* seeds) {
+    return create_impl(out, L, R, J, hh, field_kind, D, seeds);
+}
+
+int rfim_pt_destroy(rfim_pt* h) {
+    if (!h) return RFIM_OK;
+    cudaStreamSynchronize(h->stream);
+    for (void* p : h->owned) dev_free(p);
+    delete h;
+    return RFIM_OK;
+}
+
+const char* rfim_pt_last_error(rfim_pt* h) { return h ? h->err.c_str() : "null handle"; }
+
+int rfim_pt_set_stream(rfim_pt* h, void* s) {
+    if (!h) return RFIM_EINVAL;
+    CU(cudaStreamSynchronize(h->stream));
+    h->stream = reinterpret_cast<cudaStream_t>(s);
+    return RFIM_OK;
+}
+
+int rfim_pt_synchronize(rfim_pt* h) {
+    if (!h) return RFIM_EINVAL;
+    CU(cudaStreamSynchronize(h->stream));
+    return RFIM_OK;
+}
+
+int rfim_pt_set_packing(rfim_pt* h, int bits) {
+    if (!h) return RFIM_EINVAL;
+    if (bits == 8) { h->packing = 8; return RFIM_OK; }
+    return fail(h, RFIM_EINVAL, "packing must be 8 (bit-packed storage is not built yet)");
+}
+
+int rfim_pt_set_kernel_variant(rfim_pt* h, int variant) {
+    if (!h) return RFIM_EINVAL;
+    if (variant < 0 || variant > 2) return fail(h, RFIM_EINVAL, "unknown kernel variant");
+    if (variant == 2 && h->v.W == 0) return fail(h, RFIM_EINVAL, "word kernel needs L % 8 == 0");
+    h->variant = variant;
+    return RFIM_OK;
+}
+
+int rfim_pt_set_adapt_params(rfim_pt* h, int exchange_every, int insertions) {
+    if (!h) return RFIM_EINVAL;
+    if (exchange_every < 1 || insertions < 1) return fail(h, RFIM_EINVAL, "adapt parameters must be >= 1");
+    h->adapt_k = exchange_every; h->adapt_a = insertions;
+    return RFIM_OK;
+}
+
+int rfim_pt_set_temperatures(rfim_pt* h, const double* T, int n) {
+    if (!h) return RFIM_EINVAL;
+    if (!T || n < 1 || n > h->R) return fail(h, RFIM_EINVAL, "need 1 <= n <= R temperatures");
+    for (int t = 0; t < n; ++t) {
+        if (!(T[t] > 0.0) || !std::isfinite(T[t])) return fail(h, RFIM_EINVAL, "temperatures must be positive and finite");
+        if (t > 0 && !(T[t] > T[t - 1])) return fail(h, RFIM_EINVAL, "temperatures must be strictly ascending");
+    }
+    h->n = n; h->v.n = n;
+    std::vector<int32_t> t2r((size_t)h->D * h->R, -1);
+    for (int d = 0; d < h->D; ++d)
+        for (int t = 0; t < n; ++t) { h->T[(size_t)d * h->R + t] = T[t]; t2r[(size_t)d * h->R + t] = t; }
+    int rc;
+    if ((rc = upload_permutation(h, t2r))) return rc;
+    if ((rc = upload_tables(h))) return rc;
+    if ((rc = reset_statistics(h))) return rc;
+    h->have_T = true;
+    return RFIM_OK;
+}
+
+int rfim_pt_sweep(rfim_pt* h, int64_t n_sweeps, int exchange_every) {
+    if (!h) return RFIM_EINVAL;
+    return do_sweeps(h, n_sweeps, exchange_every);
+}
+
+int rfim_pt_adapt_temperatures(rfim_pt* h, int64_t trial_sweeps) {
+    if (!h) return RFIM_EINVAL;
+    if (!h->have_T) return fail(h, RFIM_ESTATE, "temperatures not set");
+    if (trial_sweeps < 0) return fail(h, RFIM_EINVAL, "negative argument");
+    int rc;
+    if ((rc = reset_statistics(h))) return rc;
+    if ((rc = do_sweeps(h, trial_sweeps, h->adapt_k))) return rc;
+    const int D = h->D, R = h->R, n = h->n;
+    const size_t DR = (size_t)D * R;
+    std::vector<unsigned long long> att(DR), acc(DR);
+    std::vector<int32_t> t2r(DR);
+    CU(cudaMemcpyAsync(att.data(), h->v.att, DR * 8, cudaMemcpyDeviceToHost, h->stream));
+    CU(cudaMemcpyAsync(acc.data(), h->v.accn, DR * 8, cudaMemcpyDeviceToHost, h->stream));
+    CU(cudaMemcpyAsync(t2r.data(), h->v.t2r, DR * 4, cudaMemcpyDeviceToHost, h->stream));
+    CU(cudaStreamSynchronize(h->stream));
+    std::vector<AdaptPlan> plans(D);
+    for (int d = 0; d < D; ++d) {
+        std::vector<double> Td(h->T.begin() + (size_t)d * R, h->T.begin() + (size_t)d * R + n), rate(std::max(n - 1, 0));
+        for (int t = 0; t < n - 1; ++t) {
+            if (att[(size_t)d * R + t] == 0) return fail(h, RFIM_ESTATE, "a pair saw no exchange attempt in the trial");
+            rate[t] = (double)acc[(size_t)d * R + t] / (double)att[(size_t)d * R + t];
+        }
+        plans[d] = plan_adaptation(Td, rate, n, R, h->adapt_a);
+        if (plans[d].T.size() != plans[0].T.size()) return fail(h, RFIM_ESTATE, "members disagree on the new replica count");
+    }
+    const int n_new = (int)plans[0].T.size();
+    std::vector<int32_t> new_t2r(DR, -1);
+    for (int d = 0; d < D; ++d) {
+        int next_slot = n;                         // pool slots n..R-1
+        for (int j = 0; j < n_new; ++j) {
+            const AdaptPlan& p = plans[d];
+            int slot;
+            if (n_new == n) {
+                slot = t2r[(size_t)d * R + j];     // fixed count: the slot at rank j keeps rank j
+            } else if (p.keep_of[j] >= 0) {
+                slot = t2r[(size_t)d * R + p.keep_of[j]];
+            } else {
+                slot = next_slot++;
+                const int src = t2r[(size_t)d * R + p.copy_of[j]];
+                CU(cudaMemcpyAsync(h->v.spins + ((size_t)d * R + slot) * h->N, h->v.spins + ((size_t)d * R + src) * h->N,
+                                   (size_t)h->N, cudaMemcpyDeviceToDevice, h->stream));
+            }
+            new_t2r[(size_t)d * R + j] = slot;
+            h->T[(size_t)d * R + j] = p.T[j];
+        }
+    }
+    h->n = n_new; h->v.n = n_new;
+    if ((rc = upload_permutation(h, new_t2r))) return rc;
+    if ((rc = upload_tables(h))) return rc;
+    if ((rc = reset_statistics(h))) return rc;
+    CU(cudaStreamSynchronize(h->stream));
+    return RFIM_OK;
+}
+
+int rfim_pt_observables(rfim_pt* h, double* E, double* M, double* rate) {
+    if (!h) return RFIM_EINVAL;
+    if (!h->have_T) return fail(h, RFIM_ESTATE, "temperatures not set");
+    std::vector<long long> terms; std::vector<int32_t> t2r;
+    int rc = measure_now(h, terms, t2r);
+    if (rc) return rc;
+    const int D = h->D, n = h->n, R = h->R;
+    for (int d = 0; d < D; ++d)
+        for (int t = 0; t < n; ++t) {
+            const long long* q = &terms[((size_t)d * n + t) * 3];
+            if (E) E[(size_t)d * n + t] = (-h->J * (double)q[0]) - (h->v.hs * (double)q[1]);
+            if (M) M[(size_t)d * n + t] = (double)q[2] / (double)h->N;
+        }
+    if (rate) {
+        const size_t DR = (size_t)D * R;
+        std::vector<unsigned long long> att(DR), acc(DR);
+        CU(cudaMemcpyAsync(att.data(), h->v.att, DR * 8, cudaMemcpyDeviceToHost, h->stream));
+        CU(cudaMemcpyAsync(acc.data(), h->v.accn, DR * 8, cudaMemcpyDeviceToHost, h->stream));
+        CU(cudaStreamSynchronize(h->stream));
+        for (int d = 0; d < D; ++d)
+            for (int t = 0; t < n - 1; ++t)
+                rate[(size_t)d * (n - 1) + t] = att[(size_t)d * R + t] ? (double)acc[(size_t)d * R + t] / (double)att[(size_t)d * R + t] : -1.0;
+    }
+    return RFIM_OK;
+}
+
+int rfim_pt_get_info(rfim_pt* h, int* L, int* R, int* n, int* D, int* kind) {
+    if (!h) return RFIM_EINVAL;
+    if (L) *L = h->L; if (R) *R = h->R; if (n) *n = h->n; if (D) *D = h->D; if (kind) *kind = h->kind;
+    return RFIM_OK;
+}
+
+int rfim_pt_get_spins_slot(rfim_pt* h, int d, int slot, int8_t* out) {
+    int rc = check_member(h, d);
+    if (rc) return rc;
+    if (slot < 0 || slot >= h->R || !out) return fail(h, RFIM_EINVAL, "bad slot or null buffer");
+    if ((rc = ensure_stage(h, (size_t)h->N))) return rc;
+    k_export_spins<<<grid_for(h->N, 1), 256, 0, h->stream>>>(h->v, d * h->R + slot, h->stage);
+    h->launches += 1;
+    CU(cudaGetLastError());
+    CU(cudaMemcpyAsync(out, h->stage, (size_t)h->N, cudaMemcpyDeviceToHost, h->stream));
+    CU(cudaStreamSynchronize(h->stream));
+    return RFIM_OK;
+}
+
+int rfim_pt_get_spins_member(rfim_pt* h, int d, int temp_rank, int8_t* out) {
+    int rc = check_member(h, d);
+    if (rc) return rc;
+    if (!h->have_T) return fail(h, RFIM_ESTATE, "temperatures not set");
+    if (temp_rank < 0 || temp_rank >= h->n) return fail(h, RFIM_EINVAL, "temperature rank out of range");
+    int32_t slot = -1;
+    CU(cudaMemcpyAsync(&slot, h->v.t2r + (size_t)d * h->R + temp_rank, 4, cudaMemcpyDeviceToHost, h->stream));
+    CU(cudaStreamSynchronize(h->stream));
+    return rfim_pt_get_spins_slot(h, d, slot, out);
+}
+
+int rfim_pt_get_spins(rfim_pt* h, int temp_rank, int8_t* out) { return rfim_pt_get_spins_member(h, 0, temp_rank, out); }
+
+int rfim_pt_set_spins_slot(rfim_pt* h, int d, int slot, const int8_t* in) {
+    int rc = check_member(h, d);
+    if (rc) return rc;
+    if (slot < 0 || slot >= h->R || !in) return fail(h, RFIM_EINVAL, "bad slot or null buffer");
+    for (long long i = 0; i < h->N; ++i)
+        if (in[i] != 1 && in[i] != -1) return fail(h, RFIM_EINVAL, "spins must be +1 or -1");
+    if ((rc = ensure_stage(h, (size_t)h->N))) return rc;
+    CU(cudaMemcpyAsync(h->stage, in, (size_t)h->N, cudaMemcpyHostToDevice, h->stream));
+    k_import_spins<<<grid_for(h->N, 1), 256, 0, h->stream>>>(h->v, d * h->R + slot, h->stage);
+    h->launches += 1;
+    CU(cudaGetLastError());
+    CU(cudaStreamSynchronize(h->stream));
+    return RFIM_OK;
+}
+
+int rfim_pt_get_spins_all(rfim_pt* h, int8_t* out) {
+    if (!h || !out) return RFIM_EINVAL;
+    const int DR = h->D * h->R;
+    int rc = ensure_stage(h, (size_t)DR * h->N);
+    if (rc) return rc;
+    k_export_spins<<<grid_for(h->N, DR), 256, 0, h->stream>>>(h->v, 0, h->stage);
+    h->launches += 1;
+    CU(cudaGetLastError());
+    CU(cudaMemcpyAsync(out, h->stage, (size_t)DR * h->N, cudaMemcpyDeviceToHost, h->stream));
+    CU(cudaStreamSynchronize(h->stream));
+    return RFIM_OK;
+}
+
+int rfim_pt_set_spins_all(rfim_pt* h, const int8_t* in) {
+    if (!h || !in) return RFIM_EINVAL;
+    const int DR = h->D * h->R;
+    int rc = ensure_stage(h, (size_t)DR * h->N);
+    if (rc) return rc;
+    CU(cudaMemcpyAsync(h->stage, in, (size_t)DR * h->N, cudaMemcpyHostToDevice, h->stream));
+    k_import_spins<<<grid_for(h->N, DR), 256, 0, h->stream>>>(h->v, 0, h->stage);
+    h->launches += 1;
+    CU(cudaGetLastError());
+    return RFIM_OK;
+}
+
+int rfim_pt_get_field(rfim_pt* h, int d, int32_t* out) {
+    int rc = check_member(h, d);
+    if (rc) return rc;
+    if (!out) return fail(h, RFIM_EINVAL, "null buffer");
+    std::memcpy(out, h->field_nat.data() + (size_t)d * h->N, (size_t)h->N * 4);
+    return RFIM_OK;
+}
+
+int rfim_pt_set_field(rfim_pt* h, int d, const int32_t* in) {
+    int rc = check_member(h, d);
+    if (rc) return rc;
+    if (!in) return fail(h, RFIM_EINVAL, "null buffer");
+    for (long long i = 0; i < h->N; ++i) {
+        if (h->kind == RFIM_FIELD_BIMODAL) { if (in[i] != 1 && in[i] != -1) return fail(h, RFIM_EINVAL, "bimodal field must be +-1"); }
+        else if (in[i] > kFieldClamp || in[i] < -kFieldClamp) return fail(h, RFIM_EINVAL, "Gaussian field out of range");
+    }
+    CU(cudaStreamSynchronize(h->stream));
+    std::memcpy(h->field_nat.data() + (size_t)d * h->N, in, (size_t)h->N * 4);
+    if ((rc = upload_field(h, d))) return rc;
+    if (h->have_T && (rc = upload_tables(h))) return rc;     // the guard band depends on max |a_i|
+    return RFIM_OK;
+}
+
+int rfim_pt_get_permutation(rfim_pt* h, int d, int32_t* t2r) {
+    int rc = check_member(h, d);
+    if (rc) return rc;
+    if (!t2r) return fail(h, RFIM_EINVAL, "null buffer");
+    CU(cudaMemcpyAsync(t2r, h->v.t2r + (size_t)d * h->R, (size_t)h->n * 4, cudaMemcpyDeviceToHost, h->stream));
+    CU(cudaStreamSynchronize(h->stream));
+    return RFIM_OK;
+}
+
+int rfim_pt_set_permutation(rfim_pt* h, int d, const int32_t* t2r_in) {
+    int rc = check_member(h, d);
+    if (rc) return rc;
+    if (!t2r_in || !h->have_T) return fail(h, RFIM_EINVAL, "null buffer or temperatures not set");
+    const size_t DR = (size_t)h->D * h->R;
+    std::vector<int32_t> t2r(DR);
+    CU(cudaMemcpyAsync(t2r.data(), h->v.t2r, DR * 4, cudaMemcpyDeviceToHost, h->stream));
+    CU(cudaStreamSynchronize(h->stream));
+    std::vector<char> seen(h->R, 0);
+    for (int t = 0; t < h->n; ++t) {
+        const int s = t2r_in[t];
+        if (s < 0 || s >= h->R || seen[s]) return fail(h, RFIM_EINVAL, "not a permutation of slots");
+        seen[s] = 1;
+        t2r[(size_t)d * h->R + t] = s;
+    }
+    return upload_permutation(h, t2r);
+}
+
+int rfim_pt_get_temperatures(rfim_pt* h, int d, double* T, int* n) {
+    int rc = check_member(h, d);
+    if (rc) return rc;
+    if (n) *n = h->n;
+    if (T) for (int t = 0; t < h->n; ++t) T[t] = h->T[(size_t)d * h->R + t];
+    return RFIM_OK;
+}
+
+int rfim_pt_get_counters(rfim_pt* h, uint64_t* sweep_index, uint64_t* exchange_step) {
+    if (!h) return RFIM_EINVAL;
+    if (sweep_index) *sweep_index = h->sweep_g;
+    if (exchange_step) *exchange_step = h->xstep;
+    return RFIM_OK;
+}
+
+int rfim_pt_set_counters(rfim_pt* h, uint64_t sweep_index, uint64_t exchange_step) {
+    if (!h) return RFIM_EINVAL;
+    h->sweep_g = sweep_index; h->xstep = exchange_step;
+    return RFIM_OK;
+}
+
+int rfim_pt_get_energy_terms(rfim_pt* h, int d, int64_t* Eb, int64_t* Ef, int64_t* Msum) {
+    int rc = check_member(h, d);
+    if (rc) return rc;
+    if (!h->have_T) return fail(h, RFIM_ESTATE, "temperatures not set");
+    std::vector<long long> terms; std::vector<int32_t> t2r;
+    if ((rc = measure_now(h, terms, t2r))) return rc;
+    for (int t = 0; t < h->n; ++t) {
+        const long long* q = &terms[((size_t)d * h->n + t) * 3];
+        if (Eb) Eb[t] = q[0]; if (Ef) Ef[t] = q[1]; if (Msum) Msum[t] = q[2];
+    }
+    return RFIM_OK;
+}
+
+int64_t rfim_pt_timeseries_steps(rfim_pt* h) { return h ? h->series_steps : 0; }
+
+int rfim_pt_get_timeseries(rfim_pt* h, int d, int64_t* Eb, int64_t* Ef, int64_t* Msum) {
+    int rc = check_member(h, d);
+    if (rc) return rc;
+    const long long steps = h->series_steps;
+    if (steps == 0) return RFIM_OK;
+    const size_t row = (size_t)h->D * h->R * 3;
+    std::vector<long long> buf((size_t)steps * row);
+    CU(cudaMemcpyAsync(buf.data(), h->v.series, buf.size() * 8, cudaMemcpyDeviceToHost, h->stream));
+    CU(cudaStreamSynchronize(h->stream));
+    for (long long s = 0; s < steps; ++s)
+        for (int t = 0; t < h->n; ++t) {
+            const long long* q = &buf[(size_t)s * row + ((size_t)d * h->R + t) * 3];
+            if (Eb) Eb[s * h->n + t] = q[0]; if (Ef) Ef[s * h->n + t] = q[1]; if (Msum) Msum[s * h->n + t] = q[2];
+        }
+    return RFIM_OK;
+}
+
+int rfim_pt_get_exchange_counts(rfim_pt* h, int d, uint64_t* attempted, uint64_t* accepted) {
+    int rc = check_member(h, d);
+    if (rc) return rc;
+    const int m = std::max(h->n - 1, 0);
+    if (attempted) CU(cudaMemcpyAsync(attempted, h->v.att + (size_t)d * h->R, (size_t)m * 8, cudaMemcpyDeviceToHost, h->stream));
+    if (accepted) CU(cudaMemcpyAsync(accepted, h->v.accn + (size_t)d * h->R, (size_t)m * 8, cudaMemcpyDeviceToHost, h->stream));
+    CU(cudaStreamSynchronize(h->stream));
+    return RFIM_OK;
+}
+
+int rfim_pt_get_bimodal_threshold(rfim_pt* h, int d, int rank, int k, int b, uint64_t* thr) {
+    int rc = check_member(h, d);
+    if (rc) return rc;
+    if (h->kind != RFIM_FIELD_BIMODAL || !h->have_T || rank < 0 || rank >= h->n || k < 0 || k > 6 || b < 0 || b > 1 || !thr)
+        return fail(h, RFIM_EINVAL, "bad threshold query");
+    // device index for s = +1: n1 = k, hb = b (s = +1 so b = hb)
+    const int idx = k | (1 << 3) | (b << 4);
+    uint32_t e = 0, nv = 0;
+    CU(cudaMemcpyAsync(&e, h->v.etab + ((size_t)d * h->R + rank) * 32 + idx, 4, cudaMemcpyDeviceToHost, h->stream));
+    CU(cudaMemcpyAsync(&nv, h->v.never + (size_t)d * h->R + rank, 4, cudaMemcpyDeviceToHost, h->stream));
+    CU(cudaStreamSynchronize(h->stream));
+    *thr = ((nv >> idx) & 1u) ? 0ull : (uint64_t)e + 1ull;
+    return RFIM_OK;
+}
+
+int rfim_pt_get_diagnostics(rfim_pt* h, uint64_t diag[4]) {
+    if (!h || !diag) return RFIM_EINVAL;
+    unsigned long long d4[4];
+    CU(cudaMemcpyAsync(d4, h->v.diag, 32, cudaMemcpyDeviceToHost, h->stream));
+    CU(cudaStreamSynchronize(h->stream));
+    diag[0] = h->launches; diag[1] = d4[1]; diag[2] = d4[2]; diag[3] = d4[3];
+    return RFIM_OK;
+}
+
+}  // extern "C"
+
+// ---- roofline microbenchmarks ---------------------------------------------------------------------
+namespace {
+
+__global__ void k_bench_philox(uint32_t* out, int calls, uint32_t sweep, uint32_t slot) {
+    uint32_t acc = 0, c0 = blockIdx.x * blockDim.x + threadIdx.x;
+    for (int i = 0; i < calls; ++i) {
+        const Words4 w = philox4x32_10(0x9E3779B9u, 0x1234567u, c0, sweep, slot, kDomColour0);
+        acc ^= w.w0 ^ w.w1 ^ w.w2 ^ w.w3;
+        c0 += gridDim.x * blockDim.x;
+    }
+    out[blockIdx.x * blockDim.x + threadIdx.x] = acc;
+}
+
+__global__ void k_bench_stream(uint4* p, size_t n16) {
+    const size_t stride = (size_t)gridDim.x * blockDim.x;
+    for (size_t i = (size_t)blockIdx.x * blockDim.x + threadIdx.x; i < n16; i += stride) {
+        uint4 q = p[i];
+        q.x ^= 0x01010101u; q.y ^= 0x01010101u; q.z ^= 0x01010101u; q.w ^= 0x01010101u;
+        p[i] = q;
+    }
+}
+
+template <class F>
+int time_launch(cudaStream_t s, F launch, double* ms) {
+    cudaEvent_t a, b;
+    if (cudaEventCreate(&a) != cudaSuccess || cudaEventCreate(&b) != cudaSuccess) return RFIM_ECUDA;
+    launch();                                   // warm-up
+    float best = 1e30f;
+    for (int rep = 0; rep < 5; ++rep) {
+        cudaEventRecord(a, s);
+        launch();
+        cudaEventRecord(b, s);
+        if (cudaEventSynchronize(b) != cudaSuccess) { cudaEventDestroy(a); cudaEventDestroy(b); return RFIM_ECUDA; }
+        float t = 0.f;
+        cudaEventElapsedTime(&t, a, b);
+        best = std::min(best, t);
+    }
+    cudaEventDestroy(a); cudaEventDestroy(b);
+    *ms = best;
+    return cudaGetLastError() == cudaSuccess ? RFIM_OK : RFIM_ECUDA;
+}
+
+}  // namespace
+
+extern "C" {
+
+int rfim_pt_bench_philox(void* stream, int calls_per_thread, double* ms, double* attempts) {
+    if (calls_per_thread < 1 || !ms || !attempts) return RFIM_EINVAL;
+    cudaStream_t s = reinterpret_cast<cudaStream_t>(stream);
+    int dev = 0, sms = 0;
+    if (cudaGetDevice(&dev) != cudaSuccess) return RFIM_ECUDA;
+    cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev);
+    const int blocks = sms * 8, threads = 256;
+    uint32_t* out = reinterpret_cast<uint32_t*>(dev_alloc((size_t)blocks * threads * 4));
+    if (!out) return RFIM_ENOMEM;
+    int rc = time_launch(s, [&] { k_bench_philox<<<blocks, threads, 0, s>>>(out, calls_per_thread, 7u, 3u); }, ms);
+    dev_free(out);
+    *attempts = 4.0 * (double)blocks * threads * calls_per_thread;
+    return rc;
+}
+
+int rfim_pt_bench_stream(void* stream, size_t bytes, double* ms, double* bytes_moved) {
+    if (bytes < 16 || !ms || !bytes_moved) return RFIM_EINVAL;
+    cudaStream_t s = reinterpret_cast<cudaStream_t>(stream);
+    int dev = 0, sms = 0;
+    if (cudaGetDevice(&dev) != cudaSuccess) return RFIM_ECUDA;
+    cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev);
+    uint4* p = reinterpret_cast<uint4*>(dev_alloc(bytes));
+    if (!p) return RFIM_ENOMEM;
+    cudaMemsetAsync(p, 0, bytes, s);
+    const size_t n16 = bytes / 16;
+    int rc = time_launch(s, [&] { k_bench_stream<<<sms * 8, 512, 0, s>>>(p, n16); }, ms);
+    dev_free(p);
+    *bytes_moved = 2.0 * (double)n16 * 16.0;
+    return rc;
+}
+
+}  // extern "C"
