@@ -1,0 +1,290 @@
+#!/usr/bin/env python
+"""bench.py -- spin-flip attempts/ns of the whole PT hot path on BASELINE.json's config 4
+(L=64, R=128, Gaussian field h=2.0, geometric T in [0.8, 6.0], exchange every 10, seed 4).
+
+One "step" = one parallel-tempering move: exchange_every (=10) checkerboard Metropolis
+sweeps of all 128 replicas + the per-replica energy reduction + one exchange step.
+
+  python bench.py [--gpus N] [--steps K] [--warmup W] [--impl ours|reference] [--workload cfg4]
+
+N > 1 (torchrun, one rank per GPU): every rank runs its own disorder realisation of the same
+workload (seed 4 + rank) -- independent problems, no data-path collective, "scaling": "weak".
+Prints ONE JSON line on rank 0.
+"""
+import argparse
+import json
+import os
+import subprocess
+import sys
+import threading
+import time
+
+ROOT = os.path.dirname(os.path.abspath(__file__))
+if ROOT not in sys.path:
+    sys.path.insert(0, ROOT)
+
+METRIC = "spin-flip attempts/ns (all replicas) at L=64,R=128; % of sweep roofline"
+UNIT = "attempts/ns"
+
+
+def parse():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=200)
+    ap.add_argument("--warmup", type=int, default=20)
+    ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
+    ap.add_argument("--workload", default="cfg4")
+    ap.add_argument("--variant", type=int, default=0, help="kernel variant (0 = automatic)")
+    ap.add_argument("--packing", type=int, default=8)
+    ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--no-e2e", action="store_true")
+    return ap.parse_args()
+
+
+class ClockSampler:
+    """nvidia-smi clocks / throttle reasons sampled during the timed region (B200_PROFILING.md)."""
+    Q = ("clocks.sm,clocks.max.sm,power.draw,clocks_event_reasons.hw_slowdown,clocks_event_reasons.hw_thermal_slowdown,"
+         "clocks_event_reasons.sw_thermal_slowdown,clocks_event_reasons.sw_power_cap")
+
+    def __init__(self, index):
+        self.index, self.rows, self.proc = index, [], None
+
+    def start(self):
+        try:
+            self.proc = subprocess.Popen(["nvidia-smi", "-i", str(self.index), "--query-gpu=" + self.Q,
+                                          "--format=csv,noheader,nounits", "-lms", "100"],
+                                         stdout=subprocess.PIPE, stderr=subprocess.DEVNULL, text=True)
+            self.thread = threading.Thread(target=self._read, daemon=True)
+            self.thread.start()
+        except Exception:
+            self.proc = None
+
+    def _read(self):
+        for line in self.proc.stdout:
+            self.rows.append([c.strip() for c in line.split(",")])
+
+    def stop(self):
+        if not self.proc:
+            return {"sm_mhz": None, "sm_max_mhz": None, "reasons": ["nvidia-smi unavailable"]}
+        self.proc.terminate()
+        try:
+            self.proc.wait(timeout=2)
+        except Exception:
+            self.proc.kill()
+        sm, mx, reasons, pw = [], [], set(), []
+        names = ["hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown", "sw_power_cap"]
+        for r in self.rows:
+            try:
+                sm.append(float(r[0])); mx.append(float(r[1])); pw.append(float(r[2]))
+                for nm, val in zip(names, r[3:7]):
+                    if val.lower().startswith("active"):
+                        reasons.add(nm)
+            except Exception:
+                pass
+        sm.sort()
+        return {"sm_mhz": sm[len(sm) // 2] if sm else None, "sm_max_mhz": max(mx) if mx else None,
+                "power_w_max": max(pw) if pw else None, "samples": len(sm), "reasons": sorted(reasons)}
+
+
+def oracle_sample(wl, threads, r_sample, sweeps, steps, warmup, seed):
+    """Time the oracle, as it stands, on a bounded sample of the workload: r_sample replicas spread over
+    the ladder, `sweeps` sweeps + one exchange step per step.  Returns attempts/ns."""
+    import numpy as np
+    import oracle
+    T = wl.temperatures()
+    sel = np.unique(np.round(np.linspace(0, wl.R - 1, r_sample)).astype(int))
+    o = oracle.Oracle(wl.L, len(sel), wl.J, wl.h, wl.field_kind, seed, threads=threads)
+    o.set_temperatures(T[sel])
+    for _ in range(warmup):
+        o.sweep(sweeps, sweeps)
+    t0 = time.perf_counter()
+    for _ in range(steps):
+        o.sweep(sweeps, sweeps)
+    dt = time.perf_counter() - t0
+    attempts = float(wl.N) * len(sel) * sweeps * steps
+    return attempts / dt * 1e-9, dt / max(steps, 1) * 1e3, len(sel)
+
+
+def run_reference(args, wl, rank, world):
+    if rank != 0:
+        return
+    cores = os.cpu_count() or 1
+    # size the per-step sample so that (steps + warmup) steps end within ~2 minutes
+    total_steps = args.steps + args.warmup
+    rate_guess = 0.02e9 * max(1, min(cores, 16)) * 0.6            # attempts/s, from the oracle's measured single-core rate
+    budget_attempts = 100.0 * rate_guess / max(total_steps, 1)
+    sweeps = wl.exchange_every
+    r_sample = int(budget_attempts / (wl.N * sweeps))
+    if r_sample < 2:
+        r_sample = 2
+        sweeps = max(1, int(budget_attempts / (wl.N * 2)))
+        sweeps = min(sweeps, wl.exchange_every)
+    r_sample = min(r_sample, wl.R)
+    threads = max(1, min(cores, r_sample))
+    value, ms_per_step, r_used = oracle_sample(wl, threads, r_sample, sweeps, args.steps, args.warmup, wl.seeds[0])
+    sample = f"{r_used} of {wl.R} replicas (evenly spread over the ladder) x {sweeps} sweeps + 1 exchange step per step, L={wl.L}"
+    line = {"impl": "reference", "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": args.gpus, "steps": args.steps,
+            "warmup": args.warmup, "ms_per_step": ms_per_step, "higher_is_better": True, "scaling": "weak",
+            "vs_baseline": None, "dtype": "u8", "data": "synthetic",
+            "config": {"workload": f"{wl.name}: L={wl.L} R={wl.R} Gaussian h={wl.h} T geometric [{wl.t_min},{wl.t_max}] k={wl.exchange_every}",
+                       "reference": "CPU oracle (oracle/rfim_oracle.cpp) as it stands, bounded sample per step"},
+            "cpu_baseline": {"value": value, "unit": UNIT, "cores": threads, "kind": "oracle", "sample": sample},
+            "e2e": {"value": value, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
+            "gpu_launches": 0}
+    print(json.dumps(line), flush=True)
+
+
+def main():
+    args = parse()
+    from paper_1508_06268_b200 import workloads
+    wl = workloads.CONFIGS[args.workload]
+    rank = int(os.environ.get("RANK", "0"))
+    world = int(os.environ.get("WORLD_SIZE", "1"))
+    local_rank = int(os.environ.get("LOCAL_RANK", "0"))
+    if args.impl == "reference":
+        run_reference(args, wl, rank, world)
+        return
+
+    import numpy as np
+    import torch
+    import torch.distributed as dist
+    from paper_1508_06268_b200 import binding
+
+    if not torch.cuda.is_available():
+        raise SystemExit("bench.py needs a CUDA device: the product has no CPU fallback")
+    torch.cuda.set_device(local_rank)
+    if world > 1:
+        dist.init_process_group("nccl", device_id=torch.device("cuda", local_rank))
+
+    def barrier():
+        if world > 1:
+            dist.barrier()
+        torch.cuda.synchronize()
+
+    k = wl.exchange_every
+    seeds = [s + rank for s in wl.seeds]           # each rank: its own disorder realisation(s)
+    if wl.D == 1:
+        g = binding.RfimPT(wl.L, wl.R, wl.J, wl.h, wl.field_kind, seed=seeds[0])
+    else:
+        g = binding.RfimPT(wl.L, wl.R, wl.J, wl.h, wl.field_kind, seeds=seeds)
+    if args.packing != 8:
+        g.set_packing(args.packing)
+    if args.variant:
+        g.set_kernel_variant(args.variant)
+    g.set_temperatures(wl.temperatures())
+    attempts_per_step = float(wl.N) * wl.R * wl.D * k
+
+    flush = torch.empty(256 << 20, dtype=torch.uint8, device="cuda")   # > 126 MB L2
+
+    def timed_steps(n_steps, exchange_every):
+        """n_steps steps, each bracketed by CUDA events on the launch stream, L2 flushed between steps."""
+        ev = [(torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)) for _ in range(n_steps)]
+        for a, b in ev:
+            flush.zero_()
+            a.record()
+            g.sweep(k, exchange_every)
+            b.record()
+        torch.cuda.synchronize()
+        return [a.elapsed_time(b) for a, b in ev]
+
+    for _ in range(max(args.warmup, 3)):
+        g.sweep(k, k)
+    barrier()
+    sampler = ClockSampler(local_rank)
+    sampler.start()
+    l0 = g.diagnostics()["launches"]
+    barrier()
+    t_wall = time.perf_counter()
+    ms = timed_steps(args.steps, k)
+    barrier()
+    t_wall = time.perf_counter() - t_wall
+    l1 = g.diagnostics()["launches"]
+    # dominant kernel alone (sweeps only, no reduction / exchange), same launch configuration
+    ms_sweep = timed_steps(args.steps, 0)
+    clocks = sampler.stop()
+    total_ms = float(sum(ms))
+    total_ms_sweep = float(sum(ms_sweep))
+    if world > 1:
+        tt = torch.tensor([total_ms, total_ms_sweep], device="cuda", dtype=torch.float64)
+        dist.all_reduce(tt, op=dist.ReduceOp.MAX)
+        total_ms, total_ms_sweep = float(tt[0]), float(tt[1])
+    value = attempts_per_step * args.steps * world / (total_ms * 1e6)
+    sweep_rate = attempts_per_step * args.steps / (total_ms_sweep * 1e6)      # per GPU
+
+    # the two candidate bounds, measured in this run on this GPU (north_star)
+    ph_ms, ph_att = binding.bench_philox(4000, stream=torch.cuda.current_stream().cuda_stream)
+    philox_bound = ph_att / (ph_ms * 1e6)
+    st_ms, st_bytes = binding.bench_stream(1 << 30, stream=torch.cuda.current_stream().cuda_stream)
+    stream_gbs = st_bytes / (st_ms * 1e6)
+    peaks = {}
+    try:
+        peaks = json.load(open(os.path.join(ROOT, "MEASURED_PEAKS.json")))
+    except Exception:
+        pass
+    hbm_peak = float(peaks.get("hbm_gbs", 6650.0))
+    bytes_per_attempt = 2.0 if args.packing == 8 else 0.25
+    hbm_bound = hbm_peak / bytes_per_attempt                                  # attempts/ns if HBM were the limit
+    bound = min(philox_bound, hbm_bound)
+    roofline = {"bound": "alu", "achieved": sweep_rate, "peak": bound, "unit": UNIT, "frac": sweep_rate / bound,
+                "traffic": None,
+                "kernel": "sweep (both colours), timed alone with CUDA events over the same steps",
+                "philox_bound_measured": philox_bound, "hbm_bound": hbm_bound,
+                "hbm_peak_gbs": hbm_peak, "hbm_peak_source": "MEASURED_PEAKS.json" if peaks else "fallback 6650 GB/s",
+                "stream_rmw_gbs_this_run": stream_gbs,
+                "algorithmic_bytes_per_attempt": bytes_per_attempt,
+                "achieved_algorithmic_gbs": sweep_rate * bytes_per_attempt,
+                "whole_step_frac": (value / world) / bound}
+
+    line = {"metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps, "warmup": max(args.warmup, 3),
+            "ms_per_step": total_ms / args.steps, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
+            "dtype": "u8" if args.packing == 8 else "u1", "data": "synthetic",
+            "config": {"workload": f"{wl.name}: L={wl.L} R={wl.R} D={wl.D} {'Gaussian' if wl.field_kind else 'bimodal'} h={wl.h} "
+                                   f"T {wl.ladder} [{wl.t_min},{wl.t_max}] exchange_every={k} seed={wl.seeds[0]}",
+                       "step": f"{k} sweeps + energy reduction + 1 exchange step", "l2": "flushed between steps (256 MiB memset)",
+                       "packing_bits": args.packing, "kernel_variant": args.variant,
+                       "parallelism": "1 GPU" if world == 1 else f"{world} independent realisations, one per GPU"},
+            "clocks": clocks, "gpu_launches": int(l1 - l0), "wall_s_timed_region": t_wall, "roofline": roofline}
+
+    # end to end through the C ABI with HOST buffers: H2D of every lattice, the step, D2H of lattices + observables
+    if not args.no_e2e:
+        n_e2e = max(3, min(args.steps, 20))
+        host = torch.empty((wl.D, wl.R, wl.N), dtype=torch.int8).pin_memory().numpy()
+        g.get_spins_all(out=host)
+        E = None
+        for it in range(2 + n_e2e):
+            if it == 2:
+                barrier()
+                t0 = time.perf_counter()
+            g.set_spins_all(host)
+            g.sweep(k, k)
+            g.get_spins_all(out=host)
+            E, M, _ = g.observables()
+        barrier()
+        dt = time.perf_counter() - t0
+        if world > 1:
+            tt = torch.tensor([dt], device="cuda", dtype=torch.float64)
+            dist.all_reduce(tt, op=dist.ReduceOp.MAX)
+            dt = float(tt[0])
+        obs_bytes = 2 * 8 * wl.D * wl.R
+        line["e2e"] = {"value": attempts_per_step * n_e2e * world / (dt * 1e9), "unit": UNIT,
+                       "h2d_bytes_per_step": int(host.nbytes), "d2h_bytes_per_step": int(host.nbytes + obs_bytes),
+                       "steps": n_e2e, "what": "rfim_pt_set_spins_all(host) + rfim_pt_sweep(k,k) + rfim_pt_get_spins_all(host) + rfim_pt_observables"}
+
+    d = g.diagnostics()
+    line["diagnostics"] = d
+    if rank == 0 and world == 1 and not args.no_cpu_baseline:
+        cores = os.cpu_count() or 1
+        threads = max(1, min(cores, 16))
+        r_s = min(wl.R, 4 * threads)
+        v, ms_b, r_used = oracle_sample(wl, threads, r_s, k, 1, 0, wl.seeds[0])
+        line["cpu_baseline"] = {"value": v, "unit": UNIT, "cores": threads, "kind": "oracle",
+                                "sample": f"{r_used} of {wl.R} replicas x {k} sweeps + 1 exchange step, L={wl.L} ({ms_b / 1e3:.1f} s wall)"}
+    if rank == 0:
+        print(json.dumps(line), flush=True)
+    g.close()
+    if world > 1:
+        dist.destroy_process_group()
+
+
+if __name__ == "__main__":
+    main()
