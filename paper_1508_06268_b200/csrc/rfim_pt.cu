@@ -14,7 +14,9 @@
 
 #include "../../include/rfim_pt.h"
 #include "kernels_ref.cuh"
+#include "launch.h"
 #include "philox.cuh"
+#include "sweep_flow.cuh"
 #include "view.h"
 
 using namespace rfim;
@@ -49,6 +51,10 @@ struct rfim_pt {
     int adapt_k = 10, adapt_a = 4;
     int packing = 8, variant = 0;
     uint64_t launches = 0;
+    uint32_t* flow_prog = nullptr;    // [D][R][32] progress words of the flow kernel
+    uint32_t flow_epoch = 0;
+    int flow_rr = 4;                  // replicas per work item
+    bool has_never = false;           // some reachable bimodal table entry has threshold 0
     std::string err;
 };
 
@@ -172,6 +178,7 @@ int upload_tables(rfim_pt* h) {
     CU(cudaMemcpyAsync(const_cast<double*>(h->v.beta), beta.data(), beta.size() * sizeof(double), cudaMemcpyHostToDevice, h->stream));
     if (h->kind == RFIM_FIELD_BIMODAL) {
         std::vector<uint32_t> etab((size_t)D * R * 32, 0u), never((size_t)D * R, 0u);
+        h->has_never = false;
         for (int d = 0; d < D; ++d)
             for (int t = 0; t < n; ++t) {
                 const double b = beta[(size_t)d * R + t];
@@ -183,7 +190,7 @@ int upload_tables(rfim_pt* h) {
                     const int bb = (s == hb) ? 1 : 0;                         // b = (s*h_i + 1)/2
                     const double dE = 2.0 * (h->J * (double)(2 * k - 6) + h->h * (double)(2 * bb - 1));
                     const uint64_t thr = threshold33(dE * b);
-                    if (thr == 0) nv |= 1u << idx;
+                    if (thr == 0) { nv |= 1u << idx; h->has_never = true; }
                     etab[((size_t)d * R + t) * 32 + idx] = (uint32_t)(thr - 1);
                 }
                 never[(size_t)d * R + t] = nv;
@@ -265,11 +272,19 @@ int ensure_stage(rfim_pt* h, size_t bytes) {
 }
 
 // ---- launches ------------------------------------------------------------------------------
+// kernel variants: 0 automatic, 1 site kernel, 2 word kernel, 3 flow kernel (L = 32 or 64)
+bool flow_supported(const rfim_pt* h) { return h->L == 32 || h->L == 64; }
+
+int chosen_variant(const rfim_pt* h) {
+    if (h->variant != 0) return h->variant;
+    if (flow_supported(h)) return 3;
+    return h->v.W > 0 ? 2 : 1;
+}
+
 int launch_sweep(rfim_pt* h) {
     const int ny = h->D * h->n;
     const uint32_t g32 = (uint32_t)h->sweep_g;
-    const bool word = (h->variant == 2) || (h->variant == 0 && h->v.W > 0);
-    if (h->variant == 2 && h->v.W == 0) return fail(h, RFIM_EINVAL, "word kernel needs L % 8 == 0");
+    const bool word = chosen_variant(h) == 2;
     for (int colour = 0; colour < 2; ++colour) {
         if (word) k_sweep_word<<<grid_for(h->Nh / 4, ny), 256, 0, h->stream>>>(h->v, colour, g32);
         else k_sweep_site<<<grid_for(h->Nh, ny), 256, 0, h->stream>>>(h->v, colour, g32);
@@ -279,8 +294,55 @@ int launch_sweep(rfim_pt* h) {
     return RFIM_OK;
 }
 
+template <int KIND, int C, int CPT, bool NEVER>
+int launch_flow_t(rfim_pt* h, const FlowParams& fp, long long items) {
+    auto kernel = k_sweep_flow<KIND, C, CPT, NEVER>;
+    long long blocks = max_coresident_blocks(kernel, kFlowThreads);
+    if (blocks < 1) return fail(h, RFIM_ECUDA, "flow kernel does not fit on the device");
+    blocks = std::min(blocks, items);
+    CU(launch_cooperative(kernel, dim3((unsigned)blocks), dim3(kFlowThreads), h->stream, h->v, fp));
+    h->launches += 1;
+    return RFIM_OK;
+}
+
+// `sweeps` (<= 127) sweeps of every active replica in one persistent launch per <= 32 members
+int launch_flow(rfim_pt* h, int sweeps) {
+    const int C = h->L / 32, CPT = h->L == 64 ? 2 : 1;
+    const int ZT = kFlowThreads * CPT / (h->L * C), S = h->L / ZT;
+    for (int d0 = 0; d0 < h->D; d0 += kFlowMaxMembers) {
+        FlowParams fp{};
+        fp.RR = h->flow_rr;
+        fp.G = (h->n + fp.RR - 1) / fp.RR;
+        fp.d0 = d0;
+        fp.nd = std::min(kFlowMaxMembers, h->D - d0);
+        fp.phases = 2 * sweeps;
+        fp.sweep0 = (uint32_t)h->sweep_g;
+        fp.epoch = ++h->flow_epoch;
+        fp.prog = h->flow_prog;
+        fp.prog_stride_d = h->R * 32;
+        fp.prog_stride_g = 32;
+        fp.diag = h->v.diag;
+        for (int dl = 0; dl < fp.nd; ++dl) {
+            uint32_t k0 = (uint32_t)(h->seeds[d0 + dl] & 0xFFFFFFFFull), k1 = (uint32_t)(h->seeds[d0 + dl] >> 32);
+            for (int r = 0; r < 10; ++r) { fp.rk[dl][2 * r] = k0; fp.rk[dl][2 * r + 1] = k1; k0 += kPhiloxW0; k1 += kPhiloxW1; }
+        }
+        const long long items = (long long)fp.phases * fp.nd * fp.G * S;
+        int rc;
+        if (h->kind == RFIM_FIELD_BIMODAL) {
+            if (h->L == 64) rc = h->has_never ? launch_flow_t<0, 2, 2, true>(h, fp, items) : launch_flow_t<0, 2, 2, false>(h, fp, items);
+            else rc = h->has_never ? launch_flow_t<0, 1, 1, true>(h, fp, items) : launch_flow_t<0, 1, 1, false>(h, fp, items);
+        } else {
+            if (h->L == 64) rc = launch_flow_t<1, 2, 2, false>(h, fp, items);
+            else rc = launch_flow_t<1, 1, 1, false>(h, fp, items);
+        }
+        if (rc) return rc;
+    }
+    return RFIM_OK;
+}
+
 int launch_reduce(rfim_pt* h) {
-    k_reduce_site<<<grid_for(h->Nh, h->D * h->n), 256, 0, h->stream>>>(h->v);
+    if (h->v.W > 0) k_reduce_word<<<grid_for(h->Nh / 4, h->D * h->n), 256, 0, h->stream>>>(h->v);
+    else k_reduce_site<<<grid_for(h->Nh, h->D * h->n), 256, 0, h->stream>>>(h->v);
     h->launches += 1;
     CU(cudaGetLastError());
     return RFIM_OK;
@@ -304,10 +366,18 @@ int do_sweeps(rfim_pt* h, int64_t n_sweeps, int k) {
         int rc = ensure_series(h, h->series_steps + steps);
         if (rc) return rc;
     }
-    for (int64_t it = 0; it < n_sweeps; ++it) {
-        int rc = launch_sweep(h);
+    const bool flow = chosen_variant(h) == 3;
+    int64_t left = n_sweeps;
+    while (left > 0) {
+        int64_t chunk = 1;
+        if (flow) {
+            chunk = std::min<int64_t>(left, 127);
+            if (k > 0) chunk = std::min<int64_t>(chunk, (int64_t)k - (int64_t)(h->sweep_g % (uint64_t)k));
+        }
+        int rc = flow ? launch_flow(h, (int)chunk) : launch_sweep(h);
         if (rc) return rc;
-        h->sweep_g += 1;
+        h->sweep_g += (uint64_t)chunk;
+        left -= chunk;
         if (k > 0 && (h->sweep_g % (uint64_t)k) == 0) {
             if ((rc = launch_reduce(h))) return rc;
             if ((rc = launch_exchange(h))) return rc;
@@ -388,12 +458,14 @@ int create_impl(rfim_pt** out, int L, int R, double J, double hh, int kind, int 
     A(alloc_into(h, &v.att, DR));
     A(alloc_into(h, &v.accn, DR));
     A(alloc_into(h, &v.diag, 4));
+    A(alloc_into(h, &h->flow_prog, DR * 32));
     if (rc != RFIM_OK) { rfim_pt_destroy(h); return rc; }
     auto body = [&]() -> int {
         std::vector<uint32_t> keys((size_t)D * 2);
         for (int d = 0; d < D; ++d) { keys[2 * d] = (uint32_t)(seeds[d] & 0xFFFFFFFFull); keys[2 * d + 1] = (uint32_t)(seeds[d] >> 32); }
         CU(cudaMemcpyAsync(const_cast<uint32_t*>(v.keys), keys.data(), keys.size() * 4, cudaMemcpyHostToDevice, h->stream));
         CU(cudaMemsetAsync(v.diag, 0, 32, h->stream));
+        CU(cudaMemsetAsync(h->flow_prog, 0, DR * 32 * 4, h->stream));
         CU(cudaMemsetAsync(v.t2r, 0xFF, DR * 4, h->stream));
         CU(cudaMemsetAsync(v.r2t, 0xFF, DR * 4, h->stream));
         CU(cudaStreamSynchronize(h->stream));
@@ -512,8 +584,9 @@ int rfim_pt_set_packing(rfim_pt* h, int bits) {
 
 int rfim_pt_set_kernel_variant(rfim_pt* h, int variant) {
     if (!h) return RFIM_EINVAL;
-    if (variant < 0 || variant > 2) return fail(h, RFIM_EINVAL, "unknown kernel variant");
+    if (variant < 0 || variant > 3) return fail(h, RFIM_EINVAL, "unknown kernel variant");
     if (variant == 2 && h->v.W == 0) return fail(h, RFIM_EINVAL, "word kernel needs L % 8 == 0");
+    if (variant == 3 && !flow_supported(h)) return fail(h, RFIM_EINVAL, "flow kernel needs L = 32 or 64");
     h->variant = variant;
     return RFIM_OK;
 }
@@ -834,6 +907,7 @@ int rfim_pt_get_diagnostics(rfim_pt* h, uint64_t diag[4]) {
     unsigned long long d4[4];
     CU(cudaMemcpyAsync(d4, h->v.diag, 32, cudaMemcpyDeviceToHost, h->stream));
     CU(cudaStreamSynchronize(h->stream));
+    if (d4[0] != 0) return fail(h, RFIM_ESTATE, "a flow-kernel dependency wait timed out: results are invalid");
     diag[0] = h->launches; diag[1] = d4[1]; diag[2] = d4[2]; diag[3] = d4[3];
     return RFIM_OK;
 }

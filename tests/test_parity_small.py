@@ -194,3 +194,45 @@ def test_adaptation_matches_oracle(grow):
     g.sweep(20, k); o.sweep(20, k)
     assert_same_state(g, o, what="after adapt")
     assert_same_series(g, o)
+
+
+# ---- the tuned persistent "flow" kernel (variant 3; L = 32 or 64) ---------------------------------------
+@pytest.mark.parametrize("L,R", [(32, 5), (64, 3)])
+@pytest.mark.parametrize("kind,h", [(BIMODAL, 2.0), (GAUSSIAN, 1.5)])
+def test_flow_kernel_bit_exact(L, R, kind, h):
+    T = np.geomspace(0.8, 5.0, R)                    # R is not a multiple of the replica group size
+    g, o = make_pair(L, R, 1.0, h, kind, 31 * L + R, T)
+    g.set_kernel_variant(3)
+    for chunk, k in [(1, 0), (4, 2), (3, 3), (7, 5)]:
+        g.sweep(chunk, k); o.sweep(chunk, k)
+        assert_same_state(g, o, what=f"flow L={L} after chunk {chunk},{k}")
+    assert_same_series(g, o)
+    d = g.diagnostics()
+    assert d["ulp_ambiguous"] == 0
+
+
+@pytest.mark.parametrize("kind", [BIMODAL, GAUSSIAN])
+def test_flow_kernel_extreme_temperatures_and_long_launch(kind):
+    # thresholds 0 (the "never" table entries) and ~2^32; 130 sweeps without exchange = two launches (127 + 3)
+    T = np.array([1e-30, 0.05, 1.0, 1e3, 1e30])
+    g, o = make_pair(32, 5, 1.0, 1.3, kind, 5, T)
+    g.set_kernel_variant(3)
+    g.sweep(6, 2); o.sweep(6, 2)
+    assert_same_state(g, o, what="flow extreme T")
+    g.sweep(130, 0); o.sweep(130, 0)
+    assert_same_state(g, o, what="flow 130 sweeps")
+
+
+def test_flow_kernel_batch_and_reference_kernels_agree():
+    from paper_1508_06268_b200 import binding
+    seeds = [11, 12, 13]
+    T = np.geomspace(1.0, 6.0, 6)
+    a = binding.RfimPT(32, 6, 1.0, 1.5, GAUSSIAN, seeds=seeds); a.set_kernel_variant(3)
+    b = binding.RfimPT(32, 6, 1.0, 1.5, GAUSSIAN, seeds=seeds); b.set_kernel_variant(2)
+    a.set_temperatures(T); b.set_temperatures(T)
+    a.sweep(12, 4); b.sweep(12, 4)
+    assert np.array_equal(a.get_spins_all(), b.get_spins_all())
+    for d in range(3):
+        assert np.array_equal(a.get_permutation(d=d), b.get_permutation(d=d))
+        for x, y in zip(a.get_timeseries(d=d), b.get_timeseries(d=d)):
+            assert np.array_equal(x, y)
