@@ -93,8 +93,11 @@ int rfim_pt_set_allocator(rfim_pt_alloc_fn alloc, rfim_pt_free_fn release);
 const char* rfim_pt_last_error(rfim_pt* h);
 /* 8 = one byte per spin (default), 1 = bit-packed.  Converts the stored lattices in place. */
 int rfim_pt_set_packing(rfim_pt* h, int bits);
-/* which sweep implementation runs: 0 = automatic (default), others are listed in DESIGN.md. */
+/* which sweep implementation runs: 0 = automatic (default), 1 site, 2 word, 3 flow, 4 resident. */
 int rfim_pt_set_kernel_variant(rfim_pt* h, int variant);
+/* tuning knobs (tests use them to force many-CTA partitions on small problems): key 0 = replicas per
+ * work item of the flow kernel (1..64), key 1 = CTA limit of the resident kernel (0 = one per SM). */
+int rfim_pt_set_tuning(rfim_pt* h, int key, int value);
 /* exchange period used by adapt's trial (default 10) and insertions per trial
  * (default 4, Fig. 6; the paper recommends 1-5). */
 int rfim_pt_set_adapt_params(rfim_pt* h, int exchange_every, int insertions);

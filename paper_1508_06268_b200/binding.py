@@ -45,6 +45,7 @@ SIGNATURES = {
     "rfim_pt_last_error": (ctypes.c_char_p, [_vp]),
     "rfim_pt_set_packing": (ctypes.c_int, [_vp, ctypes.c_int]),
     "rfim_pt_set_kernel_variant": (ctypes.c_int, [_vp, ctypes.c_int]),
+    "rfim_pt_set_tuning": (ctypes.c_int, [_vp, ctypes.c_int, ctypes.c_int]),
     "rfim_pt_set_adapt_params": (ctypes.c_int, [_vp, ctypes.c_int, ctypes.c_int]),
     "rfim_pt_get_info": (ctypes.c_int, [_vp, _ip, _ip, _ip, _ip, _ip]),
     "rfim_pt_get_spins_member": (ctypes.c_int, [_vp, ctypes.c_int, ctypes.c_int, _i8p]),
@@ -207,6 +208,9 @@ class RfimPT:
 
     def set_kernel_variant(self, variant):
         self._ck(load().rfim_pt_set_kernel_variant(self._h, variant))
+
+    def set_tuning(self, key, value):
+        self._ck(load().rfim_pt_set_tuning(self._h, key, value))
 
     def set_adapt_params(self, exchange_every, insertions):
         self._ck(load().rfim_pt_set_adapt_params(self._h, exchange_every, insertions))

@@ -17,6 +17,7 @@
 #include "launch.h"
 #include "philox.cuh"
 #include "sweep_flow.cuh"
+#include "sweep_res.cuh"
 #include "view.h"
 
 using namespace rfim;
@@ -29,6 +30,7 @@ rfim_pt_free_fn g_free = nullptr;
 constexpr double kTwo32 = 4294967296.0;
 constexpr double kFieldScale = 1048576.0;   // 2^20
 constexpr int32_t kFieldClamp = 8 * 1048576;
+constexpr int kResMaxGrid = 255;            // owners are stored in 8 bits (sweep_res.cuh)
 
 }  // namespace
 
@@ -55,6 +57,12 @@ struct rfim_pt {
     uint32_t flow_epoch = 0;
     int flow_rr = 4;                  // replicas per work item
     bool has_never = false;           // some reachable bimodal table entry has threshold 0
+    float* fielda_res = nullptr;      // resident-kernel copies of the field (task order), L = 32 or 64
+    uint8_t* fieldb_res = nullptr;
+    uint32_t* res_prog = nullptr;     // [kResMaxGrid] progress words of the resident kernel
+    uint32_t res_epoch = 0;
+    int res_grid_limit = 0;           // 0 = one CTA per SM
+    int sm_count = 0, smem_optin = 0;
     std::string err;
 };
 
@@ -103,6 +111,15 @@ inline long long layout_index(const rfim_pt* h, int x, int y, int z, int* colour
     return (long long)(x >> 1) + (long long)(h->L / 2) * (y + (long long)h->L * z);
 }
 
+// position of site (x,y,z) inside one member's field copy in the resident kernel's task order (sweep_res.cuh):
+// [colour][z][class s = (y+z)&1][word w = xh/4][row i = y/2][site xh%4], i.e. 16 bytes (bimodal: [piece xh/16][i][xh%16])
+inline long long res_field_index(const rfim_pt* h, int x, int y, int z) {
+    const int L = h->L, LH = L / 2, c = (x + y + z) & 1, xh = x >> 1, s = (y + z) & 1, i = y >> 1;
+    const long long blk = ((long long)c * L + z) * 2 + s;              // block of L/2 rows x L/2 sites
+    if (h->kind == RFIM_FIELD_BIMODAL) return ((blk * (L / 32) + xh / 16) * LH + i) * 16 + xh % 16;
+    return ((blk * (L / 8) + xh / 4) * LH + i) * 4 + xh % 4;
+}
+
 dim3 grid_for(long long work, int ny, int threads = 256) {
     long long bx = (work + threads - 1) / threads;
     if (bx < 1) bx = 1;
@@ -141,6 +158,13 @@ int upload_field(rfim_pt* h, int d) {
             fb[(long long)c * h->Nh + j] = f[x + (long long)L * (y + (long long)L * z)] > 0 ? 0x10 : 0x00;
         }
         CU(cudaMemcpyAsync(const_cast<uint8_t*>(h->v.fieldb) + (long long)d * h->N, fb.data(), h->N, cudaMemcpyHostToDevice, h->stream));
+        if (h->fieldb_res) {
+            std::vector<uint8_t> fr(h->N);
+            for (int z = 0; z < L; ++z) for (int y = 0; y < L; ++y) for (int x = 0; x < L; ++x)
+                fr[res_field_index(h, x, y, z)] = f[x + (long long)L * (y + (long long)L * z)] > 0 ? 0x80 : 0x00;
+            CU(cudaMemcpyAsync(h->fieldb_res + (long long)d * h->N, fr.data(), h->N, cudaMemcpyHostToDevice, h->stream));
+            CU(cudaStreamSynchronize(h->stream));
+        }
         CU(cudaStreamSynchronize(h->stream));
         h->amax[d] = std::fabs(hs);
     } else {
@@ -157,6 +181,13 @@ int upload_field(rfim_pt* h, int d) {
         }
         CU(cudaMemcpyAsync(const_cast<float*>(h->v.fielda) + (long long)d * h->N, fa.data(), h->N * sizeof(float), cudaMemcpyHostToDevice, h->stream));
         CU(cudaMemcpyAsync(const_cast<int32_t*>(h->v.fieldg) + (long long)d * h->N, fg.data(), h->N * sizeof(int32_t), cudaMemcpyHostToDevice, h->stream));
+        if (h->fielda_res) {
+            std::vector<float> fr(h->N);
+            for (int z = 0; z < L; ++z) for (int y = 0; y < L; ++y) for (int x = 0; x < L; ++x)
+                fr[res_field_index(h, x, y, z)] = (float)(hs * (double)f[x + (long long)L * (y + (long long)L * z)]);
+            CU(cudaMemcpyAsync(h->fielda_res + (long long)d * h->N, fr.data(), h->N * sizeof(float), cudaMemcpyHostToDevice, h->stream));
+            CU(cudaStreamSynchronize(h->stream));
+        }
         CU(cudaStreamSynchronize(h->stream));
         h->amax[d] = amax;
     }
@@ -272,11 +303,32 @@ int ensure_stage(rfim_pt* h, size_t bytes) {
 }
 
 // ---- launches ------------------------------------------------------------------------------
-// kernel variants: 0 automatic, 1 site kernel, 2 word kernel, 3 flow kernel (L = 32 or 64)
+// kernel variants: 0 automatic, 1 site kernel, 2 word kernel, 3 flow kernel, 4 resident kernel (3, 4: L = 32 or 64)
 bool flow_supported(const rfim_pt* h) { return h->L == 32 || h->L == 64; }
+
+// the resident kernel's partition of the D*n*L planes over the grid, and whether the largest run fits in shared memory
+struct ResPlan { int grid, total, q, rem, cap_planes, cap_reps; size_t smem; bool ok; };
+ResPlan res_plan(const rfim_pt* h) {
+    ResPlan p{};
+    p.ok = false;
+    if (!flow_supported(h) || h->n < 1 || h->sm_count < 1) return p;
+    p.grid = std::min(h->sm_count, kResMaxGrid);
+    if (h->res_grid_limit > 0) p.grid = std::min(p.grid, h->res_grid_limit);
+    const long long total = (long long)h->D * h->n * h->L;
+    if (total > (long long)p.grid * 32767) return p;
+    p.total = (int)total;
+    p.q = p.total / p.grid; p.rem = p.total % p.grid;
+    p.cap_planes = p.q + (p.rem ? 1 : 0);
+    p.cap_reps = (p.cap_planes + h->L - 2) / h->L + 1;
+    if (p.cap_reps > 255) return p;
+    p.smem = res_smem_bytes(h->L, p.cap_planes, p.cap_reps);
+    p.ok = p.smem <= (size_t)h->smem_optin;
+    return p;
+}
 
 int chosen_variant(const rfim_pt* h) {
     if (h->variant != 0) return h->variant;
+    if (res_plan(h).ok) return 4;
     if (flow_supported(h)) return 3;
     return h->v.W > 0 ? 2 : 1;
 }
@@ -340,6 +392,37 @@ int launch_flow(rfim_pt* h, int sweeps) {
     return RFIM_OK;
 }
 
+template <int KIND, int K, bool NEVER>
+int launch_res_t(rfim_pt* h, const ResPlan& pl, const ResParams& rp) {
+    auto kernel = k_sweep_res<KIND, K, NEVER>;
+    CU(cudaFuncSetAttribute(kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)pl.smem));
+    void* argv[] = {const_cast<void*>(static_cast<const void*>(&h->v)), const_cast<void*>(static_cast<const void*>(&rp))};
+    CU(cudaLaunchCooperativeKernel(reinterpret_cast<const void*>(kernel), dim3((unsigned)pl.grid), dim3(kResThreads), argv, pl.smem, h->stream));
+    h->launches += 1;
+    return RFIM_OK;
+}
+
+// `sweeps` (<= 127) sweeps of every active replica of every member in one cooperative launch
+int launch_res(rfim_pt* h, int sweeps) {
+    const ResPlan pl = res_plan(h);
+    if (!pl.ok) return fail(h, RFIM_EINVAL, "resident kernel: the planes of one CTA do not fit in shared memory");
+    ResParams rp{};
+    rp.phases = 2 * sweeps;
+    rp.sweep0 = (uint32_t)h->sweep_g;
+    rp.epoch = ++h->res_epoch;
+    rp.prog = h->res_prog;
+    rp.total_planes = pl.total; rp.q = pl.q; rp.rem = pl.rem;
+    rp.cap_planes = pl.cap_planes; rp.cap_reps = pl.cap_reps;
+    rp.fielda_res = h->fielda_res; rp.fieldb_res = h->fieldb_res;
+    rp.diag = h->v.diag;
+    if (h->kind == RFIM_FIELD_BIMODAL) {
+        if (h->L == 64) return h->has_never ? launch_res_t<0, 2, true>(h, pl, rp) : launch_res_t<0, 2, false>(h, pl, rp);
+        return h->has_never ? launch_res_t<0, 1, true>(h, pl, rp) : launch_res_t<0, 1, false>(h, pl, rp);
+    }
+    if (h->L == 64) return launch_res_t<1, 2, false>(h, pl, rp);
+    return launch_res_t<1, 1, false>(h, pl, rp);
+}
+
 int launch_reduce(rfim_pt* h) {
     if (h->v.W > 0) k_reduce_word<<<grid_for(h->Nh / 4, h->D * h->n), 256, 0, h->stream>>>(h->v);
     else k_reduce_site<<<grid_for(h->Nh, h->D * h->n), 256, 0, h->stream>>>(h->v);
@@ -366,7 +449,8 @@ int do_sweeps(rfim_pt* h, int64_t n_sweeps, int k) {
         int rc = ensure_series(h, h->series_steps + steps);
         if (rc) return rc;
     }
-    const bool flow = chosen_variant(h) == 3;
+    const int variant = chosen_variant(h);
+    const bool flow = variant == 3 || variant == 4;
     int64_t left = n_sweeps;
     while (left > 0) {
         int64_t chunk = 1;
@@ -374,7 +458,7 @@ int do_sweeps(rfim_pt* h, int64_t n_sweeps, int k) {
             chunk = std::min<int64_t>(left, 127);
             if (k > 0) chunk = std::min<int64_t>(chunk, (int64_t)k - (int64_t)(h->sweep_g % (uint64_t)k));
         }
-        int rc = flow ? launch_flow(h, (int)chunk) : launch_sweep(h);
+        int rc = variant == 4 ? launch_res(h, (int)chunk) : (flow ? launch_flow(h, (int)chunk) : launch_sweep(h));
         if (rc) return rc;
         h->sweep_g += (uint64_t)chunk;
         left -= chunk;
@@ -459,6 +543,18 @@ int create_impl(rfim_pt** out, int L, int R, double J, double hh, int kind, int 
     A(alloc_into(h, &v.accn, DR));
     A(alloc_into(h, &v.diag, 4));
     A(alloc_into(h, &h->flow_prog, DR * 32));
+    A(alloc_into(h, &h->res_prog, (size_t)kResMaxGrid + 1));
+    if (flow_supported(h)) {
+        if (kind == RFIM_FIELD_BIMODAL) A(alloc_into(h, &h->fieldb_res, (size_t)D * h->N));
+        else A(alloc_into(h, &h->fielda_res, (size_t)D * h->N));
+    }
+    {
+        int dev = 0;
+        if (cudaGetDevice(&dev) == cudaSuccess) {
+            cudaDeviceGetAttribute(&h->sm_count, cudaDevAttrMultiProcessorCount, dev);
+            cudaDeviceGetAttribute(&h->smem_optin, cudaDevAttrMaxSharedMemoryPerBlockOptin, dev);
+        }
+    }
     if (rc != RFIM_OK) { rfim_pt_destroy(h); return rc; }
     auto body = [&]() -> int {
         std::vector<uint32_t> keys((size_t)D * 2);
@@ -466,6 +562,7 @@ int create_impl(rfim_pt** out, int L, int R, double J, double hh, int kind, int 
         CU(cudaMemcpyAsync(const_cast<uint32_t*>(v.keys), keys.data(), keys.size() * 4, cudaMemcpyHostToDevice, h->stream));
         CU(cudaMemsetAsync(v.diag, 0, 32, h->stream));
         CU(cudaMemsetAsync(h->flow_prog, 0, DR * 32 * 4, h->stream));
+        CU(cudaMemsetAsync(h->res_prog, 0, ((size_t)kResMaxGrid + 1) * 4, h->stream));
         CU(cudaMemsetAsync(v.t2r, 0xFF, DR * 4, h->stream));
         CU(cudaMemsetAsync(v.r2t, 0xFF, DR * 4, h->stream));
         CU(cudaStreamSynchronize(h->stream));
@@ -584,11 +681,19 @@ int rfim_pt_set_packing(rfim_pt* h, int bits) {
 
 int rfim_pt_set_kernel_variant(rfim_pt* h, int variant) {
     if (!h) return RFIM_EINVAL;
-    if (variant < 0 || variant > 3) return fail(h, RFIM_EINVAL, "unknown kernel variant");
+    if (variant < 0 || variant > 4) return fail(h, RFIM_EINVAL, "unknown kernel variant");
+    if (variant == 4 && !flow_supported(h)) return fail(h, RFIM_EINVAL, "resident kernel needs L = 32 or 64");
     if (variant == 2 && h->v.W == 0) return fail(h, RFIM_EINVAL, "word kernel needs L % 8 == 0");
     if (variant == 3 && !flow_supported(h)) return fail(h, RFIM_EINVAL, "flow kernel needs L = 32 or 64");
     h->variant = variant;
     return RFIM_OK;
+}
+
+int rfim_pt_set_tuning(rfim_pt* h, int key, int value) {
+    if (!h) return RFIM_EINVAL;
+    if (key == 0 && value >= 1 && value <= 64) { h->flow_rr = value; return RFIM_OK; }
+    if (key == 1 && value >= 0 && value <= kResMaxGrid) { h->res_grid_limit = value; return RFIM_OK; }
+    return fail(h, RFIM_EINVAL, "unknown tuning key or value out of range");
 }
 
 int rfim_pt_set_adapt_params(rfim_pt* h, int exchange_every, int insertions) {

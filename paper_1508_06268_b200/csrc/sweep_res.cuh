@@ -1,0 +1,401 @@
+// sweep_res.cuh -- the shared-memory-resident sweep: every lattice plane stays in the shared memory of
+// one SM for a whole launch (all phases of an exchange period).  DESIGN.md section 6.
+//
+// Decomposition.  The D*n active replicas (by temperature rank) are stacked into one list of
+// D*n*L planes (plane P = (d*n + t)*L + z).  CTA b of a cooperative launch owns the contiguous run
+// [start_b, start_b + count_b) with counts differing by at most one, so 148 SMs hold 55 or 56 planes
+// each at L = 64, R = 128: no replica-granular imbalance (128 replicas do not divide over 148 SMs).
+// A run is loaded once, swept 2*sweeps phases (colour 0, colour 1, ...) in place, and stored once.
+// Only the planes at the ends of a run (and at a replica seam inside it) have a z-neighbour in
+// another CTA: after every phase their freshly written colour is also stored to global memory and
+// the CTA's progress word is released; the neighbour acquires it before it reads those rows
+// straight from L2.  Boundary planes are processed first in every phase, so the neighbour has a
+// whole phase of slack.  All CTAs are co-resident (cooperative launch), hence no deadlock.
+//
+// In shared memory a spin is a byte holding 0 or SP (= 8), four same-colour sites per 32-bit word
+// exactly as in global memory (where it is 0/1), so the six-neighbour count of four sites is three
+// IADD3, and count*SP + spin*8*SP [+ field bit] is directly the byte offset of the site's entry in
+// the replica's 8-byte acceptance table: one PRMT splices it into the (256-byte aligned) table
+// address, one LDS.64 fetches the entry.
+//
+// A thread owns one row of one colour (L/2 sites = 4K words = 4K Philox calls); the 32 lanes of a
+// warp own 32 rows of the same checkerboard class s = (y+z)&1, so the direction of the second
+// x-neighbour ((s+colour)&1) is warp-uniform.  Shared memory is laid out [colour][s][piece][row],
+// which makes every 16-byte access of a warp contiguous (no bank conflicts); the field is read from
+// a copy stored in the same task order (coalesced 16-byte loads from L2).
+#pragma once
+#include <cstdint>
+#include "kernels_ref.cuh"
+#include "philox.cuh"
+#include "sweep_flow.cuh"
+#include "view.h"
+
+namespace rfim {
+
+constexpr int kResThreads = 512;
+constexpr int kResWarps = kResThreads / 32;
+constexpr uint32_t kResSP = 8;                  // shared-memory spin coding: 0 / SP
+constexpr int kResTabBytes = 256;               // per-replica acceptance table slot (256-byte aligned)
+
+struct ResParams {
+    int phases;                  // 2 * sweeps of this launch, <= 254
+    uint32_t sweep0;             // global sweep index of phase 0
+    uint32_t epoch;              // launch id: progress words hold (epoch << 8) | phases published
+    uint32_t* prog;              // [grid]
+    int total_planes;            // D * n * L
+    int q, rem;                  // run of CTA b: start = b*q + min(b, rem), count = q + (b < rem)
+    int cap_planes, cap_reps;    // shared-memory carve (planes, replicas) -- same for every CTA
+    const float* fielda_res;     // Gaussian: [D][2][L][2][4K][L/2] float4 (task order), (float)(hs * g_i)
+    const uint8_t* fieldb_res;   // bimodal:  [D][2][L][2][K][L/2] uint4, 0x80 where h_i = +1
+    unsigned long long* diag;
+};
+
+struct ResPlane {                // 8 bytes per resident plane
+    int16_t zp_pl, zm_pl;        // local index of plane z+1 / z-1, or -1: it lives in another CTA
+    uint8_t zp_owner, zm_owner;  // that CTA
+    uint8_t rep, z;
+};
+
+struct ResRep {                  // per replica touched by the run
+    int ds, d, slot, tr;
+    float band; uint32_t never;
+    double beta;
+    uint32_t rk[20];             // Philox round keys rk[2r] = k0 + r*W0, rk[2r+1] = k1 + r*W1
+};
+
+__host__ __device__ inline size_t res_smem_bytes(int L, int cap_planes, int cap_reps) {
+    size_t b = (size_t)cap_reps * kResTabBytes + (size_t)cap_planes * L * L;
+    b += (size_t)cap_reps * sizeof(ResRep);
+    b += (size_t)cap_planes * sizeof(ResPlane);
+    b += (size_t)((cap_planes * (L / 2) + 31) / 32) * sizeof(int);       // block order
+    b += 16;                                                             // counters
+    return (b + 15) & ~(size_t)15;
+}
+
+__device__ __forceinline__ uint2 lds64(uint32_t saddr) {
+    uint2 r;
+#if defined(__CUDA_ARCH__)
+    asm volatile("ld.shared.v2.u32 {%0, %1}, [%2];" : "=r"(r.x), "=r"(r.y) : "r"(saddr));
+#else
+    r.x = r.y = 0;
+#endif
+    return r;
+}
+
+// prmt.b32 in its default mode: selector nibble n picks byte (n & 7) of {b, a}; bit 3 replicates that byte's sign
+// bit over the whole byte (the CUDA intrinsic __byte_perm ignores bit 3)
+__device__ __forceinline__ uint32_t prmt(uint32_t a, uint32_t b, uint32_t sel) {
+    uint32_t r;
+#if defined(__CUDA_ARCH__)
+    asm("prmt.b32 %0, %1, %2, %3;" : "=r"(r) : "r"(a), "r"(b), "r"(sel));
+#else
+    r = 0;
+#endif
+    return r;
+}
+
+// exact rule for the four sites of one word whose table-offset bytes are idx8 = SP*n1 + 8*SP*s (rare)
+__device__ __noinline__ uint32_t res_gauss_word_exact(const View& v, uint32_t idx8, const int32_t* __restrict__ g4, double beta,
+                                                      uint32_t u0, uint32_t u1, uint32_t u2, uint32_t u3) {
+    uint32_t flips = 0;
+    const uint32_t u[4] = {u0, u1, u2, u3};
+#pragma unroll
+    for (int k = 0; k < 4; ++k) {
+        const uint32_t b = (idx8 >> (8 * k)) & 0xFFu;
+        if (gauss_accept_exact(v, (int)(b >> 6), (int)((b >> 3) & 7u), g4[k], beta, u[k])) flips |= kResSP << (8 * k);
+    }
+    return flips;
+}
+
+__device__ __forceinline__ Words4 philox_rkreg(const uint32_t (&rk)[20], uint32_t c0, uint32_t c1, uint32_t c2, uint32_t c3) {
+#pragma unroll
+    for (int r = 0; r < 10; ++r) {
+        const uint32_t hi0 = __umulhi(kPhiloxM0, c0), lo0 = kPhiloxM0 * c0;
+        const uint32_t hi1 = __umulhi(kPhiloxM1, c2), lo1 = kPhiloxM1 * c2;
+        const uint32_t n0 = hi1 ^ c1 ^ rk[2 * r];
+        const uint32_t n2 = hi0 ^ c3 ^ rk[2 * r + 1];
+        c1 = lo1; c3 = lo0; c0 = n0; c2 = n2;
+    }
+    Words4 w;
+    w.w0 = c0; w.w1 = c1; w.w2 = c2; w.w3 = c3;
+    return w;
+}
+
+// K = 16-byte pieces per row per colour (L = 32 K)
+template <int KIND, int K, bool NEVER>
+__global__ void __launch_bounds__(kResThreads, 1) k_sweep_res(const View v, const ResParams rp) {
+    constexpr int L = 32 * K;
+    constexpr int LH = L / 2;                   // rows per class per plane
+    constexpr int ROWB = 16 * K;                // bytes (= sites) per row per colour
+    constexpr int W = 4 * K;                    // words (= Philox calls) per row
+    extern __shared__ __align__(1024) uint8_t smem[];
+
+    const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
+    const int b = blockIdx.x;
+    const int start = b * rp.q + min(b, rp.rem);
+    const int count = rp.q + (b < rp.rem ? 1 : 0);
+    if (count == 0) return;
+    const int Ecap = rp.cap_planes * LH;        // rows per (colour, class) array
+    const int E = count * LH;                   // rows in use
+    const int nb = (E + 31) / 32;               // 32-row blocks per class
+
+    uint8_t* s_tab = smem;
+    uint4* s_sp = reinterpret_cast<uint4*>(smem + (size_t)rp.cap_reps * kResTabBytes);
+    ResRep* s_rep = reinterpret_cast<ResRep*>(reinterpret_cast<uint8_t*>(s_sp) + (size_t)rp.cap_planes * L * L);
+    ResPlane* s_plane = reinterpret_cast<ResPlane*>(s_rep + rp.cap_reps);
+    int* s_order = reinterpret_cast<int*>(s_plane + rp.cap_planes);
+    int* s_ctl = s_order + (Ecap + 31) / 32;    // [0] boundary tasks done (cumulative), [1] boundary blocks
+    auto A = [&](int col, int s, int k, int e) { return ((col * 2 + s) * K + k) * Ecap + e; };
+
+    // ---- set-up: plane table, replica contexts, block order --------------------------------------------
+    const int dt0 = start / L;
+    const int nrep = (start + count - 1) / L - dt0 + 1;
+    for (int p = tid; p < count; p += kResThreads) {
+        const int P = start + p, dt = P / L, z = P % L;
+        const int Pzp = dt * L + (z + 1 == L ? 0 : z + 1), Pzm = dt * L + (z == 0 ? L - 1 : z - 1);
+        auto owner = [&](int Q) {
+            const int big = rp.rem * (rp.q + 1);
+            return Q < big ? Q / (rp.q + 1) : rp.rem + (Q - big) / rp.q;
+        };
+        ResPlane pi;
+        const bool lp = Pzp >= start && Pzp < start + count, lm = Pzm >= start && Pzm < start + count;
+        pi.zp_pl = lp ? (int16_t)(Pzp - start) : (int16_t)-1;
+        pi.zm_pl = lm ? (int16_t)(Pzm - start) : (int16_t)-1;
+        pi.zp_owner = lp ? 0 : (uint8_t)owner(Pzp);
+        pi.zm_owner = lm ? 0 : (uint8_t)owner(Pzm);
+        pi.rep = (uint8_t)(dt - dt0);
+        pi.z = (uint8_t)z;
+        s_plane[p] = pi;
+    }
+    for (int r = tid; r < nrep; r += kResThreads) {
+        const int dt = dt0 + r, d = dt / v.n, t = dt % v.n;
+        ResRep rr;
+        rr.d = d; rr.tr = d * v.R + t; rr.slot = v.t2r[rr.tr]; rr.ds = d * v.R + rr.slot;
+        rr.band = KIND == 0 ? 0.f : v.band[rr.tr];
+        rr.never = KIND == 0 ? v.never[rr.tr] : 0u;
+        rr.beta = v.beta[rr.tr];
+        uint32_t k0 = v.keys[2 * d], k1 = v.keys[2 * d + 1];
+        for (int i = 0; i < 10; ++i) { rr.rk[2 * i] = k0; rr.rk[2 * i + 1] = k1; k0 += kPhiloxW0; k1 += kPhiloxW1; }
+        s_rep[r] = rr;
+    }
+    // acceptance tables, 8-byte entries at byte offset SP*n1 + 8*SP*s (+ 16*SP*hb): Gaussian {x, y}, bimodal {thr-1, never}
+    for (int i = tid; i < nrep * 32; i += kResThreads) {
+        const int r = i >> 5, idx = i & 31;
+        const int dt = dt0 + r, d = dt / v.n, t = dt % v.n, tr = d * v.R + t;
+        uint2 ent = make_uint2(0u, 0u);
+        if (KIND == 0) {
+            ent.x = v.etab[(long long)tr * 32 + idx];
+            ent.y = (v.never[tr] >> idx) & 1u;
+        } else if (idx < 16) {
+            const GaussEntry g = v.gtab[(long long)tr * 16 + idx];
+            ent.x = __float_as_uint(g.x); ent.y = __float_as_uint(g.y);
+        }
+        reinterpret_cast<uint2*>(s_tab + (size_t)r * kResTabBytes)[idx] = ent;
+    }
+    __syncthreads();
+    if (tid == 0) {
+        int nbd = 0;
+        auto is_boundary = [&](int eb) {
+            const int p0 = (eb * 32) / LH, p1 = min((eb * 32 + 31) / LH, count - 1);
+            for (int p = p0; p <= p1; ++p)
+                if (s_plane[p].zp_pl < 0 || s_plane[p].zm_pl < 0) return true;
+            return false;
+        };
+        for (int eb = 0; eb < nb; ++eb) if (is_boundary(eb)) s_order[nbd++] = eb;
+        int k = nbd;
+        for (int eb = 0; eb < nb; ++eb) if (!is_boundary(eb)) s_order[k++] = eb;
+        s_ctl[0] = 0; s_ctl[1] = nbd;
+    }
+
+    // ---- load the run: global [colour][z][y][ROWB] (0/1) -> shared [colour][s][k][row] (0/SP) ------------------
+    {
+        const int units = count * 2 * L * K;            // 16-byte pieces
+        for (int u = tid; u < units; u += kResThreads) {
+            const int k = u % K, y = (u / K) % L, col = (u / (K * L)) & 1, p = u / (2 * K * L);
+            const ResPlane pi = s_plane[p];
+            const int ds = s_rep[pi.rep].ds, z = pi.z;
+            const uint8_t* src = v.spins + ((long long)ds * 2 + col) * v.Nh + ((long long)z * L + y) * ROWB + 16 * k;
+            uint4 x = ld_cg16(src);
+            x.x *= kResSP; x.y *= kResSP; x.z *= kResSP; x.w *= kResSP;
+            s_sp[A(col, (y + z) & 1, k, p * LH + (y >> 1))] = x;
+        }
+    }
+    __syncthreads();
+    const int n_bblocks = s_ctl[1];
+    const int n_btasks = 2 * n_bblocks;
+    const uint32_t tab0 = (uint32_t)__cvta_generic_to_shared(s_tab);
+
+    // ---- phases ------------------------------------------------------------------------------------
+    for (int p = 0; p < rp.phases; ++p) {
+        const int c = p & 1, oc = 1 - c;
+        const uint32_t sweep = rp.sweep0 + (uint32_t)(p >> 1);
+        const uint32_t dom = c == 0 ? kDomColour0 : kDomColour1;
+        for (int task = warp; task < 2 * nb; task += kResWarps) {
+            const int bidx = task >> 1, s = task & 1;
+            const int eb = s_order[bidx];
+            const bool btask = bidx < n_bblocks;
+            const int e_raw = eb * 32 + lane;
+            const bool valid = e_raw < E;
+            const int e = valid ? e_raw : E - 1;
+            const int pl = e / LH, i = e % LH;
+            const ResPlane pi = s_plane[pl];
+            const ResRep* rr = s_rep + pi.rep;
+            const int z = pi.z, ys = (s + z) & 1, y = 2 * i + ys;
+            const int dir = (s + c) & 1;                  // 0: second x-neighbour at xh-1, 1: at xh+1 (warp-uniform)
+            const int ds = rr->ds;
+            const bool remote_p = pi.zp_pl < 0, remote_m = pi.zm_pl < 0;
+
+            // wait until the owners of my remote neighbour planes have published phase p-1
+            if (btask && p > 0) {
+                const uint32_t want = (rp.epoch << 8) | (uint32_t)p;
+                int spins = 0;
+                for (;;) {
+                    bool ok = true;
+                    if (remote_p) ok = ok && (int32_t)(ld_acquire_gpu(rp.prog + pi.zp_owner) - want) >= 0;
+                    if (remote_m) ok = ok && (int32_t)(ld_acquire_gpu(rp.prog + pi.zm_owner) - want) >= 0;
+                    if (__all_sync(0xFFFFFFFFu, ok)) break;
+                    backoff();
+                    if (++spins > (1 << 22)) { if (lane == 0) atomicOr(rp.diag, 1ull); break; }
+                }
+            }
+
+            // ---- neighbour words of the row: t = SP * (number of up neighbours) per byte -----------------------
+            uint32_t cw[W], t[W], me[W];
+            const int e_yp = pl * LH + (ys ? (i + 1 == LH ? 0 : i + 1) : i);
+            const int e_ym = pl * LH + (ys ? i : (i == 0 ? LH - 1 : i - 1));
+#pragma unroll
+            for (int k = 0; k < K; ++k) {
+                const uint4 x = s_sp[A(oc, s, k, e)];
+                const uint4 yp = s_sp[A(oc, 1 - s, k, e_yp)];
+                const uint4 ym = s_sp[A(oc, 1 - s, k, e_ym)];
+                uint4 zp, zm;
+                if (!remote_p) zp = s_sp[A(oc, 1 - s, k, pi.zp_pl * LH + i)];
+                else {
+                    const int zq = z + 1 == L ? 0 : z + 1;
+                    zp = ld_cg16(v.spins + ((long long)ds * 2 + oc) * v.Nh + ((long long)zq * L + y) * ROWB + 16 * k);
+                    zp.x *= kResSP; zp.y *= kResSP; zp.z *= kResSP; zp.w *= kResSP;
+                }
+                if (!remote_m) zm = s_sp[A(oc, 1 - s, k, pi.zm_pl * LH + i)];
+                else {
+                    const int zq = z == 0 ? L - 1 : z - 1;
+                    zm = ld_cg16(v.spins + ((long long)ds * 2 + oc) * v.Nh + ((long long)zq * L + y) * ROWB + 16 * k);
+                    zm.x *= kResSP; zm.y *= kResSP; zm.z *= kResSP; zm.w *= kResSP;
+                }
+                const uint4 m = s_sp[A(c, s, k, e)];
+                cw[4 * k + 0] = x.x; cw[4 * k + 1] = x.y; cw[4 * k + 2] = x.z; cw[4 * k + 3] = x.w;
+                t[4 * k + 0] = yp.x + ym.x + zp.x + zm.x; t[4 * k + 1] = yp.y + ym.y + zp.y + zm.y;
+                t[4 * k + 2] = yp.z + ym.z + zp.z + zm.z; t[4 * k + 3] = yp.w + ym.w + zp.w + zm.w;
+                me[4 * k + 0] = m.x; me[4 * k + 1] = m.y; me[4 * k + 2] = m.z; me[4 * k + 3] = m.w;
+            }
+            const long long blk = (((long long)rr->d * 2 + c) * L + z) * 2 + s;      // field block of this (colour, plane, class)
+            if (KIND == 0) {
+#pragma unroll
+                for (int k = 0; k < K; ++k) {
+                    const uint4 f = __ldg(reinterpret_cast<const uint4*>(rp.fieldb_res) + (blk * K + k) * LH + i);
+                    t[4 * k + 0] += f.x; t[4 * k + 1] += f.y; t[4 * k + 2] += f.z; t[4 * k + 3] += f.w;
+                }
+            }
+            uint32_t idx8[W];
+            if (dir == 0) {
+#pragma unroll
+                for (int w = 0; w < W; ++w) idx8[w] = t[w] + cw[w] + __funnelshift_r(cw[(w + W - 1) % W], cw[w], 24) + (me[w] << 3);
+            } else {
+#pragma unroll
+                for (int w = 0; w < W; ++w) idx8[w] = t[w] + cw[w] + __funnelshift_r(cw[w], cw[(w + 1) % W], 8) + (me[w] << 3);
+            }
+
+            // ---- per-task constants ---------------------------------------------------------------------------
+            uint32_t rk[20];
+#pragma unroll
+            for (int j = 0; j < 5; ++j) {
+                const uint4 q4 = reinterpret_cast<const uint4*>(rr->rk)[j];
+                rk[4 * j] = q4.x; rk[4 * j + 1] = q4.y; rk[4 * j + 2] = q4.z; rk[4 * j + 3] = q4.w;
+            }
+            const uint32_t slot = (uint32_t)rr->slot;
+            const uint32_t tab_addr = tab0 + (uint32_t)pi.rep * kResTabBytes;
+            const float band = rr->band;
+            const uint32_t q0 = (uint32_t)W * (uint32_t)(y + L * z);
+            const float4* fa = reinterpret_cast<const float4*>(rp.fielda_res) + (blk * W) * LH + i;
+
+            // ---- the 4K words of the row -------------------------------------------------------------------
+#pragma unroll
+            for (int w = 0; w < W; ++w) {
+                const Words4 r = philox_rkreg(rk, q0 + (uint32_t)w, sweep, slot, dom);
+                const uint32_t u[4] = {r.w0, r.w1, r.w2, r.w3};
+                uint32_t flips;
+                if (KIND == 0) {
+                    flips = 0;
+#pragma unroll
+                    for (int k = 0; k < 4; ++k) {
+                        const uint2 ent = lds64(__byte_perm(idx8[w], tab_addr, 0x7650 + k));
+                        bool acc = u[k] <= ent.x;
+                        if (NEVER) acc = acc && ent.y == 0u;
+                        if (acc) flips |= kResSP << (8 * k);
+                    }
+                } else {
+                    const float4 a4 = __ldg(fa + (long long)w * LH);
+                    const float a[4] = {a4.x, a4.y, a4.z, a4.w};
+                    uint32_t db[4];
+                    bool amb = false;
+#pragma unroll
+                    for (int k = 0; k < 4; ++k) {
+                        const uint2 ent = lds64(__byte_perm(idx8[w], tab_addr, 0x7650 + k));
+                        const float P = ex2_approx(fmaf(a[k], __uint_as_float(ent.y), __uint_as_float(ent.x)));
+                        const float d = __uint2float_rn(u[k]) - P;
+                        amb = amb || (fabsf(d) < band);
+                        db[k] = __float_as_uint(d);
+                    }
+                    // sign bytes of the four differences -> 0xFF where d < 0 (accept)
+                    const uint32_t m01 = prmt(db[0], db[1], 0x00FBu);
+                    const uint32_t m23 = prmt(db[2], db[3], 0xFB00u);
+                    flips = prmt(m01, m23, 0x7610u) & (kResSP * 0x01010101u);
+                    if (amb) {
+                        const int32_t* g4 = v.fieldg + ((long long)rr->d * 2 + c) * v.Nh + ((long long)z * L + y) * ROWB + 4 * w;
+                        flips = res_gauss_word_exact(v, idx8[w], g4, rr->beta, u[0], u[1], u[2], u[3]);
+                    }
+                }
+                me[w] ^= flips;
+            }
+
+            // ---- write back -----------------------------------------------------------------------------------
+            if (valid) {
+#pragma unroll
+                for (int k = 0; k < K; ++k)
+                    s_sp[A(c, s, k, e)] = make_uint4(me[4 * k], me[4 * k + 1], me[4 * k + 2], me[4 * k + 3]);
+                if (remote_p || remote_m) {
+                    uint8_t* dst = v.spins + ((long long)ds * 2 + c) * v.Nh + ((long long)z * L + y) * ROWB;
+#pragma unroll
+                    for (int k = 0; k < K; ++k)
+                        *reinterpret_cast<uint4*>(dst + 16 * k) = make_uint4(me[4 * k] >> 3, me[4 * k + 1] >> 3, me[4 * k + 2] >> 3, me[4 * k + 3] >> 3);
+                }
+            }
+            if (btask) {
+                __syncwarp();
+                if (lane == 0) {
+                    __threadfence();
+                    const int done = atomicAdd(&s_ctl[0], 1) + 1;
+                    if (done == n_btasks * (p + 1)) {
+                        __threadfence();
+                        st_release_gpu(rp.prog + b, (rp.epoch << 8) | (uint32_t)(p + 1));
+                    }
+                }
+            }
+        }
+        __syncthreads();
+    }
+
+    // ---- store the run back ------------------------------------------------------------------------------
+    {
+        const int units = count * 2 * L * K;
+        for (int u = tid; u < units; u += kResThreads) {
+            const int k = u % K, y = (u / K) % L, col = (u / (K * L)) & 1, p = u / (2 * K * L);
+            const ResPlane pi = s_plane[p];
+            const int ds = s_rep[pi.rep].ds, z = pi.z;
+            uint4 x = s_sp[A(col, (y + z) & 1, k, p * LH + (y >> 1))];
+            x.x >>= 3; x.y >>= 3; x.z >>= 3; x.w >>= 3;
+            *reinterpret_cast<uint4*>(v.spins + ((long long)ds * 2 + col) * v.Nh + ((long long)z * L + y) * ROWB + 16 * k) = x;
+        }
+    }
+}
+
+}  // namespace rfim

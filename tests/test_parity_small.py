@@ -236,3 +236,48 @@ def test_flow_kernel_batch_and_reference_kernels_agree():
         assert np.array_equal(a.get_permutation(d=d), b.get_permutation(d=d))
         for x, y in zip(a.get_timeseries(d=d), b.get_timeseries(d=d)):
             assert np.array_equal(x, y)
+
+
+# ---- the shared-memory-resident kernel (variant 4; L = 32 or 64) ------------------------------------------
+@pytest.mark.parametrize("L,R,grid", [(32, 5, 0), (32, 5, 7), (32, 3, 148), (64, 3, 0), (64, 3, 5), (64, 2, 4)])
+@pytest.mark.parametrize("kind,h", [(BIMODAL, 2.0), (GAUSSIAN, 1.5)])
+def test_resident_kernel_bit_exact(L, R, grid, kind, h):
+    # grid limits force runs of many planes per CTA, runs that cross replica seams, odd plane counts (ragged
+    # last 32-row block at L = 32) and the one-plane-per-CTA extreme
+    T = np.geomspace(0.8, 5.0, R)
+    g, o = make_pair(L, R, 1.0, h, kind, 31 * L + R, T)
+    g.set_kernel_variant(4)
+    g.set_tuning(1, grid)
+    for chunk, k in [(1, 0), (4, 2), (3, 3), (7, 5)]:
+        g.sweep(chunk, k); o.sweep(chunk, k)
+        assert_same_state(g, o, what=f"resident L={L} grid={grid} after chunk {chunk},{k}")
+    assert_same_series(g, o)
+    d = g.diagnostics()
+    assert d["ulp_ambiguous"] == 0
+
+
+@pytest.mark.parametrize("kind", [BIMODAL, GAUSSIAN])
+def test_resident_kernel_extreme_temperatures_and_long_launch(kind):
+    T = np.array([1e-30, 0.05, 1.0, 1e3, 1e30])
+    g, o = make_pair(32, 5, 1.0, 1.3, kind, 5, T)
+    g.set_kernel_variant(4)
+    g.set_tuning(1, 11)
+    g.sweep(6, 2); o.sweep(6, 2)
+    assert_same_state(g, o, what="resident extreme T")
+    g.sweep(130, 0); o.sweep(130, 0)
+    assert_same_state(g, o, what="resident 130 sweeps")
+
+
+def test_resident_kernel_batch_n_less_than_R_and_flow_kernel_agree():
+    from paper_1508_06268_b200 import binding
+    seeds = [11, 12, 13]
+    T = np.geomspace(1.0, 6.0, 5)                                      # n = 5 < R = 6
+    a = binding.RfimPT(32, 6, 1.0, 1.5, GAUSSIAN, seeds=seeds); a.set_kernel_variant(4); a.set_tuning(1, 9)
+    b = binding.RfimPT(32, 6, 1.0, 1.5, GAUSSIAN, seeds=seeds); b.set_kernel_variant(3)
+    a.set_temperatures(T); b.set_temperatures(T)
+    a.sweep(12, 4); b.sweep(12, 4)
+    assert np.array_equal(a.get_spins_all(), b.get_spins_all())
+    for d in range(3):
+        assert np.array_equal(a.get_permutation(d=d), b.get_permutation(d=d))
+        for x, y in zip(a.get_timeseries(d=d), b.get_timeseries(d=d)):
+            assert np.array_equal(x, y)
