@@ -105,8 +105,11 @@ def use_torch_allocator():
             return None
 
     def _free(ptr):
-        if ptr:
-            torch.cuda.caching_allocator_delete(ptr)
+        try:
+            if ptr:
+                torch.cuda.caching_allocator_delete(ptr)
+        except (AttributeError, TypeError):           # interpreter shutdown: torch is already torn down
+            pass
 
     a, f = _ALLOC_FN(_alloc), _FREE_FN(_free)
     _alloc_refs["alloc"], _alloc_refs["free"] = a, f          # keep the thunks alive

@@ -392,14 +392,19 @@ int launch_flow(rfim_pt* h, int sweeps) {
     return RFIM_OK;
 }
 
-template <int KIND, int K, bool NEVER>
+template <int KIND, int K, bool NEVER, bool UNI>
 int launch_res_t(rfim_pt* h, const ResPlan& pl, const ResParams& rp) {
-    auto kernel = k_sweep_res<KIND, K, NEVER>;
+    auto kernel = k_sweep_res<KIND, K, NEVER, UNI, kResThreads>;
     CU(cudaFuncSetAttribute(kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)pl.smem));
     void* argv[] = {const_cast<void*>(static_cast<const void*>(&h->v)), const_cast<void*>(static_cast<const void*>(&rp))};
     CU(cudaLaunchCooperativeKernel(reinterpret_cast<const void*>(kernel), dim3((unsigned)pl.grid), dim3(kResThreads), argv, pl.smem, h->stream));
     h->launches += 1;
     return RFIM_OK;
+}
+
+template <int KIND, int K, bool NEVER>
+int launch_res_u(rfim_pt* h, const ResPlan& pl, const ResParams& rp) {
+    return h->D == 1 ? launch_res_t<KIND, K, NEVER, true>(h, pl, rp) : launch_res_t<KIND, K, NEVER, false>(h, pl, rp);
 }
 
 // `sweeps` (<= 127) sweeps of every active replica of every member in one cooperative launch
@@ -415,12 +420,16 @@ int launch_res(rfim_pt* h, int sweeps) {
     rp.cap_planes = pl.cap_planes; rp.cap_reps = pl.cap_reps;
     rp.fielda_res = h->fielda_res; rp.fieldb_res = h->fieldb_res;
     rp.diag = h->v.diag;
-    if (h->kind == RFIM_FIELD_BIMODAL) {
-        if (h->L == 64) return h->has_never ? launch_res_t<0, 2, true>(h, pl, rp) : launch_res_t<0, 2, false>(h, pl, rp);
-        return h->has_never ? launch_res_t<0, 1, true>(h, pl, rp) : launch_res_t<0, 1, false>(h, pl, rp);
+    {
+        uint32_t k0 = (uint32_t)(h->seeds[0] & 0xFFFFFFFFull), k1 = (uint32_t)(h->seeds[0] >> 32);
+        for (int r = 0; r < 10; ++r) { rp.rk0[2 * r] = k0; rp.rk0[2 * r + 1] = k1; k0 += kPhiloxW0; k1 += kPhiloxW1; }
     }
-    if (h->L == 64) return launch_res_t<1, 2, false>(h, pl, rp);
-    return launch_res_t<1, 1, false>(h, pl, rp);
+    if (h->kind == RFIM_FIELD_BIMODAL) {
+        if (h->L == 64) return h->has_never ? launch_res_u<0, 2, true>(h, pl, rp) : launch_res_u<0, 2, false>(h, pl, rp);
+        return h->has_never ? launch_res_u<0, 1, true>(h, pl, rp) : launch_res_u<0, 1, false>(h, pl, rp);
+    }
+    if (h->L == 64) return launch_res_u<1, 2, false>(h, pl, rp);
+    return launch_res_u<1, 1, false>(h, pl, rp);
 }
 
 int launch_reduce(rfim_pt* h) {

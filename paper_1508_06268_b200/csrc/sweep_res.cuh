@@ -12,6 +12,12 @@
 // straight from L2.  Boundary planes are processed first in every phase, so the neighbour has a
 // whole phase of slack.  All CTAs are co-resident (cooperative launch), hence no deadlock.
 //
+// Inside a CTA there is no barrier between phases either.  Work is cut into warp tasks (phase, 32-row
+// block, class); warps draw task numbers from one shared counter (phase-major), and a task starts as
+// soon as the blocks holding its own plane and its two z-neighbour planes have finished the previous
+// phase (per-block completion counters in shared memory).  A task only ever waits for lower-numbered
+// tasks, so the lowest outstanding task can always run: no deadlock, no tail at the end of a phase.
+//
 // In shared memory a spin is a byte holding 0 or SP (= 8), four same-colour sites per 32-bit word
 // exactly as in global memory (where it is 0/1), so the six-neighbour count of four sites is three
 // IADD3, and count*SP + spin*8*SP [+ field bit] is directly the byte offset of the site's entry in
@@ -33,7 +39,6 @@
 namespace rfim {
 
 constexpr int kResThreads = 512;
-constexpr int kResWarps = kResThreads / 32;
 constexpr uint32_t kResSP = 8;                  // shared-memory spin coding: 0 / SP
 constexpr int kResTabBytes = 256;               // per-replica acceptance table slot (256-byte aligned)
 
@@ -48,6 +53,7 @@ struct ResParams {
     const float* fielda_res;     // Gaussian: [D][2][L][2][4K][L/2] float4 (task order), (float)(hs * g_i)
     const uint8_t* fieldb_res;   // bimodal:  [D][2][L][2][K][L/2] uint4, 0x80 where h_i = +1
     unsigned long long* diag;
+    uint32_t rk0[20];            // Philox round keys of member 0 (used from the constant bank when D == 1)
 };
 
 struct ResPlane {                // 8 bytes per resident plane
@@ -67,7 +73,7 @@ __host__ __device__ inline size_t res_smem_bytes(int L, int cap_planes, int cap_
     size_t b = (size_t)cap_reps * kResTabBytes + (size_t)cap_planes * L * L;
     b += (size_t)cap_reps * sizeof(ResRep);
     b += (size_t)cap_planes * sizeof(ResPlane);
-    b += (size_t)((cap_planes * (L / 2) + 31) / 32) * sizeof(int);       // block order
+    b += (size_t)((cap_planes * (L / 2) + 31) / 32) * 2 * sizeof(int);   // block order, block completion counters
     b += 16;                                                             // counters
     return (b + 15) & ~(size_t)15;
 }
@@ -94,11 +100,13 @@ __device__ __forceinline__ uint32_t prmt(uint32_t a, uint32_t b, uint32_t sel) {
     return r;
 }
 
-// exact rule for the four sites of one word whose table-offset bytes are idx8 = SP*n1 + 8*SP*s (rare)
+// exact rule for the four sites of one word whose table-offset bytes are idx8 = SP*n1 + 8*SP*s (rare: some site
+// of the word fell inside the float path's guard band).  Redraws the word's random numbers.
 __device__ __noinline__ uint32_t res_gauss_word_exact(const View& v, uint32_t idx8, const int32_t* __restrict__ g4, double beta,
-                                                      uint32_t u0, uint32_t u1, uint32_t u2, uint32_t u3) {
+                                                      uint32_t k0, uint32_t k1, uint32_t q, uint32_t sweep, uint32_t slot, uint32_t dom) {
+    const Words4 r = philox4x32_10(k0, k1, q, sweep, slot, dom);
+    const uint32_t u[4] = {r.w0, r.w1, r.w2, r.w3};
     uint32_t flips = 0;
-    const uint32_t u[4] = {u0, u1, u2, u3};
 #pragma unroll
     for (int k = 0; k < 4; ++k) {
         const uint32_t b = (idx8 >> (8 * k)) & 0xFFu;
@@ -106,6 +114,8 @@ __device__ __noinline__ uint32_t res_gauss_word_exact(const View& v, uint32_t id
     }
     return flips;
 }
+
+__device__ __forceinline__ int lds_volatile(const int* p) { return *reinterpret_cast<const volatile int*>(p); }
 
 __device__ __forceinline__ Words4 philox_rkreg(const uint32_t (&rk)[20], uint32_t c0, uint32_t c1, uint32_t c2, uint32_t c3) {
 #pragma unroll
@@ -121,16 +131,16 @@ __device__ __forceinline__ Words4 philox_rkreg(const uint32_t (&rk)[20], uint32_
     return w;
 }
 
-// K = 16-byte pieces per row per colour (L = 32 K)
-template <int KIND, int K, bool NEVER>
-__global__ void __launch_bounds__(kResThreads, 1) k_sweep_res(const View v, const ResParams rp) {
+// K = 16-byte pieces per row per colour (L = 32 K); UNI: one member, round keys come from the constant bank
+template <int KIND, int K, bool NEVER, bool UNI, int THREADS>
+__global__ void __launch_bounds__(THREADS, 1) k_sweep_res(const View v, const ResParams rp) {
     constexpr int L = 32 * K;
     constexpr int LH = L / 2;                   // rows per class per plane
     constexpr int ROWB = 16 * K;                // bytes (= sites) per row per colour
     constexpr int W = 4 * K;                    // words (= Philox calls) per row
     extern __shared__ __align__(1024) uint8_t smem[];
 
-    const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
+    const int tid = threadIdx.x, lane = tid & 31;
     const int b = blockIdx.x;
     const int start = b * rp.q + min(b, rp.rem);
     const int count = rp.q + (b < rp.rem ? 1 : 0);
@@ -138,19 +148,21 @@ __global__ void __launch_bounds__(kResThreads, 1) k_sweep_res(const View v, cons
     const int Ecap = rp.cap_planes * LH;        // rows per (colour, class) array
     const int E = count * LH;                   // rows in use
     const int nb = (E + 31) / 32;               // 32-row blocks per class
+    const int nbcap = (Ecap + 31) / 32;
 
     uint8_t* s_tab = smem;
     uint4* s_sp = reinterpret_cast<uint4*>(smem + (size_t)rp.cap_reps * kResTabBytes);
     ResRep* s_rep = reinterpret_cast<ResRep*>(reinterpret_cast<uint8_t*>(s_sp) + (size_t)rp.cap_planes * L * L);
     ResPlane* s_plane = reinterpret_cast<ResPlane*>(s_rep + rp.cap_reps);
     int* s_order = reinterpret_cast<int*>(s_plane + rp.cap_planes);
-    int* s_ctl = s_order + (Ecap + 31) / 32;    // [0] boundary tasks done (cumulative), [1] boundary blocks
+    int* s_done = s_order + nbcap;              // per block: tasks completed so far (2 per phase)
+    int* s_ctl = s_done + nbcap;                // [0],[1] boundary tasks done in the open even / odd phase, [2] next task number, [3] boundary blocks
     auto A = [&](int col, int s, int k, int e) { return ((col * 2 + s) * K + k) * Ecap + e; };
 
     // ---- set-up: plane table, replica contexts, block order --------------------------------------------
     const int dt0 = start / L;
     const int nrep = (start + count - 1) / L - dt0 + 1;
-    for (int p = tid; p < count; p += kResThreads) {
+    for (int p = tid; p < count; p += THREADS) {
         const int P = start + p, dt = P / L, z = P % L;
         const int Pzp = dt * L + (z + 1 == L ? 0 : z + 1), Pzm = dt * L + (z == 0 ? L - 1 : z - 1);
         auto owner = [&](int Q) {
@@ -167,7 +179,7 @@ __global__ void __launch_bounds__(kResThreads, 1) k_sweep_res(const View v, cons
         pi.z = (uint8_t)z;
         s_plane[p] = pi;
     }
-    for (int r = tid; r < nrep; r += kResThreads) {
+    for (int r = tid; r < nrep; r += THREADS) {
         const int dt = dt0 + r, d = dt / v.n, t = dt % v.n;
         ResRep rr;
         rr.d = d; rr.tr = d * v.R + t; rr.slot = v.t2r[rr.tr]; rr.ds = d * v.R + rr.slot;
@@ -179,7 +191,7 @@ __global__ void __launch_bounds__(kResThreads, 1) k_sweep_res(const View v, cons
         s_rep[r] = rr;
     }
     // acceptance tables, 8-byte entries at byte offset SP*n1 + 8*SP*s (+ 16*SP*hb): Gaussian {x, y}, bimodal {thr-1, never}
-    for (int i = tid; i < nrep * 32; i += kResThreads) {
+    for (int i = tid; i < nrep * 32; i += THREADS) {
         const int r = i >> 5, idx = i & 31;
         const int dt = dt0 + r, d = dt / v.n, t = dt % v.n, tr = d * v.R + t;
         uint2 ent = make_uint2(0u, 0u);
@@ -192,6 +204,7 @@ __global__ void __launch_bounds__(kResThreads, 1) k_sweep_res(const View v, cons
         }
         reinterpret_cast<uint2*>(s_tab + (size_t)r * kResTabBytes)[idx] = ent;
     }
+    for (int i = tid; i < nb; i += THREADS) s_done[i] = 0;
     __syncthreads();
     if (tid == 0) {
         int nbd = 0;
@@ -204,13 +217,13 @@ __global__ void __launch_bounds__(kResThreads, 1) k_sweep_res(const View v, cons
         for (int eb = 0; eb < nb; ++eb) if (is_boundary(eb)) s_order[nbd++] = eb;
         int k = nbd;
         for (int eb = 0; eb < nb; ++eb) if (!is_boundary(eb)) s_order[k++] = eb;
-        s_ctl[0] = 0; s_ctl[1] = nbd;
+        s_ctl[0] = 0; s_ctl[1] = 0; s_ctl[2] = 0; s_ctl[3] = nbd;
     }
 
     // ---- load the run: global [colour][z][y][ROWB] (0/1) -> shared [colour][s][k][row] (0/SP) ------------------
     {
         const int units = count * 2 * L * K;            // 16-byte pieces
-        for (int u = tid; u < units; u += kResThreads) {
+        for (int u = tid; u < units; u += THREADS) {
             const int k = u % K, y = (u / K) % L, col = (u / (K * L)) & 1, p = u / (2 * K * L);
             const ResPlane pi = s_plane[p];
             const int ds = s_rep[pi.rep].ds, z = pi.z;
@@ -221,173 +234,206 @@ __global__ void __launch_bounds__(kResThreads, 1) k_sweep_res(const View v, cons
         }
     }
     __syncthreads();
-    const int n_bblocks = s_ctl[1];
+    const int n_bblocks = s_ctl[3];
     const int n_btasks = 2 * n_bblocks;
+    const int ntasks = 2 * nb;
+    const int total_tasks = ntasks * rp.phases;
     const uint32_t tab0 = (uint32_t)__cvta_generic_to_shared(s_tab);
 
-    // ---- phases ------------------------------------------------------------------------------------
-    for (int p = 0; p < rp.phases; ++p) {
+    // ---- the task flow ------------------------------------------------------------------------------
+    for (;;) {
+        int g = 0;
+        if (lane == 0) g = atomicAdd(&s_ctl[2], 1);
+        g = __shfl_sync(0xFFFFFFFFu, g, 0);
+        if (g >= total_tasks) break;
+        const int p = g / ntasks, task = g - p * ntasks;
         const int c = p & 1, oc = 1 - c;
         const uint32_t sweep = rp.sweep0 + (uint32_t)(p >> 1);
         const uint32_t dom = c == 0 ? kDomColour0 : kDomColour1;
-        for (int task = warp; task < 2 * nb; task += kResWarps) {
-            const int bidx = task >> 1, s = task & 1;
-            const int eb = s_order[bidx];
-            const bool btask = bidx < n_bblocks;
-            const int e_raw = eb * 32 + lane;
-            const bool valid = e_raw < E;
-            const int e = valid ? e_raw : E - 1;
-            const int pl = e / LH, i = e % LH;
-            const ResPlane pi = s_plane[pl];
-            const ResRep* rr = s_rep + pi.rep;
-            const int z = pi.z, ys = (s + z) & 1, y = 2 * i + ys;
-            const int dir = (s + c) & 1;                  // 0: second x-neighbour at xh-1, 1: at xh+1 (warp-uniform)
-            const int ds = rr->ds;
-            const bool remote_p = pi.zp_pl < 0, remote_m = pi.zm_pl < 0;
+        const int bidx = task >> 1, s = task & 1;
+        const int eb = s_order[bidx];
+        const bool btask = bidx < n_bblocks;
+        const int e_raw = eb * 32 + lane;
+        const bool valid = e_raw < E;
+        const int e = valid ? e_raw : E - 1;
+        const int pl = e / LH, i = e % LH;
+        const ResPlane pi = s_plane[pl];
+        const ResRep* rr = s_rep + pi.rep;
+        const int z = pi.z, ys = (s + z) & 1, y = 2 * i + ys;
+        const int dir = (s + c) & 1;                  // 0: second x-neighbour at xh-1, 1: at xh+1 (warp-uniform)
+        const int ds = rr->ds;
+        const bool remote_p = pi.zp_pl < 0, remote_m = pi.zm_pl < 0;
+        const long long blk = (((long long)rr->d * 2 + c) * L + z) * 2 + s;      // field block of this (colour, plane, class)
 
-            // wait until the owners of my remote neighbour planes have published phase p-1
-            if (btask && p > 0) {
-                const uint32_t want = (rp.epoch << 8) | (uint32_t)p;
-                int spins = 0;
-                for (;;) {
-                    bool ok = true;
+        // field of the row: issued first, consumed last
+        float4 fa[W];
+        uint4 fb[K];
+        if (KIND == 0) {
+#pragma unroll
+            for (int k = 0; k < K; ++k) fb[k] = __ldg(reinterpret_cast<const uint4*>(rp.fieldb_res) + (blk * K + k) * LH + i);
+        } else {
+            const float4* fp = reinterpret_cast<const float4*>(rp.fielda_res) + (blk * W) * LH + i;
+#pragma unroll
+            for (int w = 0; w < W; ++w) fa[w] = __ldg(fp + (long long)w * LH);
+        }
+
+        // dependencies: the blocks of my plane and of its z-neighbours have finished phase p-1 (both classes);
+        // remote neighbour planes: their owners have published phase p-1
+        if (p > 0) {
+            const int need = 2 * p;
+            const uint32_t want = (rp.epoch << 8) | (uint32_t)p;
+            const int b_own = eb, b_zp = remote_p ? eb : (pi.zp_pl * LH) >> 5, b_zm = remote_m ? eb : (pi.zm_pl * LH) >> 5;
+            int spins = 0;
+            for (;;) {
+                bool ok = lds_volatile(s_done + b_own) >= need && lds_volatile(s_done + b_zp) >= need && lds_volatile(s_done + b_zm) >= need;
+                if (btask) {
                     if (remote_p) ok = ok && (int32_t)(ld_acquire_gpu(rp.prog + pi.zp_owner) - want) >= 0;
                     if (remote_m) ok = ok && (int32_t)(ld_acquire_gpu(rp.prog + pi.zm_owner) - want) >= 0;
-                    if (__all_sync(0xFFFFFFFFu, ok)) break;
-                    backoff();
-                    if (++spins > (1 << 22)) { if (lane == 0) atomicOr(rp.diag, 1ull); break; }
                 }
+                if (__all_sync(0xFFFFFFFFu, ok)) break;
+                backoff();
+                if (++spins > (1 << 22)) { if (lane == 0) atomicOr(rp.diag, 1ull); break; }
             }
+            __threadfence_block();
+        }
 
-            // ---- neighbour words of the row: t = SP * (number of up neighbours) per byte -----------------------
-            uint32_t cw[W], t[W], me[W];
-            const int e_yp = pl * LH + (ys ? (i + 1 == LH ? 0 : i + 1) : i);
-            const int e_ym = pl * LH + (ys ? i : (i == 0 ? LH - 1 : i - 1));
+        // ---- neighbour words of the row: t = SP * (number of up neighbours) per byte -----------------------
+        uint32_t cw[W], t[W], me[W];
+        const int e_yp = pl * LH + (ys ? (i + 1 == LH ? 0 : i + 1) : i);
+        const int e_ym = pl * LH + (ys ? i : (i == 0 ? LH - 1 : i - 1));
 #pragma unroll
-            for (int k = 0; k < K; ++k) {
-                const uint4 x = s_sp[A(oc, s, k, e)];
-                const uint4 yp = s_sp[A(oc, 1 - s, k, e_yp)];
-                const uint4 ym = s_sp[A(oc, 1 - s, k, e_ym)];
-                uint4 zp, zm;
-                if (!remote_p) zp = s_sp[A(oc, 1 - s, k, pi.zp_pl * LH + i)];
-                else {
-                    const int zq = z + 1 == L ? 0 : z + 1;
-                    zp = ld_cg16(v.spins + ((long long)ds * 2 + oc) * v.Nh + ((long long)zq * L + y) * ROWB + 16 * k);
-                    zp.x *= kResSP; zp.y *= kResSP; zp.z *= kResSP; zp.w *= kResSP;
-                }
-                if (!remote_m) zm = s_sp[A(oc, 1 - s, k, pi.zm_pl * LH + i)];
-                else {
-                    const int zq = z == 0 ? L - 1 : z - 1;
-                    zm = ld_cg16(v.spins + ((long long)ds * 2 + oc) * v.Nh + ((long long)zq * L + y) * ROWB + 16 * k);
-                    zm.x *= kResSP; zm.y *= kResSP; zm.z *= kResSP; zm.w *= kResSP;
-                }
-                const uint4 m = s_sp[A(c, s, k, e)];
-                cw[4 * k + 0] = x.x; cw[4 * k + 1] = x.y; cw[4 * k + 2] = x.z; cw[4 * k + 3] = x.w;
-                t[4 * k + 0] = yp.x + ym.x + zp.x + zm.x; t[4 * k + 1] = yp.y + ym.y + zp.y + zm.y;
-                t[4 * k + 2] = yp.z + ym.z + zp.z + zm.z; t[4 * k + 3] = yp.w + ym.w + zp.w + zm.w;
-                me[4 * k + 0] = m.x; me[4 * k + 1] = m.y; me[4 * k + 2] = m.z; me[4 * k + 3] = m.w;
+        for (int k = 0; k < K; ++k) {
+            const uint4 x = s_sp[A(oc, s, k, e)];
+            const uint4 yp = s_sp[A(oc, 1 - s, k, e_yp)];
+            const uint4 ym = s_sp[A(oc, 1 - s, k, e_ym)];
+            uint4 zp, zm;
+            if (!remote_p) zp = s_sp[A(oc, 1 - s, k, pi.zp_pl * LH + i)];
+            else {
+                const int zq = z + 1 == L ? 0 : z + 1;
+                zp = ld_cg16(v.spins + ((long long)ds * 2 + oc) * v.Nh + ((long long)zq * L + y) * ROWB + 16 * k);
+                zp.x *= kResSP; zp.y *= kResSP; zp.z *= kResSP; zp.w *= kResSP;
             }
-            const long long blk = (((long long)rr->d * 2 + c) * L + z) * 2 + s;      // field block of this (colour, plane, class)
-            if (KIND == 0) {
-#pragma unroll
-                for (int k = 0; k < K; ++k) {
-                    const uint4 f = __ldg(reinterpret_cast<const uint4*>(rp.fieldb_res) + (blk * K + k) * LH + i);
-                    t[4 * k + 0] += f.x; t[4 * k + 1] += f.y; t[4 * k + 2] += f.z; t[4 * k + 3] += f.w;
-                }
+            if (!remote_m) zm = s_sp[A(oc, 1 - s, k, pi.zm_pl * LH + i)];
+            else {
+                const int zq = z == 0 ? L - 1 : z - 1;
+                zm = ld_cg16(v.spins + ((long long)ds * 2 + oc) * v.Nh + ((long long)zq * L + y) * ROWB + 16 * k);
+                zm.x *= kResSP; zm.y *= kResSP; zm.z *= kResSP; zm.w *= kResSP;
             }
-            uint32_t idx8[W];
-            if (dir == 0) {
+            const uint4 m = s_sp[A(c, s, k, e)];
+            cw[4 * k + 0] = x.x; cw[4 * k + 1] = x.y; cw[4 * k + 2] = x.z; cw[4 * k + 3] = x.w;
+            t[4 * k + 0] = yp.x + ym.x + zp.x + zm.x; t[4 * k + 1] = yp.y + ym.y + zp.y + zm.y;
+            t[4 * k + 2] = yp.z + ym.z + zp.z + zm.z; t[4 * k + 3] = yp.w + ym.w + zp.w + zm.w;
+            me[4 * k + 0] = m.x; me[4 * k + 1] = m.y; me[4 * k + 2] = m.z; me[4 * k + 3] = m.w;
+            if (KIND == 0) { t[4 * k + 0] += fb[k].x; t[4 * k + 1] += fb[k].y; t[4 * k + 2] += fb[k].z; t[4 * k + 3] += fb[k].w; }
+        }
+        uint32_t idx8[W];
+        if (dir == 0) {
 #pragma unroll
-                for (int w = 0; w < W; ++w) idx8[w] = t[w] + cw[w] + __funnelshift_r(cw[(w + W - 1) % W], cw[w], 24) + (me[w] << 3);
-            } else {
+            for (int w = 0; w < W; ++w) idx8[w] = t[w] + cw[w] + __funnelshift_r(cw[(w + W - 1) % W], cw[w], 24) + (me[w] << 3);
+        } else {
 #pragma unroll
-                for (int w = 0; w < W; ++w) idx8[w] = t[w] + cw[w] + __funnelshift_r(cw[w], cw[(w + 1) % W], 8) + (me[w] << 3);
-            }
+            for (int w = 0; w < W; ++w) idx8[w] = t[w] + cw[w] + __funnelshift_r(cw[w], cw[(w + 1) % W], 8) + (me[w] << 3);
+        }
 
-            // ---- per-task constants ---------------------------------------------------------------------------
-            uint32_t rk[20];
+        // ---- per-task constants ---------------------------------------------------------------------------
+        uint32_t rk[20];
+        if (UNI) {
+#pragma unroll
+            for (int j = 0; j < 20; ++j) rk[j] = rp.rk0[j];
+        } else {
 #pragma unroll
             for (int j = 0; j < 5; ++j) {
                 const uint4 q4 = reinterpret_cast<const uint4*>(rr->rk)[j];
                 rk[4 * j] = q4.x; rk[4 * j + 1] = q4.y; rk[4 * j + 2] = q4.z; rk[4 * j + 3] = q4.w;
             }
-            const uint32_t slot = (uint32_t)rr->slot;
-            const uint32_t tab_addr = tab0 + (uint32_t)pi.rep * kResTabBytes;
-            const float band = rr->band;
-            const uint32_t q0 = (uint32_t)W * (uint32_t)(y + L * z);
-            const float4* fa = reinterpret_cast<const float4*>(rp.fielda_res) + (blk * W) * LH + i;
+        }
+        const uint32_t slot = (uint32_t)rr->slot;
+        const uint32_t tab_addr = tab0 + (uint32_t)pi.rep * kResTabBytes;
+        const float band = rr->band;
+        const uint32_t q0 = (uint32_t)W * (uint32_t)(y + L * z);
 
-            // ---- the 4K words of the row -------------------------------------------------------------------
+        // ---- the 4K words of the row -------------------------------------------------------------------
+        uint32_t ambmask = 0;
 #pragma unroll
-            for (int w = 0; w < W; ++w) {
-                const Words4 r = philox_rkreg(rk, q0 + (uint32_t)w, sweep, slot, dom);
-                const uint32_t u[4] = {r.w0, r.w1, r.w2, r.w3};
-                uint32_t flips;
-                if (KIND == 0) {
-                    flips = 0;
+        for (int w = 0; w < W; ++w) {
+            const Words4 r = philox_rkreg(rk, q0 + (uint32_t)w, sweep, slot, dom);
+            const uint32_t u[4] = {r.w0, r.w1, r.w2, r.w3};
+            uint32_t flips;
+            if (KIND == 0) {
+                flips = 0;
 #pragma unroll
-                    for (int k = 0; k < 4; ++k) {
-                        const uint2 ent = lds64(__byte_perm(idx8[w], tab_addr, 0x7650 + k));
-                        bool acc = u[k] <= ent.x;
-                        if (NEVER) acc = acc && ent.y == 0u;
-                        if (acc) flips |= kResSP << (8 * k);
-                    }
-                } else {
-                    const float4 a4 = __ldg(fa + (long long)w * LH);
-                    const float a[4] = {a4.x, a4.y, a4.z, a4.w};
-                    uint32_t db[4];
-                    bool amb = false;
-#pragma unroll
-                    for (int k = 0; k < 4; ++k) {
-                        const uint2 ent = lds64(__byte_perm(idx8[w], tab_addr, 0x7650 + k));
-                        const float P = ex2_approx(fmaf(a[k], __uint_as_float(ent.y), __uint_as_float(ent.x)));
-                        const float d = __uint2float_rn(u[k]) - P;
-                        amb = amb || (fabsf(d) < band);
-                        db[k] = __float_as_uint(d);
-                    }
-                    // sign bytes of the four differences -> 0xFF where d < 0 (accept)
-                    const uint32_t m01 = prmt(db[0], db[1], 0x00FBu);
-                    const uint32_t m23 = prmt(db[2], db[3], 0xFB00u);
-                    flips = prmt(m01, m23, 0x7610u) & (kResSP * 0x01010101u);
-                    if (amb) {
-                        const int32_t* g4 = v.fieldg + ((long long)rr->d * 2 + c) * v.Nh + ((long long)z * L + y) * ROWB + 4 * w;
-                        flips = res_gauss_word_exact(v, idx8[w], g4, rr->beta, u[0], u[1], u[2], u[3]);
-                    }
+                for (int k = 0; k < 4; ++k) {
+                    const uint2 ent = lds64(__byte_perm(idx8[w], tab_addr, 0x7650 + k));
+                    bool acc = u[k] <= ent.x;
+                    if (NEVER) acc = acc && ent.y == 0u;
+                    if (acc) flips |= kResSP << (8 * k);
                 }
-                me[w] ^= flips;
+            } else {
+                const float a[4] = {fa[w].x, fa[w].y, fa[w].z, fa[w].w};
+                uint32_t db[4];
+                bool amb = false;
+#pragma unroll
+                for (int k = 0; k < 4; ++k) {
+                    const uint2 ent = lds64(__byte_perm(idx8[w], tab_addr, 0x7650 + k));
+                    const float P = ex2_approx(fmaf(a[k], __uint_as_float(ent.y), __uint_as_float(ent.x)));
+                    const float d = __uint2float_rn(u[k]) - P;
+                    amb = amb || (fabsf(d) < band);
+                    db[k] = __float_as_uint(d);
+                }
+                // sign bytes of the four differences -> 0xFF where d < 0 (accept)
+                const uint32_t m01 = prmt(db[0], db[1], 0x00FBu);
+                const uint32_t m23 = prmt(db[2], db[3], 0xFB00u);
+                flips = prmt(m01, m23, 0x7610u) & (kResSP * 0x01010101u);
+                if (amb) ambmask |= 1u << w;
             }
+            me[w] ^= flips;
+        }
+        if (KIND == 1 && ambmask != 0u) {               // rare: redo the flagged words with the exact binary64 rule
+            const int32_t* grow = v.fieldg + ((long long)rr->d * 2 + c) * v.Nh + ((long long)z * L + y) * ROWB;
+            const double beta = rr->beta;
+#pragma unroll
+            for (int w = 0; w < W; ++w)
+                if ((ambmask >> w) & 1u)
+                    me[w] = ((idx8[w] >> 3) & (kResSP * 0x01010101u)) ^
+                            res_gauss_word_exact(v, idx8[w], grow + 4 * w, beta, rr->rk[0], rr->rk[1], q0 + (uint32_t)w, sweep, slot, dom);
+        }
 
-            // ---- write back -----------------------------------------------------------------------------------
-            if (valid) {
+        // ---- write back -----------------------------------------------------------------------------------
+        if (valid) {
+#pragma unroll
+            for (int k = 0; k < K; ++k)
+                s_sp[A(c, s, k, e)] = make_uint4(me[4 * k], me[4 * k + 1], me[4 * k + 2], me[4 * k + 3]);
+            if (remote_p || remote_m) {
+                uint8_t* dst = v.spins + ((long long)ds * 2 + c) * v.Nh + ((long long)z * L + y) * ROWB;
 #pragma unroll
                 for (int k = 0; k < K; ++k)
-                    s_sp[A(c, s, k, e)] = make_uint4(me[4 * k], me[4 * k + 1], me[4 * k + 2], me[4 * k + 3]);
-                if (remote_p || remote_m) {
-                    uint8_t* dst = v.spins + ((long long)ds * 2 + c) * v.Nh + ((long long)z * L + y) * ROWB;
-#pragma unroll
-                    for (int k = 0; k < K; ++k)
-                        *reinterpret_cast<uint4*>(dst + 16 * k) = make_uint4(me[4 * k] >> 3, me[4 * k + 1] >> 3, me[4 * k + 2] >> 3, me[4 * k + 3] >> 3);
-                }
-            }
-            if (btask) {
-                __syncwarp();
-                if (lane == 0) {
-                    __threadfence();
-                    const int done = atomicAdd(&s_ctl[0], 1) + 1;
-                    if (done == n_btasks * (p + 1)) {
-                        __threadfence();
-                        st_release_gpu(rp.prog + b, (rp.epoch << 8) | (uint32_t)(p + 1));
-                    }
-                }
+                    *reinterpret_cast<uint4*>(dst + 16 * k) = make_uint4(me[4 * k] >> 3, me[4 * k + 1] >> 3, me[4 * k + 2] >> 3, me[4 * k + 3] >> 3);
             }
         }
-        __syncthreads();
+        __syncwarp();
+        if (lane == 0) {
+            if (btask) {
+                // a neighbour CTA only needs phase p+1 of mine after it has seen phase p published, and it publishes
+                // its own phase p+1 only after that: at most two phases are open at once, one counter per parity
+                __threadfence();
+                const int done = atomicAdd(&s_ctl[p & 1], 1) + 1;
+                if (done == n_btasks) {
+                    atomicExch(&s_ctl[p & 1], 0);
+                    __threadfence();
+                    st_release_gpu(rp.prog + b, (rp.epoch << 8) | (uint32_t)(p + 1));
+                }
+            } else {
+                __threadfence_block();
+            }
+            atomicAdd(&s_done[eb], 1);
+        }
     }
+    __syncthreads();
 
     // ---- store the run back ------------------------------------------------------------------------------
     {
         const int units = count * 2 * L * K;
-        for (int u = tid; u < units; u += kResThreads) {
+        for (int u = tid; u < units; u += THREADS) {
             const int k = u % K, y = (u / K) % L, col = (u / (K * L)) & 1, p = u / (2 * K * L);
             const ResPlane pi = s_plane[p];
             const int ds = s_rep[pi.rep].ds, z = pi.z;
