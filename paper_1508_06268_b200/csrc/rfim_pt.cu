@@ -408,11 +408,12 @@ int launch_res_u(rfim_pt* h, const ResPlan& pl, const ResParams& rp) {
 }
 
 // `sweeps` (<= 127) sweeps of every active replica of every member in one cooperative launch
-int launch_res(rfim_pt* h, int sweeps) {
+int launch_res(rfim_pt* h, int sweeps, bool measure) {
     const ResPlan pl = res_plan(h);
     if (!pl.ok) return fail(h, RFIM_EINVAL, "resident kernel: the planes of one CTA do not fit in shared memory");
     ResParams rp{};
     rp.phases = 2 * sweeps;
+    rp.measure = measure ? 1 : 0;
     rp.sweep0 = (uint32_t)h->sweep_g;
     rp.epoch = ++h->res_epoch;
     rp.prog = h->res_prog;
@@ -467,12 +468,14 @@ int do_sweeps(rfim_pt* h, int64_t n_sweeps, int k) {
             chunk = std::min<int64_t>(left, 127);
             if (k > 0) chunk = std::min<int64_t>(chunk, (int64_t)k - (int64_t)(h->sweep_g % (uint64_t)k));
         }
-        int rc = variant == 4 ? launch_res(h, (int)chunk) : (flow ? launch_flow(h, (int)chunk) : launch_sweep(h));
+        // the resident kernel measures in the same launch when its chunk ends on an exchange step
+        const bool step_after = k > 0 && ((h->sweep_g + (uint64_t)chunk) % (uint64_t)k) == 0;
+        int rc = variant == 4 ? launch_res(h, (int)chunk, step_after) : (flow ? launch_flow(h, (int)chunk) : launch_sweep(h));
         if (rc) return rc;
         h->sweep_g += (uint64_t)chunk;
         left -= chunk;
-        if (k > 0 && (h->sweep_g % (uint64_t)k) == 0) {
-            if ((rc = launch_reduce(h))) return rc;
+        if (step_after) {
+            if (variant != 4 && (rc = launch_reduce(h))) return rc;
             if ((rc = launch_exchange(h))) return rc;
             h->series_steps += 1;
             h->xstep += 1;

@@ -13,10 +13,16 @@
 // whole phase of slack.  All CTAs are co-resident (cooperative launch), hence no deadlock.
 //
 // Inside a CTA there is no barrier between phases either.  Work is cut into warp tasks (phase, 32-row
-// block, class); warps draw task numbers from one shared counter (phase-major), and a task starts as
-// soon as the blocks holding its own plane and its two z-neighbour planes have finished the previous
-// phase (per-block completion counters in shared memory).  A task only ever waits for lower-numbered
-// tasks, so the lowest outstanding task can always run: no deadlock, no tail at the end of a phase.
+// block: both checkerboard classes of those rows); warps draw task numbers from one shared counter
+// (phase-major), and a task starts as soon as the blocks holding its own plane and its two z-neighbour
+// planes have finished the previous phase (per-block completion counters in shared memory).  A task
+// only ever waits for lower-numbered tasks, so the lowest outstanding task can always run: no
+// deadlock, no tail at the end of a phase.
+//
+// Measurement (S5) is one more pseudo-phase of colour 0 at the end of the launch: the same
+// neighbour words give Eb = sum over colour-0 sites of s_i * (six-neighbour sum), Msum and Ef are
+// summed over both colours of the row, per replica in shared memory, then added to View::acc with
+// integer atomics (order-independent, hence deterministic).
 //
 // In shared memory a spin is a byte holding 0 or SP (= 8), four same-colour sites per 32-bit word
 // exactly as in global memory (where it is 0/1), so the six-neighbour count of four sites is three
@@ -44,6 +50,7 @@ constexpr int kResTabBytes = 256;               // per-replica acceptance table 
 
 struct ResParams {
     int phases;                  // 2 * sweeps of this launch, <= 254
+    int measure;                 // != 0: finish with the measurement pseudo-phase (Eb, Ef, Msum -> View::acc)
     uint32_t sweep0;             // global sweep index of phase 0
     uint32_t epoch;              // launch id: progress words hold (epoch << 8) | phases published
     uint32_t* prog;              // [grid]
@@ -75,6 +82,7 @@ __host__ __device__ inline size_t res_smem_bytes(int L, int cap_planes, int cap_
     b += (size_t)cap_planes * sizeof(ResPlane);
     b += (size_t)((cap_planes * (L / 2) + 31) / 32) * 2 * sizeof(int);   // block order, block completion counters
     b += 16;                                                             // counters
+    b += (size_t)cap_reps * 3 * sizeof(long long);                       // measurement accumulators
     return (b + 15) & ~(size_t)15;
 }
 
@@ -147,7 +155,7 @@ __global__ void __launch_bounds__(THREADS, 1) k_sweep_res(const View v, const Re
     if (count == 0) return;
     const int Ecap = rp.cap_planes * LH;        // rows per (colour, class) array
     const int E = count * LH;                   // rows in use
-    const int nb = (E + 31) / 32;               // 32-row blocks per class
+    const int nb = (E + 31) / 32;               // 32-row blocks
     const int nbcap = (Ecap + 31) / 32;
 
     uint8_t* s_tab = smem;
@@ -155,8 +163,9 @@ __global__ void __launch_bounds__(THREADS, 1) k_sweep_res(const View v, const Re
     ResRep* s_rep = reinterpret_cast<ResRep*>(reinterpret_cast<uint8_t*>(s_sp) + (size_t)rp.cap_planes * L * L);
     ResPlane* s_plane = reinterpret_cast<ResPlane*>(s_rep + rp.cap_reps);
     int* s_order = reinterpret_cast<int*>(s_plane + rp.cap_planes);
-    int* s_done = s_order + nbcap;              // per block: tasks completed so far (2 per phase)
+    int* s_done = s_order + nbcap;              // per block: tasks completed so far (one per phase)
     int* s_ctl = s_done + nbcap;                // [0],[1] boundary tasks done in the open even / odd phase, [2] next task number, [3] boundary blocks
+    long long* s_acc = reinterpret_cast<long long*>(s_ctl + 4);   // [rep][3] measurement accumulators
     auto A = [&](int col, int s, int k, int e) { return ((col * 2 + s) * K + k) * Ecap + e; };
 
     // ---- set-up: plane table, replica contexts, block order --------------------------------------------
@@ -189,6 +198,7 @@ __global__ void __launch_bounds__(THREADS, 1) k_sweep_res(const View v, const Re
         uint32_t k0 = v.keys[2 * d], k1 = v.keys[2 * d + 1];
         for (int i = 0; i < 10; ++i) { rr.rk[2 * i] = k0; rr.rk[2 * i + 1] = k1; k0 += kPhiloxW0; k1 += kPhiloxW1; }
         s_rep[r] = rr;
+        s_acc[3 * r] = 0; s_acc[3 * r + 1] = 0; s_acc[3 * r + 2] = 0;
     }
     // acceptance tables, 8-byte entries at byte offset SP*n1 + 8*SP*s (+ 16*SP*hb): Gaussian {x, y}, bimodal {thr-1, never}
     for (int i = tid; i < nrep * 32; i += THREADS) {
@@ -235,9 +245,7 @@ __global__ void __launch_bounds__(THREADS, 1) k_sweep_res(const View v, const Re
     }
     __syncthreads();
     const int n_bblocks = s_ctl[3];
-    const int n_btasks = 2 * n_bblocks;
-    const int ntasks = 2 * nb;
-    const int total_tasks = ntasks * rp.phases;
+    const int total_tasks = nb * (rp.phases + (rp.measure ? 1 : 0));
     const uint32_t tab0 = (uint32_t)__cvta_generic_to_shared(s_tab);
 
     // ---- the task flow ------------------------------------------------------------------------------
@@ -246,11 +254,11 @@ __global__ void __launch_bounds__(THREADS, 1) k_sweep_res(const View v, const Re
         if (lane == 0) g = atomicAdd(&s_ctl[2], 1);
         g = __shfl_sync(0xFFFFFFFFu, g, 0);
         if (g >= total_tasks) break;
-        const int p = g / ntasks, task = g - p * ntasks;
+        const int p = g / nb, bidx = g - p * nb;
+        const bool meas = p == rp.phases;             // the measurement pseudo-phase (colour 0; phases is even)
         const int c = p & 1, oc = 1 - c;
         const uint32_t sweep = rp.sweep0 + (uint32_t)(p >> 1);
         const uint32_t dom = c == 0 ? kDomColour0 : kDomColour1;
-        const int bidx = task >> 1, s = task & 1;
         const int eb = s_order[bidx];
         const bool btask = bidx < n_bblocks;
         const int e_raw = eb * 32 + lane;
@@ -259,156 +267,230 @@ __global__ void __launch_bounds__(THREADS, 1) k_sweep_res(const View v, const Re
         const int pl = e / LH, i = e % LH;
         const ResPlane pi = s_plane[pl];
         const ResRep* rr = s_rep + pi.rep;
-        const int z = pi.z, ys = (s + z) & 1, y = 2 * i + ys;
-        const int dir = (s + c) & 1;                  // 0: second x-neighbour at xh-1, 1: at xh+1 (warp-uniform)
+        const int z = pi.z;
         const int ds = rr->ds;
         const bool remote_p = pi.zp_pl < 0, remote_m = pi.zm_pl < 0;
-        const long long blk = (((long long)rr->d * 2 + c) * L + z) * 2 + s;      // field block of this (colour, plane, class)
+        const int e_zp = remote_p ? 0 : pi.zp_pl * LH + i, e_zm = remote_m ? 0 : pi.zm_pl * LH + i;
+        const int zq_p = z + 1 == L ? 0 : z + 1, zq_m = z == 0 ? L - 1 : z - 1;
+        long long m_eb = 0, m_ef = 0, m_ms = 0;
 
-        // field of the row: issued first, consumed last
-        float4 fa[W];
-        uint4 fb[K];
-        if (KIND == 0) {
-#pragma unroll
-            for (int k = 0; k < K; ++k) fb[k] = __ldg(reinterpret_cast<const uint4*>(rp.fieldb_res) + (blk * K + k) * LH + i);
-        } else {
-            const float4* fp = reinterpret_cast<const float4*>(rp.fielda_res) + (blk * W) * LH + i;
-#pragma unroll
-            for (int w = 0; w < W; ++w) fa[w] = __ldg(fp + (long long)w * LH);
-        }
+#pragma unroll 1
+        for (int s = 0; s < 2; ++s) {
+            const int ys = (s + z) & 1, y = 2 * i + ys;
+            const int dir = (s + c) & 1;              // 0: second x-neighbour at xh-1, 1: at xh+1 (warp-uniform)
+            const long long blk = (((long long)rr->d * 2 + c) * L + z) * 2 + s;  // field block of this (colour, plane, class)
 
-        // dependencies: the blocks of my plane and of its z-neighbours have finished phase p-1 (both classes);
-        // remote neighbour planes: their owners have published phase p-1
-        if (p > 0) {
-            const int need = 2 * p;
-            const uint32_t want = (rp.epoch << 8) | (uint32_t)p;
-            const int b_own = eb, b_zp = remote_p ? eb : (pi.zp_pl * LH) >> 5, b_zm = remote_m ? eb : (pi.zm_pl * LH) >> 5;
-            int spins = 0;
-            for (;;) {
-                bool ok = lds_volatile(s_done + b_own) >= need && lds_volatile(s_done + b_zp) >= need && lds_volatile(s_done + b_zm) >= need;
-                if (btask) {
-                    if (remote_p) ok = ok && (int32_t)(ld_acquire_gpu(rp.prog + pi.zp_owner) - want) >= 0;
-                    if (remote_m) ok = ok && (int32_t)(ld_acquire_gpu(rp.prog + pi.zm_owner) - want) >= 0;
-                }
-                if (__all_sync(0xFFFFFFFFu, ok)) break;
-                backoff();
-                if (++spins > (1 << 22)) { if (lane == 0) atomicOr(rp.diag, 1ull); break; }
-            }
-            __threadfence_block();
-        }
-
-        // ---- neighbour words of the row: t = SP * (number of up neighbours) per byte -----------------------
-        uint32_t cw[W], t[W], me[W];
-        const int e_yp = pl * LH + (ys ? (i + 1 == LH ? 0 : i + 1) : i);
-        const int e_ym = pl * LH + (ys ? i : (i == 0 ? LH - 1 : i - 1));
-#pragma unroll
-        for (int k = 0; k < K; ++k) {
-            const uint4 x = s_sp[A(oc, s, k, e)];
-            const uint4 yp = s_sp[A(oc, 1 - s, k, e_yp)];
-            const uint4 ym = s_sp[A(oc, 1 - s, k, e_ym)];
-            uint4 zp, zm;
-            if (!remote_p) zp = s_sp[A(oc, 1 - s, k, pi.zp_pl * LH + i)];
-            else {
-                const int zq = z + 1 == L ? 0 : z + 1;
-                zp = ld_cg16(v.spins + ((long long)ds * 2 + oc) * v.Nh + ((long long)zq * L + y) * ROWB + 16 * k);
-                zp.x *= kResSP; zp.y *= kResSP; zp.z *= kResSP; zp.w *= kResSP;
-            }
-            if (!remote_m) zm = s_sp[A(oc, 1 - s, k, pi.zm_pl * LH + i)];
-            else {
-                const int zq = z == 0 ? L - 1 : z - 1;
-                zm = ld_cg16(v.spins + ((long long)ds * 2 + oc) * v.Nh + ((long long)zq * L + y) * ROWB + 16 * k);
-                zm.x *= kResSP; zm.y *= kResSP; zm.z *= kResSP; zm.w *= kResSP;
-            }
-            const uint4 m = s_sp[A(c, s, k, e)];
-            cw[4 * k + 0] = x.x; cw[4 * k + 1] = x.y; cw[4 * k + 2] = x.z; cw[4 * k + 3] = x.w;
-            t[4 * k + 0] = yp.x + ym.x + zp.x + zm.x; t[4 * k + 1] = yp.y + ym.y + zp.y + zm.y;
-            t[4 * k + 2] = yp.z + ym.z + zp.z + zm.z; t[4 * k + 3] = yp.w + ym.w + zp.w + zm.w;
-            me[4 * k + 0] = m.x; me[4 * k + 1] = m.y; me[4 * k + 2] = m.z; me[4 * k + 3] = m.w;
-            if (KIND == 0) { t[4 * k + 0] += fb[k].x; t[4 * k + 1] += fb[k].y; t[4 * k + 2] += fb[k].z; t[4 * k + 3] += fb[k].w; }
-        }
-        uint32_t idx8[W];
-        if (dir == 0) {
-#pragma unroll
-            for (int w = 0; w < W; ++w) idx8[w] = t[w] + cw[w] + __funnelshift_r(cw[(w + W - 1) % W], cw[w], 24) + (me[w] << 3);
-        } else {
-#pragma unroll
-            for (int w = 0; w < W; ++w) idx8[w] = t[w] + cw[w] + __funnelshift_r(cw[w], cw[(w + 1) % W], 8) + (me[w] << 3);
-        }
-
-        // ---- per-task constants ---------------------------------------------------------------------------
-        uint32_t rk[20];
-        if (UNI) {
-#pragma unroll
-            for (int j = 0; j < 20; ++j) rk[j] = rp.rk0[j];
-        } else {
-#pragma unroll
-            for (int j = 0; j < 5; ++j) {
-                const uint4 q4 = reinterpret_cast<const uint4*>(rr->rk)[j];
-                rk[4 * j] = q4.x; rk[4 * j + 1] = q4.y; rk[4 * j + 2] = q4.z; rk[4 * j + 3] = q4.w;
-            }
-        }
-        const uint32_t slot = (uint32_t)rr->slot;
-        const uint32_t tab_addr = tab0 + (uint32_t)pi.rep * kResTabBytes;
-        const float band = rr->band;
-        const uint32_t q0 = (uint32_t)W * (uint32_t)(y + L * z);
-
-        // ---- the 4K words of the row -------------------------------------------------------------------
-        uint32_t ambmask = 0;
-#pragma unroll
-        for (int w = 0; w < W; ++w) {
-            const Words4 r = philox_rkreg(rk, q0 + (uint32_t)w, sweep, slot, dom);
-            const uint32_t u[4] = {r.w0, r.w1, r.w2, r.w3};
-            uint32_t flips;
+            // field of the row: issued first, consumed last
+            float4 fa[W];
+            uint4 fb[K];
             if (KIND == 0) {
-                flips = 0;
 #pragma unroll
-                for (int k = 0; k < 4; ++k) {
-                    const uint2 ent = lds64(__byte_perm(idx8[w], tab_addr, 0x7650 + k));
-                    bool acc = u[k] <= ent.x;
-                    if (NEVER) acc = acc && ent.y == 0u;
-                    if (acc) flips |= kResSP << (8 * k);
-                }
-            } else {
-                const float a[4] = {fa[w].x, fa[w].y, fa[w].z, fa[w].w};
-                uint32_t db[4];
-                bool amb = false;
+                for (int k = 0; k < K; ++k) fb[k] = __ldg(reinterpret_cast<const uint4*>(rp.fieldb_res) + (blk * K + k) * LH + i);
+            } else if (!meas) {
+                const float4* fp = reinterpret_cast<const float4*>(rp.fielda_res) + (blk * W) * LH + i;
 #pragma unroll
-                for (int k = 0; k < 4; ++k) {
-                    const uint2 ent = lds64(__byte_perm(idx8[w], tab_addr, 0x7650 + k));
-                    const float P = ex2_approx(fmaf(a[k], __uint_as_float(ent.y), __uint_as_float(ent.x)));
-                    const float d = __uint2float_rn(u[k]) - P;
-                    amb = amb || (fabsf(d) < band);
-                    db[k] = __float_as_uint(d);
-                }
-                // sign bytes of the four differences -> 0xFF where d < 0 (accept)
-                const uint32_t m01 = prmt(db[0], db[1], 0x00FBu);
-                const uint32_t m23 = prmt(db[2], db[3], 0xFB00u);
-                flips = prmt(m01, m23, 0x7610u) & (kResSP * 0x01010101u);
-                if (amb) ambmask |= 1u << w;
+                for (int w = 0; w < W; ++w) fa[w] = __ldg(fp + (long long)w * LH);
             }
-            me[w] ^= flips;
-        }
-        if (KIND == 1 && ambmask != 0u) {               // rare: redo the flagged words with the exact binary64 rule
-            const int32_t* grow = v.fieldg + ((long long)rr->d * 2 + c) * v.Nh + ((long long)z * L + y) * ROWB;
-            const double beta = rr->beta;
-#pragma unroll
-            for (int w = 0; w < W; ++w)
-                if ((ambmask >> w) & 1u)
-                    me[w] = ((idx8[w] >> 3) & (kResSP * 0x01010101u)) ^
-                            res_gauss_word_exact(v, idx8[w], grow + 4 * w, beta, rr->rk[0], rr->rk[1], q0 + (uint32_t)w, sweep, slot, dom);
-        }
 
-        // ---- write back -----------------------------------------------------------------------------------
-        if (valid) {
+            // dependencies: the blocks of my plane and of its z-neighbours have finished phase p-1;
+            // remote neighbour planes: their owners have published phase p-1
+            if (s == 0 && p > 0) {
+                const uint32_t want = (rp.epoch << 8) | (uint32_t)p;
+                const int b_zp = remote_p ? eb : e_zp >> 5, b_zm = remote_m ? eb : e_zm >> 5;
+                int spins = 0;
+                for (;;) {
+                    bool ok = lds_volatile(s_done + eb) >= p && lds_volatile(s_done + b_zp) >= p && lds_volatile(s_done + b_zm) >= p;
+                    if (btask) {
+                        if (remote_p) ok = ok && (int32_t)(ld_acquire_gpu(rp.prog + pi.zp_owner) - want) >= 0;
+                        if (remote_m) ok = ok && (int32_t)(ld_acquire_gpu(rp.prog + pi.zm_owner) - want) >= 0;
+                    }
+                    if (__all_sync(0xFFFFFFFFu, ok)) break;
+                    backoff();
+                    if (++spins > (1 << 22)) { if (lane == 0) atomicOr(rp.diag, 1ull); break; }
+                }
+                __threadfence_block();
+            }
+
+            // ---- neighbour words of the row: t = SP * (number of up neighbours) per byte -----------------------
+            uint32_t cw[W], t[W], me[W];
+            const int e_yp = pl * LH + (ys ? (i + 1 == LH ? 0 : i + 1) : i);
+            const int e_ym = pl * LH + (ys ? i : (i == 0 ? LH - 1 : i - 1));
 #pragma unroll
-            for (int k = 0; k < K; ++k)
-                s_sp[A(c, s, k, e)] = make_uint4(me[4 * k], me[4 * k + 1], me[4 * k + 2], me[4 * k + 3]);
-            if (remote_p || remote_m) {
-                uint8_t* dst = v.spins + ((long long)ds * 2 + c) * v.Nh + ((long long)z * L + y) * ROWB;
+            for (int k = 0; k < K; ++k) {
+                const uint4 x = s_sp[A(oc, s, k, e)];
+                const uint4 yp = s_sp[A(oc, 1 - s, k, e_yp)];
+                const uint4 ym = s_sp[A(oc, 1 - s, k, e_ym)];
+                uint4 zp, zm;
+                if (!remote_p) zp = s_sp[A(oc, 1 - s, k, e_zp)];
+                else {
+                    zp = ld_cg16(v.spins + ((long long)ds * 2 + oc) * v.Nh + ((long long)zq_p * L + y) * ROWB + 16 * k);
+                    zp.x *= kResSP; zp.y *= kResSP; zp.z *= kResSP; zp.w *= kResSP;
+                }
+                if (!remote_m) zm = s_sp[A(oc, 1 - s, k, e_zm)];
+                else {
+                    zm = ld_cg16(v.spins + ((long long)ds * 2 + oc) * v.Nh + ((long long)zq_m * L + y) * ROWB + 16 * k);
+                    zm.x *= kResSP; zm.y *= kResSP; zm.z *= kResSP; zm.w *= kResSP;
+                }
+                const uint4 m = s_sp[A(c, s, k, e)];
+                cw[4 * k + 0] = x.x; cw[4 * k + 1] = x.y; cw[4 * k + 2] = x.z; cw[4 * k + 3] = x.w;
+                t[4 * k + 0] = yp.x + ym.x + zp.x + zm.x; t[4 * k + 1] = yp.y + ym.y + zp.y + zm.y;
+                t[4 * k + 2] = yp.z + ym.z + zp.z + zm.z; t[4 * k + 3] = yp.w + ym.w + zp.w + zm.w;
+                me[4 * k + 0] = m.x; me[4 * k + 1] = m.y; me[4 * k + 2] = m.z; me[4 * k + 3] = m.w;
+            }
+            uint32_t ns[W];                           // SP * (number of up neighbours) per byte
+            if (dir == 0) {
+#pragma unroll
+                for (int w = 0; w < W; ++w) ns[w] = t[w] + cw[w] + __funnelshift_r(cw[(w + W - 1) % W], cw[w], 24);
+            } else {
+#pragma unroll
+                for (int w = 0; w < W; ++w) ns[w] = t[w] + cw[w] + __funnelshift_r(cw[w], cw[(w + 1) % W], 8);
+            }
+
+            if (meas) {
+                // ---- measurement: Eb over this colour-0 row, Msum and Ef over both colours of the row ------------
+                if (valid) {
+                    int sn = 0, s0 = 0, nn = 0, s1 = 0;   // 64 sum s0 n1, 8 sum s0, 8 sum n1, 8 sum s1
+#pragma unroll
+                    for (int w = 0; w < W; ++w) {
+                        sn += dot4(me[w], ns[w]); s0 += dot4(me[w], 0x01010101u);
+                        nn += dot4(ns[w], 0x01010101u); s1 += dot4(cw[w], 0x01010101u);
+                    }
+                    // sum (2 s0 - 1)(2 n1 - 6) = 4 s0.n1 - 12 s0 - 2 n1 + 6 per site
+                    m_eb += sn / 16 - 12 * (s0 / 8) - 2 * (nn / 8) + 6 * ROWB;
+                    m_ms += 2 * ((s0 + s1) / 8) - 2 * ROWB;
+                    const long long rowoff = ((long long)z * L + y) * ROWB;
+                    if (KIND == 0) {
+                        // sum (2 hb - 1)(2 s - 1) = 4 hb.s - 2 hb - 2 s + 1 per site; hb = 0x10 flags in natural colour order
+                        const uint32_t* h0 = reinterpret_cast<const uint32_t*>(v.fieldb + ((long long)rr->d * 2 + 0) * v.Nh + rowoff);
+                        const uint32_t* h1 = reinterpret_cast<const uint32_t*>(v.fieldb + ((long long)rr->d * 2 + 1) * v.Nh + rowoff);
+                        int hs0 = 0, hh = 0;
+#pragma unroll
+                        for (int w = 0; w < W; ++w) {
+                            const uint32_t a0 = __ldg(h0 + w) >> 4, a1 = __ldg(h1 + w) >> 4;   // 0/1 per byte
+                            hs0 += dot4(a0, me[w]) + dot4(a1, cw[w]);                         // 8 sum hb s
+                            hh += dot4(a0, 0x01010101u) + dot4(a1, 0x01010101u);
+                        }
+                        m_ef += 4 * (hs0 / 8) - 2 * hh - 2 * ((s0 + s1) / 8) + 2 * ROWB;
+                    } else {
+                        const int32_t* g0 = v.fieldg + ((long long)rr->d * 2 + 0) * v.Nh + rowoff;
+                        const int32_t* g1 = v.fieldg + ((long long)rr->d * 2 + 1) * v.Nh + rowoff;
+                        long long ef = 0;
+#pragma unroll
+                        for (int w = 0; w < W; ++w) {
+                            const int4 a0 = __ldg(reinterpret_cast<const int4*>(g0) + w), a1 = __ldg(reinterpret_cast<const int4*>(g1) + w);
+                            const int ga[4] = {a0.x, a0.y, a0.z, a0.w}, gb[4] = {a1.x, a1.y, a1.z, a1.w};
+                            int part = 0;                 // |g| <= 2^23: eight terms fit easily
+#pragma unroll
+                            for (int k = 0; k < 4; ++k) {
+                                part += ((me[w] >> (8 * k)) & kResSP) ? ga[k] : -ga[k];
+                                part += ((cw[w] >> (8 * k)) & kResSP) ? gb[k] : -gb[k];
+                            }
+                            ef += part;
+                        }
+                        m_ef += ef;
+                    }
+                }
+                continue;
+            }
+
+            uint32_t idx8[W];
+#pragma unroll
+            for (int w = 0; w < W; ++w) idx8[w] = ns[w] + (me[w] << 3) + (KIND == 0 ? reinterpret_cast<const uint32_t*>(fb)[w] : 0u);
+
+            // ---- per-task constants ---------------------------------------------------------------------------
+            uint32_t rk[20];
+            if (UNI) {
+#pragma unroll
+                for (int j = 0; j < 20; ++j) rk[j] = rp.rk0[j];
+            } else {
+#pragma unroll
+                for (int j = 0; j < 5; ++j) {
+                    const uint4 q4 = reinterpret_cast<const uint4*>(rr->rk)[j];
+                    rk[4 * j] = q4.x; rk[4 * j + 1] = q4.y; rk[4 * j + 2] = q4.z; rk[4 * j + 3] = q4.w;
+                }
+            }
+            const uint32_t slot = (uint32_t)rr->slot;
+            const uint32_t tab_addr = tab0 + (uint32_t)pi.rep * kResTabBytes;
+            const float band = rr->band;
+            const uint32_t q0 = (uint32_t)W * (uint32_t)(y + L * z);
+
+            // ---- the 4K words of the row -------------------------------------------------------------------
+            uint32_t ambmask = 0;
+#pragma unroll
+            for (int w = 0; w < W; ++w) {
+                const Words4 r = philox_rkreg(rk, q0 + (uint32_t)w, sweep, slot, dom);
+                const uint32_t u[4] = {r.w0, r.w1, r.w2, r.w3};
+                uint32_t flips;
+                if (KIND == 0) {
+                    flips = 0;
+#pragma unroll
+                    for (int k = 0; k < 4; ++k) {
+                        const uint2 ent = lds64(__byte_perm(idx8[w], tab_addr, 0x7650 + k));
+                        bool acc = u[k] <= ent.x;
+                        if (NEVER) acc = acc && ent.y == 0u;
+                        if (acc) flips |= kResSP << (8 * k);
+                    }
+                } else {
+                    const float a[4] = {fa[w].x, fa[w].y, fa[w].z, fa[w].w};
+                    uint32_t db[4];
+                    bool amb = false;
+#pragma unroll
+                    for (int k = 0; k < 4; ++k) {
+                        const uint2 ent = lds64(__byte_perm(idx8[w], tab_addr, 0x7650 + k));
+                        const float P = ex2_approx(fmaf(a[k], __uint_as_float(ent.y), __uint_as_float(ent.x)));
+                        const float d = __uint2float_rn(u[k]) - P;
+                        amb = amb || (fabsf(d) < band);
+                        db[k] = __float_as_uint(d);
+                    }
+                    // sign bytes of the four differences -> 0xFF where d < 0 (accept)
+                    const uint32_t m01 = prmt(db[0], db[1], 0x00FBu);
+                    const uint32_t m23 = prmt(db[2], db[3], 0xFB00u);
+                    flips = prmt(m01, m23, 0x7610u) & (kResSP * 0x01010101u);
+                    if (amb) ambmask |= 1u << w;
+                }
+                me[w] ^= flips;
+            }
+            if (KIND == 1 && ambmask != 0u) {           // rare: redo the flagged words with the exact binary64 rule
+                const int32_t* grow = v.fieldg + ((long long)rr->d * 2 + c) * v.Nh + ((long long)z * L + y) * ROWB;
+                const double beta = rr->beta;
+#pragma unroll
+                for (int w = 0; w < W; ++w)
+                    if ((ambmask >> w) & 1u)
+                        me[w] = ((idx8[w] >> 3) & (kResSP * 0x01010101u)) ^
+                                res_gauss_word_exact(v, idx8[w], grow + 4 * w, beta, rr->rk[0], rr->rk[1], q0 + (uint32_t)w, sweep, slot, dom);
+            }
+
+            // ---- write back -----------------------------------------------------------------------------------
+            if (valid) {
 #pragma unroll
                 for (int k = 0; k < K; ++k)
-                    *reinterpret_cast<uint4*>(dst + 16 * k) = make_uint4(me[4 * k] >> 3, me[4 * k + 1] >> 3, me[4 * k + 2] >> 3, me[4 * k + 3] >> 3);
+                    s_sp[A(c, s, k, e)] = make_uint4(me[4 * k], me[4 * k + 1], me[4 * k + 2], me[4 * k + 3]);
+                if (remote_p || remote_m) {
+                    uint8_t* dst = v.spins + ((long long)ds * 2 + c) * v.Nh + ((long long)z * L + y) * ROWB;
+#pragma unroll
+                    for (int k = 0; k < K; ++k)
+                        *reinterpret_cast<uint4*>(dst + 16 * k) = make_uint4(me[4 * k] >> 3, me[4 * k + 1] >> 3, me[4 * k + 2] >> 3, me[4 * k + 3] >> 3);
+                }
             }
+        }
+
+        if (meas) {
+            // per-replica sums in shared memory: one warp usually holds one replica (a seam can split it)
+            const int rep = valid ? (int)pi.rep : -1;
+            const int rep0 = __shfl_sync(0xFFFFFFFFu, rep, 0);
+            if (__all_sync(0xFFFFFFFFu, rep == rep0)) {
+                m_eb = warp_sum(m_eb); m_ef = warp_sum(m_ef); m_ms = warp_sum(m_ms);
+                if (lane == 0 && rep0 >= 0) {
+                    atomicAdd(reinterpret_cast<unsigned long long*>(s_acc + 3 * rep0 + 0), (unsigned long long)m_eb);
+                    atomicAdd(reinterpret_cast<unsigned long long*>(s_acc + 3 * rep0 + 1), (unsigned long long)m_ef);
+                    atomicAdd(reinterpret_cast<unsigned long long*>(s_acc + 3 * rep0 + 2), (unsigned long long)m_ms);
+                }
+            } else if (rep >= 0) {
+                atomicAdd(reinterpret_cast<unsigned long long*>(s_acc + 3 * rep + 0), (unsigned long long)m_eb);
+                atomicAdd(reinterpret_cast<unsigned long long*>(s_acc + 3 * rep + 1), (unsigned long long)m_ef);
+                atomicAdd(reinterpret_cast<unsigned long long*>(s_acc + 3 * rep + 2), (unsigned long long)m_ms);
+            }
+            continue;
         }
         __syncwarp();
         if (lane == 0) {
@@ -417,7 +499,7 @@ __global__ void __launch_bounds__(THREADS, 1) k_sweep_res(const View v, const Re
                 // its own phase p+1 only after that: at most two phases are open at once, one counter per parity
                 __threadfence();
                 const int done = atomicAdd(&s_ctl[p & 1], 1) + 1;
-                if (done == n_btasks) {
+                if (done == n_bblocks) {
                     atomicExch(&s_ctl[p & 1], 0);
                     __threadfence();
                     st_release_gpu(rp.prog + b, (rp.epoch << 8) | (uint32_t)(p + 1));
@@ -430,7 +512,7 @@ __global__ void __launch_bounds__(THREADS, 1) k_sweep_res(const View v, const Re
     }
     __syncthreads();
 
-    // ---- store the run back ------------------------------------------------------------------------------
+    // ---- store the run back, hand the measurement over ------------------------------------------------------
     {
         const int units = count * 2 * L * K;
         for (int u = tid; u < units; u += THREADS) {
@@ -441,6 +523,9 @@ __global__ void __launch_bounds__(THREADS, 1) k_sweep_res(const View v, const Re
             x.x >>= 3; x.y >>= 3; x.z >>= 3; x.w >>= 3;
             *reinterpret_cast<uint4*>(v.spins + ((long long)ds * 2 + col) * v.Nh + ((long long)z * L + y) * ROWB + 16 * k) = x;
         }
+        if (rp.measure)
+            for (int r = tid; r < nrep * 3; r += THREADS)
+                atomicAdd(reinterpret_cast<unsigned long long*>(v.acc + (long long)s_rep[r / 3].ds * 3 + r % 3), (unsigned long long)s_acc[r]);
     }
 }
 
