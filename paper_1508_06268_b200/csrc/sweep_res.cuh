@@ -44,7 +44,10 @@
 
 namespace rfim {
 
-constexpr int kResThreads = 512;
+#ifndef RFIM_RES_THREADS
+#define RFIM_RES_THREADS 512
+#endif
+constexpr int kResThreads = RFIM_RES_THREADS;
 constexpr uint32_t kResSP = 8;                  // shared-memory spin coding: 0 / SP
 constexpr int kResTabBytes = 256;               // per-replica acceptance table slot (256-byte aligned)
 
@@ -278,19 +281,7 @@ __global__ void __launch_bounds__(THREADS, 1) k_sweep_res(const View v, const Re
         for (int s = 0; s < 2; ++s) {
             const int ys = (s + z) & 1, y = 2 * i + ys;
             const int dir = (s + c) & 1;              // 0: second x-neighbour at xh-1, 1: at xh+1 (warp-uniform)
-            const long long blk = (((long long)rr->d * 2 + c) * L + z) * 2 + s;  // field block of this (colour, plane, class)
-
-            // field of the row: issued first, consumed last
-            float4 fa[W];
-            uint4 fb[K];
-            if (KIND == 0) {
-#pragma unroll
-                for (int k = 0; k < K; ++k) fb[k] = __ldg(reinterpret_cast<const uint4*>(rp.fieldb_res) + (blk * K + k) * LH + i);
-            } else if (!meas) {
-                const float4* fp = reinterpret_cast<const float4*>(rp.fielda_res) + (blk * W) * LH + i;
-#pragma unroll
-                for (int w = 0; w < W; ++w) fa[w] = __ldg(fp + (long long)w * LH);
-            }
+            const int blk = ((rr->d * 2 + c) * L + z) * 2 + s;                  // field block of this (colour, plane, class)
 
             // dependencies: the blocks of my plane and of its z-neighbours have finished phase p-1;
             // remote neighbour planes: their owners have published phase p-1
@@ -311,93 +302,20 @@ __global__ void __launch_bounds__(THREADS, 1) k_sweep_res(const View v, const Re
                 __threadfence_block();
             }
 
-            // ---- neighbour words of the row: t = SP * (number of up neighbours) per byte -----------------------
-            uint32_t cw[W], t[W], me[W];
+            // row addresses: shared arrays [colour][class][piece][row], pieces Ecap apart
             const int e_yp = pl * LH + (ys ? (i + 1 == LH ? 0 : i + 1) : i);
             const int e_ym = pl * LH + (ys ? i : (i == 0 ? LH - 1 : i - 1));
-#pragma unroll
-            for (int k = 0; k < K; ++k) {
-                const uint4 x = s_sp[A(oc, s, k, e)];
-                const uint4 yp = s_sp[A(oc, 1 - s, k, e_yp)];
-                const uint4 ym = s_sp[A(oc, 1 - s, k, e_ym)];
-                uint4 zp, zm;
-                if (!remote_p) zp = s_sp[A(oc, 1 - s, k, e_zp)];
-                else {
-                    zp = ld_cg16(v.spins + ((long long)ds * 2 + oc) * v.Nh + ((long long)zq_p * L + y) * ROWB + 16 * k);
-                    zp.x *= kResSP; zp.y *= kResSP; zp.z *= kResSP; zp.w *= kResSP;
-                }
-                if (!remote_m) zm = s_sp[A(oc, 1 - s, k, e_zm)];
-                else {
-                    zm = ld_cg16(v.spins + ((long long)ds * 2 + oc) * v.Nh + ((long long)zq_m * L + y) * ROWB + 16 * k);
-                    zm.x *= kResSP; zm.y *= kResSP; zm.z *= kResSP; zm.w *= kResSP;
-                }
-                const uint4 m = s_sp[A(c, s, k, e)];
-                cw[4 * k + 0] = x.x; cw[4 * k + 1] = x.y; cw[4 * k + 2] = x.z; cw[4 * k + 3] = x.w;
-                t[4 * k + 0] = yp.x + ym.x + zp.x + zm.x; t[4 * k + 1] = yp.y + ym.y + zp.y + zm.y;
-                t[4 * k + 2] = yp.z + ym.z + zp.z + zm.z; t[4 * k + 3] = yp.w + ym.w + zp.w + zm.w;
-                me[4 * k + 0] = m.x; me[4 * k + 1] = m.y; me[4 * k + 2] = m.z; me[4 * k + 3] = m.w;
-            }
-            uint32_t ns[W];                           // SP * (number of up neighbours) per byte
-            if (dir == 0) {
-#pragma unroll
-                for (int w = 0; w < W; ++w) ns[w] = t[w] + cw[w] + __funnelshift_r(cw[(w + W - 1) % W], cw[w], 24);
-            } else {
-#pragma unroll
-                for (int w = 0; w < W; ++w) ns[w] = t[w] + cw[w] + __funnelshift_r(cw[w], cw[(w + 1) % W], 8);
-            }
+            const uint4* a_x = s_sp + A(oc, s, 0, e);
+            const uint4* a_yp = s_sp + A(oc, 1 - s, 0, e_yp);
+            const uint4* a_ym = s_sp + A(oc, 1 - s, 0, e_ym);
+            const uint4* a_zp = s_sp + A(oc, 1 - s, 0, e_zp);
+            const uint4* a_zm = s_sp + A(oc, 1 - s, 0, e_zm);
+            uint4* a_me = s_sp + A(c, s, 0, e);
+            const long long rowoff = ((long long)z * L + y) * ROWB;             // byte offset of the row inside a colour array
+            const uint8_t* g_zp = v.spins + ((long long)ds * 2 + oc) * v.Nh + ((long long)zq_p * L + y) * ROWB;
+            const uint8_t* g_zm = v.spins + ((long long)ds * 2 + oc) * v.Nh + ((long long)zq_m * L + y) * ROWB;
 
-            if (meas) {
-                // ---- measurement: Eb over this colour-0 row, Msum and Ef over both colours of the row ------------
-                if (valid) {
-                    int sn = 0, s0 = 0, nn = 0, s1 = 0;   // 64 sum s0 n1, 8 sum s0, 8 sum n1, 8 sum s1
-#pragma unroll
-                    for (int w = 0; w < W; ++w) {
-                        sn += dot4(me[w], ns[w]); s0 += dot4(me[w], 0x01010101u);
-                        nn += dot4(ns[w], 0x01010101u); s1 += dot4(cw[w], 0x01010101u);
-                    }
-                    // sum (2 s0 - 1)(2 n1 - 6) = 4 s0.n1 - 12 s0 - 2 n1 + 6 per site
-                    m_eb += sn / 16 - 12 * (s0 / 8) - 2 * (nn / 8) + 6 * ROWB;
-                    m_ms += 2 * ((s0 + s1) / 8) - 2 * ROWB;
-                    const long long rowoff = ((long long)z * L + y) * ROWB;
-                    if (KIND == 0) {
-                        // sum (2 hb - 1)(2 s - 1) = 4 hb.s - 2 hb - 2 s + 1 per site; hb = 0x10 flags in natural colour order
-                        const uint32_t* h0 = reinterpret_cast<const uint32_t*>(v.fieldb + ((long long)rr->d * 2 + 0) * v.Nh + rowoff);
-                        const uint32_t* h1 = reinterpret_cast<const uint32_t*>(v.fieldb + ((long long)rr->d * 2 + 1) * v.Nh + rowoff);
-                        int hs0 = 0, hh = 0;
-#pragma unroll
-                        for (int w = 0; w < W; ++w) {
-                            const uint32_t a0 = __ldg(h0 + w) >> 4, a1 = __ldg(h1 + w) >> 4;   // 0/1 per byte
-                            hs0 += dot4(a0, me[w]) + dot4(a1, cw[w]);                         // 8 sum hb s
-                            hh += dot4(a0, 0x01010101u) + dot4(a1, 0x01010101u);
-                        }
-                        m_ef += 4 * (hs0 / 8) - 2 * hh - 2 * ((s0 + s1) / 8) + 2 * ROWB;
-                    } else {
-                        const int32_t* g0 = v.fieldg + ((long long)rr->d * 2 + 0) * v.Nh + rowoff;
-                        const int32_t* g1 = v.fieldg + ((long long)rr->d * 2 + 1) * v.Nh + rowoff;
-                        long long ef = 0;
-#pragma unroll
-                        for (int w = 0; w < W; ++w) {
-                            const int4 a0 = __ldg(reinterpret_cast<const int4*>(g0) + w), a1 = __ldg(reinterpret_cast<const int4*>(g1) + w);
-                            const int ga[4] = {a0.x, a0.y, a0.z, a0.w}, gb[4] = {a1.x, a1.y, a1.z, a1.w};
-                            int part = 0;                 // |g| <= 2^23: eight terms fit easily
-#pragma unroll
-                            for (int k = 0; k < 4; ++k) {
-                                part += ((me[w] >> (8 * k)) & kResSP) ? ga[k] : -ga[k];
-                                part += ((cw[w] >> (8 * k)) & kResSP) ? gb[k] : -gb[k];
-                            }
-                            ef += part;
-                        }
-                        m_ef += ef;
-                    }
-                }
-                continue;
-            }
-
-            uint32_t idx8[W];
-#pragma unroll
-            for (int w = 0; w < W; ++w) idx8[w] = ns[w] + (me[w] << 3) + (KIND == 0 ? reinterpret_cast<const uint32_t*>(fb)[w] : 0u);
-
-            // ---- per-task constants ---------------------------------------------------------------------------
+            // per-row constants
             uint32_t rk[20];
             if (UNI) {
 #pragma unroll
@@ -414,62 +332,156 @@ __global__ void __launch_bounds__(THREADS, 1) k_sweep_res(const View v, const Re
             const float band = rr->band;
             const uint32_t q0 = (uint32_t)W * (uint32_t)(y + L * z);
 
-            // ---- the 4K words of the row -------------------------------------------------------------------
-            uint32_t ambmask = 0;
 #pragma unroll
-            for (int w = 0; w < W; ++w) {
-                const Words4 r = philox_rkreg(rk, q0 + (uint32_t)w, sweep, slot, dom);
-                const uint32_t u[4] = {r.w0, r.w1, r.w2, r.w3};
-                uint32_t flips;
+            for (int k = 0; k < K; ++k) {           // one 16-site piece of the row at a time
+                // field of the piece: issued first, consumed last
+                float4 fa[4];
+                uint4 fb = make_uint4(0u, 0u, 0u, 0u);
                 if (KIND == 0) {
-                    flips = 0;
+                    if (!meas) fb = __ldg(reinterpret_cast<const uint4*>(rp.fieldb_res) + (blk * K + k) * LH + i);
+                } else if (!meas) {
+                    const float4* fp = reinterpret_cast<const float4*>(rp.fielda_res) + (blk * W + 4 * k) * LH + i;
 #pragma unroll
-                    for (int k = 0; k < 4; ++k) {
-                        const uint2 ent = lds64(__byte_perm(idx8[w], tab_addr, 0x7650 + k));
-                        bool acc = u[k] <= ent.x;
-                        if (NEVER) acc = acc && ent.y == 0u;
-                        if (acc) flips |= kResSP << (8 * k);
-                    }
-                } else {
-                    const float a[4] = {fa[w].x, fa[w].y, fa[w].z, fa[w].w};
-                    uint32_t db[4];
-                    bool amb = false;
-#pragma unroll
-                    for (int k = 0; k < 4; ++k) {
-                        const uint2 ent = lds64(__byte_perm(idx8[w], tab_addr, 0x7650 + k));
-                        const float P = ex2_approx(fmaf(a[k], __uint_as_float(ent.y), __uint_as_float(ent.x)));
-                        const float d = __uint2float_rn(u[k]) - P;
-                        amb = amb || (fabsf(d) < band);
-                        db[k] = __float_as_uint(d);
-                    }
-                    // sign bytes of the four differences -> 0xFF where d < 0 (accept)
-                    const uint32_t m01 = prmt(db[0], db[1], 0x00FBu);
-                    const uint32_t m23 = prmt(db[2], db[3], 0xFB00u);
-                    flips = prmt(m01, m23, 0x7610u) & (kResSP * 0x01010101u);
-                    if (amb) ambmask |= 1u << w;
+                    for (int w = 0; w < 4; ++w) fa[w] = __ldg(fp + w * LH);
                 }
-                me[w] ^= flips;
-            }
-            if (KIND == 1 && ambmask != 0u) {           // rare: redo the flagged words with the exact binary64 rule
-                const int32_t* grow = v.fieldg + ((long long)rr->d * 2 + c) * v.Nh + ((long long)z * L + y) * ROWB;
-                const double beta = rr->beta;
-#pragma unroll
-                for (int w = 0; w < W; ++w)
-                    if ((ambmask >> w) & 1u)
-                        me[w] = ((idx8[w] >> 3) & (kResSP * 0x01010101u)) ^
-                                res_gauss_word_exact(v, idx8[w], grow + 4 * w, beta, rr->rk[0], rr->rk[1], q0 + (uint32_t)w, sweep, slot, dom);
-            }
 
-            // ---- write back -----------------------------------------------------------------------------------
-            if (valid) {
+                // ---- neighbour words: ns = SP * (number of up neighbours) per byte ---------------------------------
+                const uint4 x = a_x[k * Ecap];
+                const uint4 yp = a_yp[k * Ecap];
+                const uint4 ym = a_ym[k * Ecap];
+                uint4 zp, zm;
+                if (!remote_p) zp = a_zp[k * Ecap];
+                else {
+                    zp = ld_cg16(g_zp + 16 * k);
+                    zp.x *= kResSP; zp.y *= kResSP; zp.z *= kResSP; zp.w *= kResSP;
+                }
+                if (!remote_m) zm = a_zm[k * Ecap];
+                else {
+                    zm = ld_cg16(g_zm + 16 * k);
+                    zm.x *= kResSP; zm.y *= kResSP; zm.z *= kResSP; zm.w *= kResSP;
+                }
+                const uint4 m = a_me[k * Ecap];
+                // the word holding the far x-neighbour of the piece's edge byte (periodic in x)
+                uint32_t edge;
+                if (K == 1) edge = dir == 0 ? x.w : x.x;
+                else edge = reinterpret_cast<const uint32_t*>(a_x + ((k + K - 1) % K) * Ecap)[dir == 0 ? 3 : 0];
+                const uint32_t cw[4] = {x.x, x.y, x.z, x.w};
+                uint32_t me[4] = {m.x, m.y, m.z, m.w};
+                uint32_t ns[4] = {yp.x + ym.x + zp.x + zm.x, yp.y + ym.y + zp.y + zm.y, yp.z + ym.z + zp.z + zm.z, yp.w + ym.w + zp.w + zm.w};
+                if (dir == 0) {
+                    ns[0] += cw[0] + __funnelshift_r(edge, cw[0], 24);
 #pragma unroll
-                for (int k = 0; k < K; ++k)
-                    s_sp[A(c, s, k, e)] = make_uint4(me[4 * k], me[4 * k + 1], me[4 * k + 2], me[4 * k + 3]);
-                if (remote_p || remote_m) {
-                    uint8_t* dst = v.spins + ((long long)ds * 2 + c) * v.Nh + ((long long)z * L + y) * ROWB;
+                    for (int w = 1; w < 4; ++w) ns[w] += cw[w] + __funnelshift_r(cw[w - 1], cw[w], 24);
+                } else {
 #pragma unroll
-                    for (int k = 0; k < K; ++k)
-                        *reinterpret_cast<uint4*>(dst + 16 * k) = make_uint4(me[4 * k] >> 3, me[4 * k + 1] >> 3, me[4 * k + 2] >> 3, me[4 * k + 3] >> 3);
+                    for (int w = 0; w < 3; ++w) ns[w] += cw[w] + __funnelshift_r(cw[w], cw[w + 1], 8);
+                    ns[3] += cw[3] + __funnelshift_r(cw[3], edge, 8);
+                }
+
+                if (meas) {
+                    // ---- measurement: Eb over this colour-0 piece, Msum and Ef over both colours of it ---------------
+                    if (valid) {
+                        int sn = 0, s0 = 0, nn = 0, s1 = 0;   // 64 sum s0 n1, 8 sum s0, 8 sum n1, 8 sum s1
+#pragma unroll
+                        for (int w = 0; w < 4; ++w) {
+                            sn += dot4(me[w], ns[w]); s0 += dot4(me[w], 0x01010101u);
+                            nn += dot4(ns[w], 0x01010101u); s1 += dot4(cw[w], 0x01010101u);
+                        }
+                        // sum (2 s0 - 1)(2 n1 - 6) = 4 s0.n1 - 12 s0 - 2 n1 + 6 per site
+                        m_eb += sn / 16 - 12 * (s0 / 8) - 2 * (nn / 8) + 6 * 16;
+                        m_ms += 2 * ((s0 + s1) / 8) - 2 * 16;
+                        if (KIND == 0) {
+                            // sum (2 hb - 1)(2 s - 1) = 4 hb.s - 2 hb - 2 s + 1 per site; hb = 0x10 flags in natural colour order
+                            const uint4 h0 = __ldg(reinterpret_cast<const uint4*>(v.fieldb + ((long long)rr->d * 2 + 0) * v.Nh + rowoff) + k);
+                            const uint4 h1 = __ldg(reinterpret_cast<const uint4*>(v.fieldb + ((long long)rr->d * 2 + 1) * v.Nh + rowoff) + k);
+                            const uint32_t a0[4] = {h0.x >> 4, h0.y >> 4, h0.z >> 4, h0.w >> 4};   // 0/1 per byte
+                            const uint32_t a1[4] = {h1.x >> 4, h1.y >> 4, h1.z >> 4, h1.w >> 4};
+                            int hs0 = 0, hh = 0;
+#pragma unroll
+                            for (int w = 0; w < 4; ++w) {
+                                hs0 += dot4(a0[w], me[w]) + dot4(a1[w], cw[w]);                       // 8 sum hb s
+                                hh += dot4(a0[w], 0x01010101u) + dot4(a1[w], 0x01010101u);
+                            }
+                            m_ef += 4 * (hs0 / 8) - 2 * hh - 2 * ((s0 + s1) / 8) + 2 * 16;
+                        } else {
+                            const int4* g0 = reinterpret_cast<const int4*>(v.fieldg + ((long long)rr->d * 2 + 0) * v.Nh + rowoff) + 4 * k;
+                            const int4* g1 = reinterpret_cast<const int4*>(v.fieldg + ((long long)rr->d * 2 + 1) * v.Nh + rowoff) + 4 * k;
+                            long long ef = 0;
+#pragma unroll
+                            for (int w = 0; w < 4; ++w) {
+                                const int4 b0 = __ldg(g0 + w), b1 = __ldg(g1 + w);
+                                const int ga[4] = {b0.x, b0.y, b0.z, b0.w}, gb[4] = {b1.x, b1.y, b1.z, b1.w};
+                                int part = 0;                 // |g| <= 2^23: eight terms fit easily
+#pragma unroll
+                                for (int j = 0; j < 4; ++j) {
+                                    part += ((me[w] >> (8 * j)) & kResSP) ? ga[j] : -ga[j];
+                                    part += ((cw[w] >> (8 * j)) & kResSP) ? gb[j] : -gb[j];
+                                }
+                                ef += part;
+                            }
+                            m_ef += ef;
+                        }
+                    }
+                    continue;
+                }
+
+                const uint32_t fw[4] = {fb.x, fb.y, fb.z, fb.w};
+                uint32_t idx8[4];
+#pragma unroll
+                for (int w = 0; w < 4; ++w) idx8[w] = ns[w] + (me[w] << 3) + (KIND == 0 ? fw[w] : 0u);
+
+                // ---- the four words of the piece ---------------------------------------------------------------
+                uint32_t ambmask = 0;
+#pragma unroll
+                for (int w = 0; w < 4; ++w) {
+                    const Words4 r = philox_rkreg(rk, q0 + (uint32_t)(4 * k + w), sweep, slot, dom);
+                    const uint32_t u[4] = {r.w0, r.w1, r.w2, r.w3};
+                    uint32_t flips;
+                    if (KIND == 0) {
+                        flips = 0;
+#pragma unroll
+                        for (int j = 0; j < 4; ++j) {
+                            const uint2 ent = lds64(__byte_perm(idx8[w], tab_addr, 0x7650 + j));
+                            bool acc = u[j] <= ent.x;
+                            if (NEVER) acc = acc && ent.y == 0u;
+                            if (acc) flips |= kResSP << (8 * j);
+                        }
+                    } else {
+                        const float a[4] = {fa[w].x, fa[w].y, fa[w].z, fa[w].w};
+                        uint32_t db[4];
+                        bool amb = false;
+#pragma unroll
+                        for (int j = 0; j < 4; ++j) {
+                            const uint2 ent = lds64(__byte_perm(idx8[w], tab_addr, 0x7650 + j));
+                            const float P = ex2_approx(fmaf(a[j], __uint_as_float(ent.y), __uint_as_float(ent.x)));
+                            const float d = __uint2float_rn(u[j]) - P;
+                            amb = amb || (fabsf(d) < band);
+                            db[j] = __float_as_uint(d);
+                        }
+                        // sign bytes of the four differences -> 0xFF where d < 0 (accept)
+                        const uint32_t m01 = prmt(db[0], db[1], 0x00FBu);
+                        const uint32_t m23 = prmt(db[2], db[3], 0xFB00u);
+                        flips = prmt(m01, m23, 0x7610u) & (kResSP * 0x01010101u);
+                        if (amb) ambmask |= 1u << w;
+                    }
+                    me[w] ^= flips;
+                }
+                if (KIND == 1 && ambmask != 0u) {       // rare: redo the flagged words with the exact binary64 rule
+                    const int32_t* grow = v.fieldg + ((long long)rr->d * 2 + c) * v.Nh + rowoff + 16 * k;
+                    const double beta = rr->beta;
+#pragma unroll
+                    for (int w = 0; w < 4; ++w)
+                        if ((ambmask >> w) & 1u)
+                            me[w] = ((idx8[w] >> 3) & (kResSP * 0x01010101u)) ^
+                                    res_gauss_word_exact(v, idx8[w], grow + 4 * w, beta, rr->rk[0], rr->rk[1], q0 + (uint32_t)(4 * k + w), sweep, slot, dom);
+                }
+
+                // ---- write back ---------------------------------------------------------------------------------
+                if (valid) {
+                    a_me[k * Ecap] = make_uint4(me[0], me[1], me[2], me[3]);
+                    if (remote_p || remote_m)
+                        *reinterpret_cast<uint4*>(v.spins + ((long long)ds * 2 + c) * v.Nh + rowoff + 16 * k) =
+                            make_uint4(me[0] >> 3, me[1] >> 3, me[2] >> 3, me[3] >> 3);
                 }
             }
         }
