@@ -319,9 +319,10 @@ ResPlan res_plan(const rfim_pt* h) {
     p.total = (int)total;
     p.q = p.total / p.grid; p.rem = p.total % p.grid;
     p.cap_planes = p.q + (p.rem ? 1 : 0);
+    if (p.cap_planes > res_max_planes(h->L)) return p;
     p.cap_reps = (p.cap_planes + h->L - 2) / h->L + 1;
     if (p.cap_reps > 255) return p;
-    p.smem = res_smem_bytes(h->L, p.cap_planes, p.cap_reps);
+    p.smem = res_smem_bytes(h->L, p.cap_reps);
     p.ok = p.smem <= (size_t)h->smem_optin;
     return p;
 }
@@ -418,7 +419,7 @@ int launch_res(rfim_pt* h, int sweeps, bool measure) {
     rp.epoch = ++h->res_epoch;
     rp.prog = h->res_prog;
     rp.total_planes = pl.total; rp.q = pl.q; rp.rem = pl.rem;
-    rp.cap_planes = pl.cap_planes; rp.cap_reps = pl.cap_reps;
+    rp.cap_reps = pl.cap_reps;
     rp.fielda_res = h->fielda_res; rp.fieldb_res = h->fieldb_res;
     rp.diag = h->v.diag;
     {

@@ -25,16 +25,17 @@
 // integer atomics (order-independent, hence deterministic).
 //
 // In shared memory a spin is a byte holding 0 or SP (= 8), four same-colour sites per 32-bit word
-// exactly as in global memory (where it is 0/1), so the six-neighbour count of four sites is three
+// exactly as in global memory (where it is 0/1), so the six-neighbour count of four sites is a few
 // IADD3, and count*SP + spin*8*SP [+ field bit] is directly the byte offset of the site's entry in
 // the replica's 8-byte acceptance table: one PRMT splices it into the (256-byte aligned) table
 // address, one LDS.64 fetches the entry.
 //
-// A thread owns one row of one colour (L/2 sites = 4K words = 4K Philox calls); the 32 lanes of a
-// warp own 32 rows of the same checkerboard class s = (y+z)&1, so the direction of the second
-// x-neighbour ((s+colour)&1) is warp-uniform.  Shared memory is laid out [colour][s][piece][row],
-// which makes every 16-byte access of a warp contiguous (no bank conflicts); the field is read from
-// a copy stored in the same task order (coalesced 16-byte loads from L2).
+// A thread owns one row of one colour (L/2 sites = 4K words = 4K Philox calls) and walks it one
+// 16-site piece at a time; the 32 lanes of a warp own 32 rows of the same checkerboard class
+// s = (y+z)&1, so the direction of the second x-neighbour ((s+colour)&1) is warp-uniform.  Shared
+// memory is laid out [colour][s][piece][row] with a compile-time row capacity, which makes every
+// 16-byte access of a warp contiguous (no bank conflicts) and every array offset an immediate; the
+// field is read from a copy stored in the same task order (coalesced 16-byte loads from L2).
 #pragma once
 #include <cstdint>
 #include "kernels_ref.cuh"
@@ -51,6 +52,21 @@ constexpr int kResThreads = RFIM_RES_THREADS;
 constexpr uint32_t kResSP = 8;                  // shared-memory spin coding: 0 / SP
 constexpr int kResTabBytes = 256;               // per-replica acceptance table slot (256-byte aligned)
 
+// shared-memory geometry of the resident kernel for L = 32 K
+template <int K>
+struct ResGeom {
+    static constexpr int L = 32 * K;
+    static constexpr int LH = L / 2;                        // rows per class per plane
+    static constexpr int ROWB = 16 * K;                     // bytes (= sites) per row per colour
+    static constexpr int W = 4 * K;                         // words (= Philox calls) per row
+    static constexpr int MAXPLANES = K == 2 ? 56 : 221;     // planes one CTA can hold (227 KB of shared memory)
+    static constexpr int ECAP = MAXPLANES * LH;             // rows per (colour, class, piece) array
+    static constexpr int ARR = ECAP * 16;                   // bytes per array
+    static constexpr int SPINS_BYTES = 4 * K * ARR;         // [colour][class][piece][row] uint4
+    static constexpr int NBCAP = (ECAP + 31) / 32;          // 32-row blocks
+};
+__host__ __device__ constexpr int res_max_planes(int L) { return L == 64 ? ResGeom<2>::MAXPLANES : ResGeom<1>::MAXPLANES; }
+
 struct ResParams {
     int phases;                  // 2 * sweeps of this launch, <= 254
     int measure;                 // != 0: finish with the measurement pseudo-phase (Eb, Ef, Msum -> View::acc)
@@ -59,7 +75,7 @@ struct ResParams {
     uint32_t* prog;              // [grid]
     int total_planes;            // D * n * L
     int q, rem;                  // run of CTA b: start = b*q + min(b, rem), count = q + (b < rem)
-    int cap_planes, cap_reps;    // shared-memory carve (planes, replicas) -- same for every CTA
+    int cap_reps;                // replicas a run can touch -- same carve for every CTA
     const float* fielda_res;     // Gaussian: [D][2][L][2][4K][L/2] float4 (task order), (float)(hs * g_i)
     const uint8_t* fieldb_res;   // bimodal:  [D][2][L][2][K][L/2] uint4, 0x80 where h_i = +1
     unsigned long long* diag;
@@ -79,13 +95,16 @@ struct ResRep {                  // per replica touched by the run
     uint32_t rk[20];             // Philox round keys rk[2r] = k0 + r*W0, rk[2r+1] = k1 + r*W1
 };
 
-__host__ __device__ inline size_t res_smem_bytes(int L, int cap_planes, int cap_reps) {
-    size_t b = (size_t)cap_reps * kResTabBytes + (size_t)cap_planes * L * L;
+__host__ __device__ inline size_t res_smem_bytes(int L, int cap_reps) {
+    const size_t spins = L == 64 ? ResGeom<2>::SPINS_BYTES : ResGeom<1>::SPINS_BYTES;
+    const size_t maxpl = L == 64 ? ResGeom<2>::MAXPLANES : ResGeom<1>::MAXPLANES;
+    const size_t nbcap = L == 64 ? ResGeom<2>::NBCAP : ResGeom<1>::NBCAP;
+    size_t b = spins + (size_t)cap_reps * kResTabBytes;
     b += (size_t)cap_reps * sizeof(ResRep);
-    b += (size_t)cap_planes * sizeof(ResPlane);
-    b += (size_t)((cap_planes * (L / 2) + 31) / 32) * 2 * sizeof(int);   // block order, block completion counters
-    b += 16;                                                             // counters
-    b += (size_t)cap_reps * 3 * sizeof(long long);                       // measurement accumulators
+    b += maxpl * sizeof(ResPlane);
+    b += nbcap * 2 * sizeof(int);                           // block order, block completion counters
+    b += 16;                                                // counters
+    b += (size_t)cap_reps * 3 * sizeof(long long);          // measurement accumulators
     return (b + 15) & ~(size_t)15;
 }
 
@@ -111,21 +130,6 @@ __device__ __forceinline__ uint32_t prmt(uint32_t a, uint32_t b, uint32_t sel) {
     return r;
 }
 
-// exact rule for the four sites of one word whose table-offset bytes are idx8 = SP*n1 + 8*SP*s (rare: some site
-// of the word fell inside the float path's guard band).  Redraws the word's random numbers.
-__device__ __noinline__ uint32_t res_gauss_word_exact(const View& v, uint32_t idx8, const int32_t* __restrict__ g4, double beta,
-                                                      uint32_t k0, uint32_t k1, uint32_t q, uint32_t sweep, uint32_t slot, uint32_t dom) {
-    const Words4 r = philox4x32_10(k0, k1, q, sweep, slot, dom);
-    const uint32_t u[4] = {r.w0, r.w1, r.w2, r.w3};
-    uint32_t flips = 0;
-#pragma unroll
-    for (int k = 0; k < 4; ++k) {
-        const uint32_t b = (idx8 >> (8 * k)) & 0xFFu;
-        if (gauss_accept_exact(v, (int)(b >> 6), (int)((b >> 3) & 7u), g4[k], beta, u[k])) flips |= kResSP << (8 * k);
-    }
-    return flips;
-}
-
 __device__ __forceinline__ int lds_volatile(const int* p) { return *reinterpret_cast<const volatile int*>(p); }
 
 __device__ __forceinline__ Words4 philox_rkreg(const uint32_t (&rk)[20], uint32_t c0, uint32_t c1, uint32_t c2, uint32_t c3) {
@@ -142,13 +146,103 @@ __device__ __forceinline__ Words4 philox_rkreg(const uint32_t (&rk)[20], uint32_
     return w;
 }
 
+// the float path of one Gaussian attempt: d = float(u) - P~, P~ = 2^(a*y + x); accept iff d < 0 unless |d| < band
+__device__ __forceinline__ float res_gauss_diff(uint32_t idx8, int j, uint32_t tab_addr, float a, uint32_t u) {
+    const uint2 ent = lds64(__byte_perm(idx8, tab_addr, 0x7650 + j));
+    const float P = ex2_approx(fmaf(a, __uint_as_float(ent.y), __uint_as_float(ent.x)));
+    return __uint2float_rn(u) - P;
+}
+
+// Rare path: some site of the piece fell inside the float path's guard band.  Redo the piece's four words: sites
+// outside the band keep the float decision (the same operations, hence the same bits), sites inside it take the
+// exact binary64 rule of DESIGN.md S3.  idx8 = table-offset bytes before the update (SP*n1 + 8*SP*s).
+__device__ __noinline__ uint4 res_gauss_piece_fix(const View& v, uint4 idx8v, uint32_t tab_addr, float band, const float4* __restrict__ fa,
+                                                  int fa_stride, const int32_t* __restrict__ g16, const ResRep* rr, uint32_t q,
+                                                  uint32_t sweep, uint32_t dom) {
+    const uint32_t idx8[4] = {idx8v.x, idx8v.y, idx8v.z, idx8v.w};
+    uint32_t out[4];
+    for (int w = 0; w < 4; ++w) {
+        const Words4 r = philox4x32_10(rr->rk[0], rr->rk[1], q + (uint32_t)w, sweep, (uint32_t)rr->slot, dom);
+        const uint32_t u[4] = {r.w0, r.w1, r.w2, r.w3};
+        const float4 f4 = __ldg(fa + (long long)w * fa_stride);
+        const float a[4] = {f4.x, f4.y, f4.z, f4.w};
+        uint32_t me = (idx8[w] >> 3) & (kResSP * 0x01010101u);
+        for (int j = 0; j < 4; ++j) {
+            const float d = res_gauss_diff(idx8[w], j, tab_addr, a[j], u[j]);
+            bool acc = d < 0.0f;
+            if (fabsf(d) < band) {
+                const uint32_t bb = (idx8[w] >> (8 * j)) & 0xFFu;
+                acc = gauss_accept_exact(v, (int)(bb >> 6), (int)((bb >> 3) & 7u), g16[4 * w + j], rr->beta, u[j]);
+            }
+            if (acc) me ^= kResSP << (8 * j);
+        }
+        out[w] = me;
+    }
+    return make_uint4(out[0], out[1], out[2], out[3]);
+}
+
+// slow side of a task's dependency wait (the fast check failed, or a neighbour plane lives in another CTA)
+__device__ __noinline__ void res_wait_slow(const int* s_done, int eb, int b_zp, int b_zm, int p, const uint32_t* prog_p,
+                                           const uint32_t* prog_m, uint32_t want, unsigned long long* diag) {
+    int spins = 0;
+    for (;;) {
+        bool ok = lds_volatile(s_done + eb) >= p && lds_volatile(s_done + b_zp) >= p && lds_volatile(s_done + b_zm) >= p;
+        if (prog_p) ok = ok && (int32_t)(ld_acquire_gpu(prog_p) - want) >= 0;
+        if (prog_m) ok = ok && (int32_t)(ld_acquire_gpu(prog_m) - want) >= 0;
+        if (__all_sync(0xFFFFFFFFu, ok)) break;
+        backoff();
+        if (++spins > (1 << 22)) { if ((threadIdx.x & 31) == 0) atomicOr(diag, 1ull); break; }
+    }
+}
+
+// one 16-site piece of a row: own word, same-row words of the other colour, and ns = SP * (number of up neighbours)
+struct ResPiece { uint32_t me[4], cw[4], ns[4]; };
+
+template <int K>
+__device__ __forceinline__ ResPiece res_load_piece(const uint8_t* smem, uint32_t a_x, uint32_t a_yp, uint32_t a_ym, uint32_t a_zp,
+                                                   uint32_t a_zm, uint32_t a_me, int k, int dir, bool remote_p, bool remote_m,
+                                                   const uint8_t* g_zp, const uint8_t* g_zm) {
+    constexpr int ARR = ResGeom<K>::ARR;
+    const uint4 x = *reinterpret_cast<const uint4*>(smem + a_x + k * ARR);
+    const uint4 yp = *reinterpret_cast<const uint4*>(smem + a_yp + k * ARR);
+    const uint4 ym = *reinterpret_cast<const uint4*>(smem + a_ym + k * ARR);
+    uint4 zp = *reinterpret_cast<const uint4*>(smem + a_zp + k * ARR);
+    uint4 zm = *reinterpret_cast<const uint4*>(smem + a_zm + k * ARR);
+    const uint4 m = *reinterpret_cast<const uint4*>(smem + a_me + k * ARR);
+    if (remote_p) {
+        zp = ld_cg16(g_zp + 16 * k);
+        zp.x *= kResSP; zp.y *= kResSP; zp.z *= kResSP; zp.w *= kResSP;
+    }
+    if (remote_m) {
+        zm = ld_cg16(g_zm + 16 * k);
+        zm.x *= kResSP; zm.y *= kResSP; zm.z *= kResSP; zm.w *= kResSP;
+    }
+    // the word holding the far x-neighbour of the piece's edge byte (periodic in x)
+    uint32_t edge;
+    if (K == 1) edge = dir == 0 ? x.w : x.x;
+    else edge = *reinterpret_cast<const uint32_t*>(smem + a_x + ((k + K - 1) % K) * ARR + (dir == 0 ? 12 : 0));
+    ResPiece pc;
+    pc.me[0] = m.x; pc.me[1] = m.y; pc.me[2] = m.z; pc.me[3] = m.w;
+    pc.cw[0] = x.x; pc.cw[1] = x.y; pc.cw[2] = x.z; pc.cw[3] = x.w;
+    pc.ns[0] = yp.x + ym.x + zp.x + zm.x + x.x; pc.ns[1] = yp.y + ym.y + zp.y + zm.y + x.y;
+    pc.ns[2] = yp.z + ym.z + zp.z + zm.z + x.z; pc.ns[3] = yp.w + ym.w + zp.w + zm.w + x.w;
+    if (dir == 0) {
+        pc.ns[0] += __funnelshift_r(edge, pc.cw[0], 24);
+#pragma unroll
+        for (int w = 1; w < 4; ++w) pc.ns[w] += __funnelshift_r(pc.cw[w - 1], pc.cw[w], 24);
+    } else {
+#pragma unroll
+        for (int w = 0; w < 3; ++w) pc.ns[w] += __funnelshift_r(pc.cw[w], pc.cw[w + 1], 8);
+        pc.ns[3] += __funnelshift_r(pc.cw[3], edge, 8);
+    }
+    return pc;
+}
+
 // K = 16-byte pieces per row per colour (L = 32 K); UNI: one member, round keys come from the constant bank
 template <int KIND, int K, bool NEVER, bool UNI, int THREADS>
 __global__ void __launch_bounds__(THREADS, 1) k_sweep_res(const View v, const ResParams rp) {
-    constexpr int L = 32 * K;
-    constexpr int LH = L / 2;                   // rows per class per plane
-    constexpr int ROWB = 16 * K;                // bytes (= sites) per row per colour
-    constexpr int W = 4 * K;                    // words (= Philox calls) per row
+    using G = ResGeom<K>;
+    constexpr int L = G::L, LH = G::LH, ROWB = G::ROWB, W = G::W, ARR = G::ARR;
     extern __shared__ __align__(1024) uint8_t smem[];
 
     const int tid = threadIdx.x, lane = tid & 31;
@@ -156,20 +250,18 @@ __global__ void __launch_bounds__(THREADS, 1) k_sweep_res(const View v, const Re
     const int start = b * rp.q + min(b, rp.rem);
     const int count = rp.q + (b < rp.rem ? 1 : 0);
     if (count == 0) return;
-    const int Ecap = rp.cap_planes * LH;        // rows per (colour, class) array
-    const int E = count * LH;                   // rows in use
+    const int E = count * LH;                   // rows in use (per colour and class)
     const int nb = (E + 31) / 32;               // 32-row blocks
-    const int nbcap = (Ecap + 31) / 32;
 
-    uint8_t* s_tab = smem;
-    uint4* s_sp = reinterpret_cast<uint4*>(smem + (size_t)rp.cap_reps * kResTabBytes);
-    ResRep* s_rep = reinterpret_cast<ResRep*>(reinterpret_cast<uint8_t*>(s_sp) + (size_t)rp.cap_planes * L * L);
+    uint8_t* s_tab = smem + G::SPINS_BYTES;
+    ResRep* s_rep = reinterpret_cast<ResRep*>(s_tab + (size_t)rp.cap_reps * kResTabBytes);
     ResPlane* s_plane = reinterpret_cast<ResPlane*>(s_rep + rp.cap_reps);
-    int* s_order = reinterpret_cast<int*>(s_plane + rp.cap_planes);
-    int* s_done = s_order + nbcap;              // per block: tasks completed so far (one per phase)
-    int* s_ctl = s_done + nbcap;                // [0],[1] boundary tasks done in the open even / odd phase, [2] next task number, [3] boundary blocks
+    int* s_order = reinterpret_cast<int*>(s_plane + G::MAXPLANES);
+    int* s_done = s_order + G::NBCAP;           // per block: tasks completed so far (one per phase)
+    int* s_ctl = s_done + G::NBCAP;             // [0],[1] boundary tasks done in the open even / odd phase, [2] next task number, [3] boundary blocks
     long long* s_acc = reinterpret_cast<long long*>(s_ctl + 4);   // [rep][3] measurement accumulators
-    auto A = [&](int col, int s, int k, int e) { return ((col * 2 + s) * K + k) * Ecap + e; };
+    // byte offset of row e of array (colour, class, piece)
+    auto A = [&](int col, int s, int k, int e) { return (uint32_t)(((col * 2 + s) * K + k) * ARR + e * 16); };
 
     // ---- set-up: plane table, replica contexts, block order --------------------------------------------
     const int dt0 = start / L;
@@ -243,21 +335,24 @@ __global__ void __launch_bounds__(THREADS, 1) k_sweep_res(const View v, const Re
             const uint8_t* src = v.spins + ((long long)ds * 2 + col) * v.Nh + ((long long)z * L + y) * ROWB + 16 * k;
             uint4 x = ld_cg16(src);
             x.x *= kResSP; x.y *= kResSP; x.z *= kResSP; x.w *= kResSP;
-            s_sp[A(col, (y + z) & 1, k, p * LH + (y >> 1))] = x;
+            *reinterpret_cast<uint4*>(smem + A(col, (y + z) & 1, k, p * LH + (y >> 1))) = x;
         }
     }
     __syncthreads();
     const int n_bblocks = s_ctl[3];
     const int total_tasks = nb * (rp.phases + (rp.measure ? 1 : 0));
     const uint32_t tab0 = (uint32_t)__cvta_generic_to_shared(s_tab);
+    const uint32_t nh32 = (uint32_t)v.Nh;
 
     // ---- the task flow ------------------------------------------------------------------------------
+    int p_cur = 0, base_cur = 0;                      // phase of this warp's current task number (numbers only grow)
     for (;;) {
         int g = 0;
         if (lane == 0) g = atomicAdd(&s_ctl[2], 1);
         g = __shfl_sync(0xFFFFFFFFu, g, 0);
         if (g >= total_tasks) break;
-        const int p = g / nb, bidx = g - p * nb;
+        while (g - base_cur >= nb) { base_cur += nb; ++p_cur; }
+        const int p = p_cur, bidx = g - base_cur;
         const bool meas = p == rp.phases;             // the measurement pseudo-phase (colour 0; phases is even)
         const int c = p & 1, oc = 1 - c;
         const uint32_t sweep = rp.sweep0 + (uint32_t)(p >> 1);
@@ -271,49 +366,88 @@ __global__ void __launch_bounds__(THREADS, 1) k_sweep_res(const View v, const Re
         const ResPlane pi = s_plane[pl];
         const ResRep* rr = s_rep + pi.rep;
         const int z = pi.z;
-        const int ds = rr->ds;
+        const uint32_t ds2 = (uint32_t)rr->ds * 2u, d2 = (uint32_t)rr->d * 2u;
         const bool remote_p = pi.zp_pl < 0, remote_m = pi.zm_pl < 0;
         const int e_zp = remote_p ? 0 : pi.zp_pl * LH + i, e_zm = remote_m ? 0 : pi.zm_pl * LH + i;
-        const int zq_p = z + 1 == L ? 0 : z + 1, zq_m = z == 0 ? L - 1 : z - 1;
-        long long m_eb = 0, m_ef = 0, m_ms = 0;
+        const int zq_p = (z + 1) & (L - 1), zq_m = (z - 1) & (L - 1);
 
+        // dependencies: the blocks of my plane and of its z-neighbours have finished phase p-1;
+        // remote neighbour planes: their owners have published phase p-1
+        if (p > 0) {
+            const int b_zp = remote_p ? eb : e_zp >> 5, b_zm = remote_m ? eb : e_zm >> 5;
+            const bool ok = lds_volatile(s_done + eb) >= p && lds_volatile(s_done + b_zp) >= p && lds_volatile(s_done + b_zm) >= p;
+            if (btask || !__all_sync(0xFFFFFFFFu, ok))
+                res_wait_slow(s_done, eb, b_zp, b_zm, p, remote_p ? rp.prog + pi.zp_owner : nullptr,
+                              remote_m ? rp.prog + pi.zm_owner : nullptr, (rp.epoch << 8) | (uint32_t)p, rp.diag);
+            __threadfence_block();
+        }
+
+        long long m_eb = 0, m_ef = 0, m_ms = 0;
 #pragma unroll 1
         for (int s = 0; s < 2; ++s) {
             const int ys = (s + z) & 1, y = 2 * i + ys;
             const int dir = (s + c) & 1;              // 0: second x-neighbour at xh-1, 1: at xh+1 (warp-uniform)
-            const int blk = ((rr->d * 2 + c) * L + z) * 2 + s;                  // field block of this (colour, plane, class)
+            // row addresses: shared arrays [colour][class][piece][row]
+            const int e0 = e - i;                     // first row of my plane
+            const int i_yp = ys ? ((i + 1) & (LH - 1)) : i, i_ym = ys ? i : ((i - 1) & (LH - 1));
+            const uint32_t a_x = A(oc, s, 0, e), a_me = A(c, s, 0, e);
+            const uint32_t o_t = A(oc, 1 - s, 0, 0);
+            const uint32_t a_yp = o_t + (uint32_t)(e0 + i_yp) * 16u, a_ym = o_t + (uint32_t)(e0 + i_ym) * 16u;
+            const uint32_t a_zp = o_t + (uint32_t)e_zp * 16u, a_zm = o_t + (uint32_t)e_zm * 16u;
+            const uint32_t rowoff = (uint32_t)(z * L + y) * ROWB;               // byte offset of the row inside a colour array
+            const uint8_t* g_zp = v.spins + (size_t)((ds2 + oc) * nh32 + (uint32_t)(zq_p * L + y) * ROWB);
+            const uint8_t* g_zm = v.spins + (size_t)((ds2 + oc) * nh32 + (uint32_t)(zq_m * L + y) * ROWB);
 
-            // dependencies: the blocks of my plane and of its z-neighbours have finished phase p-1;
-            // remote neighbour planes: their owners have published phase p-1
-            if (s == 0 && p > 0) {
-                const uint32_t want = (rp.epoch << 8) | (uint32_t)p;
-                const int b_zp = remote_p ? eb : e_zp >> 5, b_zm = remote_m ? eb : e_zm >> 5;
-                int spins = 0;
-                for (;;) {
-                    bool ok = lds_volatile(s_done + eb) >= p && lds_volatile(s_done + b_zp) >= p && lds_volatile(s_done + b_zm) >= p;
-                    if (btask) {
-                        if (remote_p) ok = ok && (int32_t)(ld_acquire_gpu(rp.prog + pi.zp_owner) - want) >= 0;
-                        if (remote_m) ok = ok && (int32_t)(ld_acquire_gpu(rp.prog + pi.zm_owner) - want) >= 0;
+            if (meas) {
+                // ---- measurement: Eb over this colour-0 row, Msum and Ef over both colours of it -------------------
+                if (valid) {
+#pragma unroll 1
+                    for (int k = 0; k < K; ++k) {
+                        const ResPiece pc = res_load_piece<K>(smem, a_x, a_yp, a_ym, a_zp, a_zm, a_me, k, dir, remote_p, remote_m, g_zp, g_zm);
+                        int sn = 0, s0 = 0, nn = 0, s1 = 0;   // 64 sum s0 n1, 8 sum s0, 8 sum n1, 8 sum s1
+#pragma unroll
+                        for (int w = 0; w < 4; ++w) {
+                            sn += dot4(pc.me[w], pc.ns[w]); s0 += dot4(pc.me[w], 0x01010101u);
+                            nn += dot4(pc.ns[w], 0x01010101u); s1 += dot4(pc.cw[w], 0x01010101u);
+                        }
+                        // sum (2 s0 - 1)(2 n1 - 6) = 4 s0.n1 - 12 s0 - 2 n1 + 6 per site
+                        m_eb += sn / 16 - 12 * (s0 / 8) - 2 * (nn / 8) + 6 * 16;
+                        m_ms += 2 * ((s0 + s1) / 8) - 2 * 16;
+                        if (KIND == 0) {
+                            // sum (2 hb - 1)(2 s - 1) = 4 hb.s - 2 hb - 2 s + 1 per site; hb = 0x10 flags in natural colour order
+                            const uint4 h0 = __ldg(reinterpret_cast<const uint4*>(v.fieldb + (size_t)((d2 + 0) * nh32 + rowoff)) + k);
+                            const uint4 h1 = __ldg(reinterpret_cast<const uint4*>(v.fieldb + (size_t)((d2 + 1) * nh32 + rowoff)) + k);
+                            const uint32_t a0[4] = {h0.x >> 4, h0.y >> 4, h0.z >> 4, h0.w >> 4};   // 0/1 per byte
+                            const uint32_t a1[4] = {h1.x >> 4, h1.y >> 4, h1.z >> 4, h1.w >> 4};
+                            int hs0 = 0, hh = 0;
+#pragma unroll
+                            for (int w = 0; w < 4; ++w) {
+                                hs0 += dot4(a0[w], pc.me[w]) + dot4(a1[w], pc.cw[w]);                 // 8 sum hb s
+                                hh += dot4(a0[w], 0x01010101u) + dot4(a1[w], 0x01010101u);
+                            }
+                            m_ef += 4 * (hs0 / 8) - 2 * hh - 2 * ((s0 + s1) / 8) + 2 * 16;
+                        } else {
+                            const int4* g0 = reinterpret_cast<const int4*>(v.fieldg + (size_t)((d2 + 0) * nh32 + rowoff)) + 4 * k;
+                            const int4* g1 = reinterpret_cast<const int4*>(v.fieldg + (size_t)((d2 + 1) * nh32 + rowoff)) + 4 * k;
+                            long long ef = 0;
+#pragma unroll
+                            for (int w = 0; w < 4; ++w) {
+                                const int4 b0 = __ldg(g0 + w), b1 = __ldg(g1 + w);
+                                const int ga[4] = {b0.x, b0.y, b0.z, b0.w}, gb[4] = {b1.x, b1.y, b1.z, b1.w};
+                                int part = 0;                 // |g| <= 2^23: eight terms fit easily
+#pragma unroll
+                                for (int j = 0; j < 4; ++j) {
+                                    part += ((pc.me[w] >> (8 * j)) & kResSP) ? ga[j] : -ga[j];
+                                    part += ((pc.cw[w] >> (8 * j)) & kResSP) ? gb[j] : -gb[j];
+                                }
+                                ef += part;
+                            }
+                            m_ef += ef;
+                        }
                     }
-                    if (__all_sync(0xFFFFFFFFu, ok)) break;
-                    backoff();
-                    if (++spins > (1 << 22)) { if (lane == 0) atomicOr(rp.diag, 1ull); break; }
                 }
-                __threadfence_block();
+                continue;
             }
-
-            // row addresses: shared arrays [colour][class][piece][row], pieces Ecap apart
-            const int e_yp = pl * LH + (ys ? (i + 1 == LH ? 0 : i + 1) : i);
-            const int e_ym = pl * LH + (ys ? i : (i == 0 ? LH - 1 : i - 1));
-            const uint4* a_x = s_sp + A(oc, s, 0, e);
-            const uint4* a_yp = s_sp + A(oc, 1 - s, 0, e_yp);
-            const uint4* a_ym = s_sp + A(oc, 1 - s, 0, e_ym);
-            const uint4* a_zp = s_sp + A(oc, 1 - s, 0, e_zp);
-            const uint4* a_zm = s_sp + A(oc, 1 - s, 0, e_zm);
-            uint4* a_me = s_sp + A(c, s, 0, e);
-            const long long rowoff = ((long long)z * L + y) * ROWB;             // byte offset of the row inside a colour array
-            const uint8_t* g_zp = v.spins + ((long long)ds * 2 + oc) * v.Nh + ((long long)zq_p * L + y) * ROWB;
-            const uint8_t* g_zm = v.spins + ((long long)ds * 2 + oc) * v.Nh + ((long long)zq_m * L + y) * ROWB;
 
             // per-row constants
             uint32_t rk[20];
@@ -331,114 +465,34 @@ __global__ void __launch_bounds__(THREADS, 1) k_sweep_res(const View v, const Re
             const uint32_t tab_addr = tab0 + (uint32_t)pi.rep * kResTabBytes;
             const float band = rr->band;
             const uint32_t q0 = (uint32_t)W * (uint32_t)(y + L * z);
+            const uint32_t blk = ((d2 + (uint32_t)c) * L + (uint32_t)z) * 2u + (uint32_t)s;   // field block of this (colour, plane, class)
+            const float4* fp = reinterpret_cast<const float4*>(rp.fielda_res) + (size_t)(blk * (W * LH) + (uint32_t)i);
+            const uint4* fq = reinterpret_cast<const uint4*>(rp.fieldb_res) + (size_t)(blk * (K * LH) + (uint32_t)i);
 
 #pragma unroll
-            for (int k = 0; k < K; ++k) {           // one 16-site piece of the row at a time
+            for (int k = 0; k < K; ++k) {             // one 16-site piece of the row at a time
                 // field of the piece: issued first, consumed last
                 float4 fa[4];
                 uint4 fb = make_uint4(0u, 0u, 0u, 0u);
-                if (KIND == 0) {
-                    if (!meas) fb = __ldg(reinterpret_cast<const uint4*>(rp.fieldb_res) + (blk * K + k) * LH + i);
-                } else if (!meas) {
-                    const float4* fp = reinterpret_cast<const float4*>(rp.fielda_res) + (blk * W + 4 * k) * LH + i;
-#pragma unroll
-                    for (int w = 0; w < 4; ++w) fa[w] = __ldg(fp + w * LH);
-                }
-
-                // ---- neighbour words: ns = SP * (number of up neighbours) per byte ---------------------------------
-                const uint4 x = a_x[k * Ecap];
-                const uint4 yp = a_yp[k * Ecap];
-                const uint4 ym = a_ym[k * Ecap];
-                uint4 zp, zm;
-                if (!remote_p) zp = a_zp[k * Ecap];
+                if (KIND == 0) fb = __ldg(fq + k * LH);
                 else {
-                    zp = ld_cg16(g_zp + 16 * k);
-                    zp.x *= kResSP; zp.y *= kResSP; zp.z *= kResSP; zp.w *= kResSP;
+#pragma unroll
+                    for (int w = 0; w < 4; ++w) fa[w] = __ldg(fp + (4 * k + w) * LH);
                 }
-                if (!remote_m) zm = a_zm[k * Ecap];
-                else {
-                    zm = ld_cg16(g_zm + 16 * k);
-                    zm.x *= kResSP; zm.y *= kResSP; zm.z *= kResSP; zm.w *= kResSP;
-                }
-                const uint4 m = a_me[k * Ecap];
-                // the word holding the far x-neighbour of the piece's edge byte (periodic in x)
-                uint32_t edge;
-                if (K == 1) edge = dir == 0 ? x.w : x.x;
-                else edge = reinterpret_cast<const uint32_t*>(a_x + ((k + K - 1) % K) * Ecap)[dir == 0 ? 3 : 0];
-                const uint32_t cw[4] = {x.x, x.y, x.z, x.w};
-                uint32_t me[4] = {m.x, m.y, m.z, m.w};
-                uint32_t ns[4] = {yp.x + ym.x + zp.x + zm.x, yp.y + ym.y + zp.y + zm.y, yp.z + ym.z + zp.z + zm.z, yp.w + ym.w + zp.w + zm.w};
-                if (dir == 0) {
-                    ns[0] += cw[0] + __funnelshift_r(edge, cw[0], 24);
-#pragma unroll
-                    for (int w = 1; w < 4; ++w) ns[w] += cw[w] + __funnelshift_r(cw[w - 1], cw[w], 24);
-                } else {
-#pragma unroll
-                    for (int w = 0; w < 3; ++w) ns[w] += cw[w] + __funnelshift_r(cw[w], cw[w + 1], 8);
-                    ns[3] += cw[3] + __funnelshift_r(cw[3], edge, 8);
-                }
-
-                if (meas) {
-                    // ---- measurement: Eb over this colour-0 piece, Msum and Ef over both colours of it ---------------
-                    if (valid) {
-                        int sn = 0, s0 = 0, nn = 0, s1 = 0;   // 64 sum s0 n1, 8 sum s0, 8 sum n1, 8 sum s1
-#pragma unroll
-                        for (int w = 0; w < 4; ++w) {
-                            sn += dot4(me[w], ns[w]); s0 += dot4(me[w], 0x01010101u);
-                            nn += dot4(ns[w], 0x01010101u); s1 += dot4(cw[w], 0x01010101u);
-                        }
-                        // sum (2 s0 - 1)(2 n1 - 6) = 4 s0.n1 - 12 s0 - 2 n1 + 6 per site
-                        m_eb += sn / 16 - 12 * (s0 / 8) - 2 * (nn / 8) + 6 * 16;
-                        m_ms += 2 * ((s0 + s1) / 8) - 2 * 16;
-                        if (KIND == 0) {
-                            // sum (2 hb - 1)(2 s - 1) = 4 hb.s - 2 hb - 2 s + 1 per site; hb = 0x10 flags in natural colour order
-                            const uint4 h0 = __ldg(reinterpret_cast<const uint4*>(v.fieldb + ((long long)rr->d * 2 + 0) * v.Nh + rowoff) + k);
-                            const uint4 h1 = __ldg(reinterpret_cast<const uint4*>(v.fieldb + ((long long)rr->d * 2 + 1) * v.Nh + rowoff) + k);
-                            const uint32_t a0[4] = {h0.x >> 4, h0.y >> 4, h0.z >> 4, h0.w >> 4};   // 0/1 per byte
-                            const uint32_t a1[4] = {h1.x >> 4, h1.y >> 4, h1.z >> 4, h1.w >> 4};
-                            int hs0 = 0, hh = 0;
-#pragma unroll
-                            for (int w = 0; w < 4; ++w) {
-                                hs0 += dot4(a0[w], me[w]) + dot4(a1[w], cw[w]);                       // 8 sum hb s
-                                hh += dot4(a0[w], 0x01010101u) + dot4(a1[w], 0x01010101u);
-                            }
-                            m_ef += 4 * (hs0 / 8) - 2 * hh - 2 * ((s0 + s1) / 8) + 2 * 16;
-                        } else {
-                            const int4* g0 = reinterpret_cast<const int4*>(v.fieldg + ((long long)rr->d * 2 + 0) * v.Nh + rowoff) + 4 * k;
-                            const int4* g1 = reinterpret_cast<const int4*>(v.fieldg + ((long long)rr->d * 2 + 1) * v.Nh + rowoff) + 4 * k;
-                            long long ef = 0;
-#pragma unroll
-                            for (int w = 0; w < 4; ++w) {
-                                const int4 b0 = __ldg(g0 + w), b1 = __ldg(g1 + w);
-                                const int ga[4] = {b0.x, b0.y, b0.z, b0.w}, gb[4] = {b1.x, b1.y, b1.z, b1.w};
-                                int part = 0;                 // |g| <= 2^23: eight terms fit easily
-#pragma unroll
-                                for (int j = 0; j < 4; ++j) {
-                                    part += ((me[w] >> (8 * j)) & kResSP) ? ga[j] : -ga[j];
-                                    part += ((cw[w] >> (8 * j)) & kResSP) ? gb[j] : -gb[j];
-                                }
-                                ef += part;
-                            }
-                            m_ef += ef;
-                        }
-                    }
-                    continue;
-                }
-
+                ResPiece pc = res_load_piece<K>(smem, a_x, a_yp, a_ym, a_zp, a_zm, a_me, k, dir, remote_p, remote_m, g_zp, g_zm);
                 const uint32_t fw[4] = {fb.x, fb.y, fb.z, fb.w};
                 uint32_t idx8[4];
 #pragma unroll
-                for (int w = 0; w < 4; ++w) idx8[w] = ns[w] + (me[w] << 3) + (KIND == 0 ? fw[w] : 0u);
+                for (int w = 0; w < 4; ++w) idx8[w] = pc.ns[w] + (pc.me[w] << 3) + (KIND == 0 ? fw[w] : 0u);
 
                 // ---- the four words of the piece ---------------------------------------------------------------
-                uint32_t ambmask = 0;
+                float mn = 3.0e38f;                   // smallest |d| of the piece (Gaussian)
 #pragma unroll
                 for (int w = 0; w < 4; ++w) {
                     const Words4 r = philox_rkreg(rk, q0 + (uint32_t)(4 * k + w), sweep, slot, dom);
                     const uint32_t u[4] = {r.w0, r.w1, r.w2, r.w3};
-                    uint32_t flips;
                     if (KIND == 0) {
-                        flips = 0;
+                        uint32_t flips = 0;
 #pragma unroll
                         for (int j = 0; j < 4; ++j) {
                             const uint2 ent = lds64(__byte_perm(idx8[w], tab_addr, 0x7650 + j));
@@ -446,42 +500,30 @@ __global__ void __launch_bounds__(THREADS, 1) k_sweep_res(const View v, const Re
                             if (NEVER) acc = acc && ent.y == 0u;
                             if (acc) flips |= kResSP << (8 * j);
                         }
+                        pc.me[w] ^= flips;
                     } else {
                         const float a[4] = {fa[w].x, fa[w].y, fa[w].z, fa[w].w};
-                        uint32_t db[4];
-                        bool amb = false;
+                        float d[4];
 #pragma unroll
-                        for (int j = 0; j < 4; ++j) {
-                            const uint2 ent = lds64(__byte_perm(idx8[w], tab_addr, 0x7650 + j));
-                            const float P = ex2_approx(fmaf(a[j], __uint_as_float(ent.y), __uint_as_float(ent.x)));
-                            const float d = __uint2float_rn(u[j]) - P;
-                            amb = amb || (fabsf(d) < band);
-                            db[j] = __float_as_uint(d);
-                        }
+                        for (int j = 0; j < 4; ++j) d[j] = res_gauss_diff(idx8[w], j, tab_addr, a[j], u[j]);
+                        mn = fminf(fminf(mn, fminf(fabsf(d[0]), fabsf(d[1]))), fminf(fabsf(d[2]), fabsf(d[3])));
                         // sign bytes of the four differences -> 0xFF where d < 0 (accept)
-                        const uint32_t m01 = prmt(db[0], db[1], 0x00FBu);
-                        const uint32_t m23 = prmt(db[2], db[3], 0xFB00u);
-                        flips = prmt(m01, m23, 0x7610u) & (kResSP * 0x01010101u);
-                        if (amb) ambmask |= 1u << w;
+                        const uint32_t m01 = prmt(__float_as_uint(d[0]), __float_as_uint(d[1]), 0x00FBu);
+                        const uint32_t m23 = prmt(__float_as_uint(d[2]), __float_as_uint(d[3]), 0xFB00u);
+                        pc.me[w] ^= prmt(m01, m23, 0x7610u) & (kResSP * 0x01010101u);
                     }
-                    me[w] ^= flips;
                 }
-                if (KIND == 1 && ambmask != 0u) {       // rare: redo the flagged words with the exact binary64 rule
-                    const int32_t* grow = v.fieldg + ((long long)rr->d * 2 + c) * v.Nh + rowoff + 16 * k;
-                    const double beta = rr->beta;
-#pragma unroll
-                    for (int w = 0; w < 4; ++w)
-                        if ((ambmask >> w) & 1u)
-                            me[w] = ((idx8[w] >> 3) & (kResSP * 0x01010101u)) ^
-                                    res_gauss_word_exact(v, idx8[w], grow + 4 * w, beta, rr->rk[0], rr->rk[1], q0 + (uint32_t)(4 * k + w), sweep, slot, dom);
-                }
+                uint4 nw = make_uint4(pc.me[0], pc.me[1], pc.me[2], pc.me[3]);
+                if (KIND == 1 && mn < band)             // rare: some site needs the exact binary64 rule
+                    nw = res_gauss_piece_fix(v, make_uint4(idx8[0], idx8[1], idx8[2], idx8[3]), tab_addr, band, fp + 4 * k * LH, LH,
+                                             v.fieldg + (size_t)((d2 + (uint32_t)c) * nh32 + rowoff + 16u * k), rr, q0 + 4u * k, sweep, dom);
 
                 // ---- write back ---------------------------------------------------------------------------------
                 if (valid) {
-                    a_me[k * Ecap] = make_uint4(me[0], me[1], me[2], me[3]);
+                    *reinterpret_cast<uint4*>(smem + a_me + k * ARR) = nw;
                     if (remote_p || remote_m)
-                        *reinterpret_cast<uint4*>(v.spins + ((long long)ds * 2 + c) * v.Nh + rowoff + 16 * k) =
-                            make_uint4(me[0] >> 3, me[1] >> 3, me[2] >> 3, me[3] >> 3);
+                        *reinterpret_cast<uint4*>(v.spins + (size_t)((ds2 + (uint32_t)c) * nh32 + rowoff + 16u * k)) =
+                            make_uint4(nw.x >> 3, nw.y >> 3, nw.z >> 3, nw.w >> 3);
                 }
             }
         }
@@ -531,7 +573,7 @@ __global__ void __launch_bounds__(THREADS, 1) k_sweep_res(const View v, const Re
             const int k = u % K, y = (u / K) % L, col = (u / (K * L)) & 1, p = u / (2 * K * L);
             const ResPlane pi = s_plane[p];
             const int ds = s_rep[pi.rep].ds, z = pi.z;
-            uint4 x = s_sp[A(col, (y + z) & 1, k, p * LH + (y >> 1))];
+            uint4 x = *reinterpret_cast<const uint4*>(smem + A(col, (y + z) & 1, k, p * LH + (y >> 1)));
             x.x >>= 3; x.y >>= 3; x.z >>= 3; x.w >>= 3;
             *reinterpret_cast<uint4*>(v.spins + ((long long)ds * 2 + col) * v.Nh + ((long long)z * L + y) * ROWB + 16 * k) = x;
         }
