@@ -37,7 +37,7 @@ __device__ __noinline__ bool gauss_accept_exact(const View& v, int sbit, int n1,
 }
 
 // Gaussian attempt: float estimate with a rigorous guard band, exact binary64 rule inside the band.
-// tab = this rank's 16-entry table, a = (float)(hs*g).
+// tab = this rank's 16-entry table, a = (float)g (exact; the table's y carries hs).
 __device__ __forceinline__ bool gauss_accept(const View& v, const GaussEntry* __restrict__ tab, float band, double beta,
                                              int sbit, int n1, float a, int32_t g, uint32_t u) {
     const GaussEntry e = tab[n1 | (sbit << 3)];
@@ -244,14 +244,13 @@ __global__ void k_reduce_site(View v) {
 
 // ---- exchange step (S6): one CTA per member ------------------
 // record != 0: append the row to the time series at index `row`.  The accumulators are consumed (zeroed).
-__global__ void k_exchange(View v, uint32_t xstep, long long row, int record) {
-    const int d = blockIdx.x;
+__device__ __forceinline__ void exchange_member(const View& v, int d, uint32_t xstep, long long row, int record) {
     const int n = v.n, R = v.R;
     int32_t* t2r = v.t2r + d * R;
     int32_t* r2t = v.r2t + d * R;
     for (int t = threadIdx.x; t < n; t += blockDim.x) {
         long long* a = v.acc + (long long)(d * R + t2r[t]) * 3;
-        const long long eb = a[0], ef = a[1], ms = a[2];
+        const long long eb = __ldcg(a + 0), ef = __ldcg(a + 1), ms = __ldcg(a + 2);   // written by other CTAs' atomics: read at L2
         a[0] = 0; a[1] = 0; a[2] = 0;
         if (record) {
             long long* s = v.series + ((row * v.D + d) * R + t) * 3;
@@ -282,6 +281,10 @@ __global__ void k_exchange(View v, uint32_t xstep, long long row, int record) {
             v.accn[d * R + t] += 1ull;
         }
     }
+}
+
+__global__ void k_exchange(View v, uint32_t xstep, long long row, int record) {
+    exchange_member(v, (int)blockIdx.x, xstep, row, record);
 }
 
 }  // namespace rfim

@@ -31,6 +31,7 @@ constexpr double kTwo32 = 4294967296.0;
 constexpr double kFieldScale = 1048576.0;   // 2^20
 constexpr int32_t kFieldClamp = 8 * 1048576;
 constexpr int kResMaxGrid = 255;            // owners are stored in 8 bits (sweep_res.cuh)
+constexpr int kResFusedExchangeMaxD = 4;    // the last CTA runs the exchange step itself for batches up to this size
 
 }  // namespace
 
@@ -175,7 +176,7 @@ int upload_field(rfim_pt* h, int d) {
             int c; const long long j = layout_index(h, x, y, z, &c);
             const int32_t g = f[x + (long long)L * (y + (long long)L * z)];
             const double a = hs * (double)g;
-            fa[(long long)c * h->Nh + j] = (float)a;
+            fa[(long long)c * h->Nh + j] = (float)g;              // |g| <= 2^23: exact
             fg[(long long)c * h->Nh + j] = g;
             amax = std::max(amax, std::fabs(a));
         }
@@ -184,7 +185,7 @@ int upload_field(rfim_pt* h, int d) {
         if (h->fielda_res) {
             std::vector<float> fr(h->N);
             for (int z = 0; z < L; ++z) for (int y = 0; y < L; ++y) for (int x = 0; x < L; ++x)
-                fr[res_field_index(h, x, y, z)] = (float)(hs * (double)f[x + (long long)L * (y + (long long)L * z)]);
+                fr[res_field_index(h, x, y, z)] = (float)f[x + (long long)L * (y + (long long)L * z)];
             CU(cudaMemcpyAsync(h->fielda_res + (long long)d * h->N, fr.data(), h->N * sizeof(float), cudaMemcpyHostToDevice, h->stream));
             CU(cudaStreamSynchronize(h->stream));
         }
@@ -234,13 +235,13 @@ int upload_tables(rfim_pt* h) {
         for (int d = 0; d < D; ++d)
             for (int t = 0; t < n; ++t) {
                 const double b = beta[(size_t)d * R + t];
-                const double c = -2.0 * b * M_LOG2E;              // log2 P = c * sigma * (J n + a) ; +32 for the 2^32 scale
+                const double c = -2.0 * b * M_LOG2E;              // log2 P = c * sigma * (J n + hs g) ; +32 for the 2^32 scale
                 for (int idx = 0; idx < 16; ++idx) {
                     const int n1 = idx & 7, s = (idx >> 3) & 1;
                     const double sigma = s ? 1.0 : -1.0;
                     GaussEntry e;
                     e.x = (float)(c * sigma * h->J * (double)(2 * n1 - 6) + 32.0);
-                    e.y = (float)(c * sigma);
+                    e.y = (float)(c * sigma * h->v.hs);           // multiplies (float)g_i, which is exact
                     gtab[((size_t)d * R + t) * 16 + idx] = e;
                 }
                 // guard band: bound on |P~ - P| over the float path, in units of u
@@ -409,12 +410,18 @@ int launch_res_u(rfim_pt* h, const ResPlan& pl, const ResParams& rp) {
 }
 
 // `sweeps` (<= 127) sweeps of every active replica of every member in one cooperative launch
-int launch_res(rfim_pt* h, int sweeps, bool measure) {
+int launch_res(rfim_pt* h, int sweeps, bool measure, bool* exchanged) {
     const ResPlan pl = res_plan(h);
     if (!pl.ok) return fail(h, RFIM_EINVAL, "resident kernel: the planes of one CTA do not fit in shared memory");
     ResParams rp{};
     rp.phases = 2 * sweeps;
     rp.measure = measure ? 1 : 0;
+    rp.exchange = (measure && h->D <= kResFusedExchangeMaxD) ? 1 : 0;
+    rp.nact = pl.q > 0 ? pl.grid : pl.rem;
+    rp.xstep = (uint32_t)h->xstep;
+    rp.xrow = h->series_steps;
+    rp.ticket = h->res_prog + kResMaxGrid;       // the word after the progress words (zeroed at create, left at zero)
+    *exchanged = rp.exchange != 0;
     rp.sweep0 = (uint32_t)h->sweep_g;
     rp.epoch = ++h->res_epoch;
     rp.prog = h->res_prog;
@@ -471,13 +478,14 @@ int do_sweeps(rfim_pt* h, int64_t n_sweeps, int k) {
         }
         // the resident kernel measures in the same launch when its chunk ends on an exchange step
         const bool step_after = k > 0 && ((h->sweep_g + (uint64_t)chunk) % (uint64_t)k) == 0;
-        int rc = variant == 4 ? launch_res(h, (int)chunk, step_after) : (flow ? launch_flow(h, (int)chunk) : launch_sweep(h));
+        bool exchanged = false;
+        int rc = variant == 4 ? launch_res(h, (int)chunk, step_after, &exchanged) : (flow ? launch_flow(h, (int)chunk) : launch_sweep(h));
         if (rc) return rc;
         h->sweep_g += (uint64_t)chunk;
         left -= chunk;
         if (step_after) {
             if (variant != 4 && (rc = launch_reduce(h))) return rc;
-            if ((rc = launch_exchange(h))) return rc;
+            if (!exchanged && (rc = launch_exchange(h))) return rc;
             h->series_steps += 1;
             h->xstep += 1;
         }

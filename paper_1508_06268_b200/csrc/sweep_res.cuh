@@ -19,10 +19,13 @@
 // only ever waits for lower-numbered tasks, so the lowest outstanding task can always run: no
 // deadlock, no tail at the end of a phase.
 //
-// Measurement (S5) is one more pseudo-phase of colour 0 at the end of the launch: the same
-// neighbour words give Eb = sum over colour-0 sites of s_i * (six-neighbour sum), Msum and Ef are
-// summed over both colours of the row, per replica in shared memory, then added to View::acc with
-// integer atomics (order-independent, hence deterministic).
+// Measurement (S5) rides on the last two phases of the launch, from registers the update holds
+// anyway: each phase sums Msum and Ef of the colour it has just updated (the field copy stores g_i as
+// exact floats), and since every bond has exactly one colour-1 end the colour-1 phase also gives
+// Eb = sum over colour-1 sites of s_i' * (six-neighbour sum).  Sums go per replica to shared memory,
+// then to View::acc with integer atomics (order-independent, hence deterministic).  The
+// CTA that finishes last then runs the exchange step itself (small batches), so a whole
+// parallel-tempering move is one launch.
 //
 // In shared memory a spin is a byte holding 0 or SP (= 8), four same-colour sites per 32-bit word
 // exactly as in global memory (where it is 0/1), so the six-neighbour count of four sites is a few
@@ -69,14 +72,19 @@ __host__ __device__ constexpr int res_max_planes(int L) { return L == 64 ? ResGe
 
 struct ResParams {
     int phases;                  // 2 * sweeps of this launch, <= 254
-    int measure;                 // != 0: finish with the measurement pseudo-phase (Eb, Ef, Msum -> View::acc)
+    int measure;                 // != 0: the last phase also measures (Eb, Ef, Msum -> View::acc)
+    int exchange;                // != 0: the CTA that finishes last runs the exchange step of every member
+    int nact;                    // CTAs that own planes
+    uint32_t xstep;              // exchange step index, time-series row, record flag (exchange != 0)
+    long long xrow;
+    uint32_t* ticket;            // arrival counter of the fused exchange (left at zero)
     uint32_t sweep0;             // global sweep index of phase 0
     uint32_t epoch;              // launch id: progress words hold (epoch << 8) | phases published
     uint32_t* prog;              // [grid]
     int total_planes;            // D * n * L
     int q, rem;                  // run of CTA b: start = b*q + min(b, rem), count = q + (b < rem)
     int cap_reps;                // replicas a run can touch -- same carve for every CTA
-    const float* fielda_res;     // Gaussian: [D][2][L][2][4K][L/2] float4 (task order), (float)(hs * g_i)
+    const float* fielda_res;     // Gaussian: [D][2][L][2][4K][L/2] float4 (task order), (float)g_i (exact)
     const uint8_t* fieldb_res;   // bimodal:  [D][2][L][2][K][L/2] uint4, 0x80 where h_i = +1
     unsigned long long* diag;
     uint32_t rk0[20];            // Philox round keys of member 0 (used from the constant bank when D == 1)
@@ -146,7 +154,7 @@ __device__ __forceinline__ Words4 philox_rkreg(const uint32_t (&rk)[20], uint32_
     return w;
 }
 
-// the float path of one Gaussian attempt: d = float(u) - P~, P~ = 2^(a*y + x); accept iff d < 0 unless |d| < band
+// the float path of one Gaussian attempt: d = float(u) - P~, P~ = 2^(g*y + x); accept iff d < 0 unless |d| < band
 __device__ __forceinline__ float res_gauss_diff(uint32_t idx8, int j, uint32_t tab_addr, float a, uint32_t u) {
     const uint2 ent = lds64(__byte_perm(idx8, tab_addr, 0x7650 + j));
     const float P = ex2_approx(fmaf(a, __uint_as_float(ent.y), __uint_as_float(ent.x)));
@@ -236,6 +244,45 @@ __device__ __forceinline__ ResPiece res_load_piece(const uint8_t* smem, uint32_t
         pc.ns[3] += __funnelshift_r(pc.cw[3], edge, 8);
     }
     return pc;
+}
+
+// Measurement of one piece, taken in the last two phases of a launch from what the update holds in registers:
+// me = updated words of the piece, fb / f0..f3 = the piece's field (bimodal 0x80 flags / Gaussian g_i as floats, exact),
+// idx8 = table offsets before the update (bits 3..5 of a byte = SP * n1).  Returns {Eb, Ef, Msum} contributions of the
+// piece's 16 sites: Ef and Msum of this colour always, Eb (the six-neighbour form: every bond has one colour-1 end)
+// only when with_eb, i.e. in the colour-1 phase.  Ef fits an int: 16 terms below 2^23.
+template <int KIND>
+__device__ __noinline__ int3 res_measure_piece(uint4 mev, uint4 idx8v, uint4 fbv, float4 f0, float4 f1, float4 f2, float4 f3, int with_eb) {
+    const uint32_t me[4] = {mev.x, mev.y, mev.z, mev.w};
+    const uint32_t ns[4] = {idx8v.x & 0x38383838u, idx8v.y & 0x38383838u, idx8v.z & 0x38383838u, idx8v.w & 0x38383838u};
+    int sn = 0, s0 = 0, nn = 0;                   // 64 sum s n1, 8 sum s, 8 sum n1
+#pragma unroll
+    for (int w = 0; w < 4; ++w) {
+        sn += dot4(me[w], ns[w]); s0 += dot4(me[w], 0x01010101u); nn += dot4(ns[w], 0x01010101u);
+    }
+    int3 r;
+    r.x = with_eb ? sn / 16 - 12 * (s0 / 8) - 2 * (nn / 8) + 6 * 16 : 0;     // sum (2 s - 1)(2 n1 - 6) = 4 s.n1 - 12 s - 2 n1 + 6 per site
+    r.z = 2 * (s0 / 8) - 16;
+    if (KIND == 0) {
+        // sum (2 hb - 1)(2 s - 1) = 4 hb.s - 2 hb - 2 s + 1 per site
+        const uint32_t hb[4] = {fbv.x >> 7, fbv.y >> 7, fbv.z >> 7, fbv.w >> 7};   // 0/1 per byte
+        int hs0 = 0, hh = 0;
+#pragma unroll
+        for (int w = 0; w < 4; ++w) { hs0 += dot4(hb[w], me[w]); hh += dot4(hb[w], 0x01010101u); }
+        r.y = 4 * (hs0 / 8) - 2 * hh - 2 * (s0 / 8) + 16;
+    } else {
+        const float gf[16] = {f0.x, f0.y, f0.z, f0.w, f1.x, f1.y, f1.z, f1.w, f2.x, f2.y, f2.z, f2.w, f3.x, f3.y, f3.z, f3.w};
+        int ef = 0;
+#pragma unroll
+        for (int w = 0; w < 4; ++w)
+#pragma unroll
+            for (int j = 0; j < 4; ++j) {
+                const int g = __float2int_rn(gf[4 * w + j]);
+                ef += ((me[w] >> (8 * j)) & kResSP) ? g : -g;
+            }
+        r.y = ef;
+    }
+    return r;
 }
 
 // K = 16-byte pieces per row per colour (L = 32 K); UNI: one member, round keys come from the constant bank
@@ -340,7 +387,7 @@ __global__ void __launch_bounds__(THREADS, 1) k_sweep_res(const View v, const Re
     }
     __syncthreads();
     const int n_bblocks = s_ctl[3];
-    const int total_tasks = nb * (rp.phases + (rp.measure ? 1 : 0));
+    const int total_tasks = nb * rp.phases;
     const uint32_t tab0 = (uint32_t)__cvta_generic_to_shared(s_tab);
     const uint32_t nh32 = (uint32_t)v.Nh;
 
@@ -353,7 +400,7 @@ __global__ void __launch_bounds__(THREADS, 1) k_sweep_res(const View v, const Re
         if (g >= total_tasks) break;
         while (g - base_cur >= nb) { base_cur += nb; ++p_cur; }
         const int p = p_cur, bidx = g - base_cur;
-        const bool meas = p == rp.phases;             // the measurement pseudo-phase (colour 0; phases is even)
+        const bool meas = rp.measure && p >= rp.phases - 2;   // the last two phases also measure their colour
         const int c = p & 1, oc = 1 - c;
         const uint32_t sweep = rp.sweep0 + (uint32_t)(p >> 1);
         const uint32_t dom = c == 0 ? kDomColour0 : kDomColour1;
@@ -397,57 +444,6 @@ __global__ void __launch_bounds__(THREADS, 1) k_sweep_res(const View v, const Re
             const uint32_t rowoff = (uint32_t)(z * L + y) * ROWB;               // byte offset of the row inside a colour array
             const uint8_t* g_zp = v.spins + (size_t)((ds2 + oc) * nh32 + (uint32_t)(zq_p * L + y) * ROWB);
             const uint8_t* g_zm = v.spins + (size_t)((ds2 + oc) * nh32 + (uint32_t)(zq_m * L + y) * ROWB);
-
-            if (meas) {
-                // ---- measurement: Eb over this colour-0 row, Msum and Ef over both colours of it -------------------
-                if (valid) {
-#pragma unroll 1
-                    for (int k = 0; k < K; ++k) {
-                        const ResPiece pc = res_load_piece<K>(smem, a_x, a_yp, a_ym, a_zp, a_zm, a_me, k, dir, remote_p, remote_m, g_zp, g_zm);
-                        int sn = 0, s0 = 0, nn = 0, s1 = 0;   // 64 sum s0 n1, 8 sum s0, 8 sum n1, 8 sum s1
-#pragma unroll
-                        for (int w = 0; w < 4; ++w) {
-                            sn += dot4(pc.me[w], pc.ns[w]); s0 += dot4(pc.me[w], 0x01010101u);
-                            nn += dot4(pc.ns[w], 0x01010101u); s1 += dot4(pc.cw[w], 0x01010101u);
-                        }
-                        // sum (2 s0 - 1)(2 n1 - 6) = 4 s0.n1 - 12 s0 - 2 n1 + 6 per site
-                        m_eb += sn / 16 - 12 * (s0 / 8) - 2 * (nn / 8) + 6 * 16;
-                        m_ms += 2 * ((s0 + s1) / 8) - 2 * 16;
-                        if (KIND == 0) {
-                            // sum (2 hb - 1)(2 s - 1) = 4 hb.s - 2 hb - 2 s + 1 per site; hb = 0x10 flags in natural colour order
-                            const uint4 h0 = __ldg(reinterpret_cast<const uint4*>(v.fieldb + (size_t)((d2 + 0) * nh32 + rowoff)) + k);
-                            const uint4 h1 = __ldg(reinterpret_cast<const uint4*>(v.fieldb + (size_t)((d2 + 1) * nh32 + rowoff)) + k);
-                            const uint32_t a0[4] = {h0.x >> 4, h0.y >> 4, h0.z >> 4, h0.w >> 4};   // 0/1 per byte
-                            const uint32_t a1[4] = {h1.x >> 4, h1.y >> 4, h1.z >> 4, h1.w >> 4};
-                            int hs0 = 0, hh = 0;
-#pragma unroll
-                            for (int w = 0; w < 4; ++w) {
-                                hs0 += dot4(a0[w], pc.me[w]) + dot4(a1[w], pc.cw[w]);                 // 8 sum hb s
-                                hh += dot4(a0[w], 0x01010101u) + dot4(a1[w], 0x01010101u);
-                            }
-                            m_ef += 4 * (hs0 / 8) - 2 * hh - 2 * ((s0 + s1) / 8) + 2 * 16;
-                        } else {
-                            const int4* g0 = reinterpret_cast<const int4*>(v.fieldg + (size_t)((d2 + 0) * nh32 + rowoff)) + 4 * k;
-                            const int4* g1 = reinterpret_cast<const int4*>(v.fieldg + (size_t)((d2 + 1) * nh32 + rowoff)) + 4 * k;
-                            long long ef = 0;
-#pragma unroll
-                            for (int w = 0; w < 4; ++w) {
-                                const int4 b0 = __ldg(g0 + w), b1 = __ldg(g1 + w);
-                                const int ga[4] = {b0.x, b0.y, b0.z, b0.w}, gb[4] = {b1.x, b1.y, b1.z, b1.w};
-                                int part = 0;                 // |g| <= 2^23: eight terms fit easily
-#pragma unroll
-                                for (int j = 0; j < 4; ++j) {
-                                    part += ((pc.me[w] >> (8 * j)) & kResSP) ? ga[j] : -ga[j];
-                                    part += ((pc.cw[w] >> (8 * j)) & kResSP) ? gb[j] : -gb[j];
-                                }
-                                ef += part;
-                            }
-                            m_ef += ef;
-                        }
-                    }
-                }
-                continue;
-            }
 
             // per-row constants
             uint32_t rk[20];
@@ -524,6 +520,12 @@ __global__ void __launch_bounds__(THREADS, 1) k_sweep_res(const View v, const Re
                     if (remote_p || remote_m)
                         *reinterpret_cast<uint4*>(v.spins + (size_t)((ds2 + (uint32_t)c) * nh32 + rowoff + 16u * k)) =
                             make_uint4(nw.x >> 3, nw.y >> 3, nw.z >> 3, nw.w >> 3);
+                    if (meas) {
+                        const float4 z4 = make_float4(0.f, 0.f, 0.f, 0.f);
+                        const int3 m3 = res_measure_piece<KIND>(nw, make_uint4(idx8[0], idx8[1], idx8[2], idx8[3]), fb,
+                                                                KIND ? fa[0] : z4, KIND ? fa[1] : z4, KIND ? fa[2] : z4, KIND ? fa[3] : z4, c);
+                        m_eb += m3.x; m_ef += m3.y; m_ms += m3.z;
+                    }
                 }
             }
         }
@@ -544,7 +546,6 @@ __global__ void __launch_bounds__(THREADS, 1) k_sweep_res(const View v, const Re
                 atomicAdd(reinterpret_cast<unsigned long long*>(s_acc + 3 * rep + 1), (unsigned long long)m_ef);
                 atomicAdd(reinterpret_cast<unsigned long long*>(s_acc + 3 * rep + 2), (unsigned long long)m_ms);
             }
-            continue;
         }
         __syncwarp();
         if (lane == 0) {
@@ -580,6 +581,21 @@ __global__ void __launch_bounds__(THREADS, 1) k_sweep_res(const View v, const Re
         if (rp.measure)
             for (int r = tid; r < nrep * 3; r += THREADS)
                 atomicAdd(reinterpret_cast<unsigned long long*>(v.acc + (long long)s_rep[r / 3].ds * 3 + r % 3), (unsigned long long)s_acc[r]);
+    }
+    if (rp.exchange) {
+        // the CTA that arrives last has every replica's sums in View::acc (integer atomics at L2): it runs the exchange step
+        __threadfence();
+        __syncthreads();
+        if (tid == 0) s_ctl[0] = (atomicAdd(rp.ticket, 1u) == (uint32_t)(rp.nact - 1)) ? 1 : 0;
+        __syncthreads();
+        if (s_ctl[0]) {
+            __threadfence();
+            for (int d = 0; d < v.D; ++d) {
+                exchange_member(v, d, rp.xstep, rp.xrow, 1);
+                __syncthreads();
+            }
+            if (tid == 0) *rp.ticket = 0u;
+        }
     }
 }
 

@@ -11,7 +11,7 @@
 
 namespace rfim {
 
-struct GaussEntry { float x, y; };   // arg = fma(a_i, y, x): log2 of the acceptance probability, + 32
+struct GaussEntry { float x, y; };   // arg = fma((float)g_i, y, x): log2 of the acceptance probability, + 32
 
 struct View {
     int L, Lh, R, n, D, kind;
@@ -19,7 +19,7 @@ struct View {
     long long N, Nh;
     uint8_t* spins;                // [D][R][2][Nh]
     const uint8_t* fieldb;         // bimodal: [D][2][Nh], 0x10 where h_i = +1, 0 where h_i = -1
-    const float* fielda;           // Gaussian: [D][2][Nh], (float)(h * 2^-20 * g_i)
+    const float* fielda;           // Gaussian: [D][2][Nh], (float)g_i (exact: |g_i| <= 2^23)
     const int32_t* fieldg;         // Gaussian: [D][2][Nh], g_i
     const uint32_t* etab;          // bimodal: [D][R(rank)][32], thr - 1 (accept iff u <= e), idx = n1 | s<<3 | hb<<4
     const uint32_t* never;         // bimodal: [D][R(rank)], bit idx set where thr = 0
