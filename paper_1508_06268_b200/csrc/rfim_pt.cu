@@ -1043,12 +1043,31 @@ int rfim_pt_get_diagnostics(rfim_pt* h, uint64_t diag[4]) {
 // ---- roofline microbenchmarks ---------------------------------------------------------------------
 namespace {
 
-__global__ void k_bench_philox(uint32_t* out, int calls, uint32_t sweep, uint32_t slot) {
-    uint32_t acc = 0, c0 = blockIdx.x * blockDim.x + threadIdx.x;
-    for (int i = 0; i < calls; ++i) {
-        const Words4 w = philox4x32_10(0x9E3779B9u, 0x1234567u, c0, sweep, slot, kDomColour0);
-        acc ^= w.w0 ^ w.w1 ^ w.w2 ^ w.w3;
-        c0 += gridDim.x * blockDim.x;
+// Philox4x32-10 alone, with the sweep's own counter layout (S2): c0 = word index (varies per call), c1 = sweep,
+// c2 = slot, c3 = domain (warp-uniform), round keys from the constant bank; four independent calls in flight per
+// thread.  The compiler hoists the warp-uniform part of the first two rounds exactly as it does in the sweep kernels,
+// so this is the tightest Philox-only bound for this method: ~18 wide multiplies + ~18 three-input XORs per call.
+struct BenchKeys { uint32_t k[20]; };
+__global__ void __launch_bounds__(256) k_bench_philox(uint32_t* out, int calls, BenchKeys rk, uint32_t sweep, uint32_t slot) {
+    constexpr int ILP = 4;
+    uint32_t acc = 0, base = (blockIdx.x * blockDim.x + threadIdx.x) * ILP;
+    for (int i = 0; i < calls; i += ILP) {
+        uint32_t c0[ILP], c1[ILP], c2[ILP], c3[ILP];
+#pragma unroll
+        for (int j = 0; j < ILP; ++j) { c0[j] = base + j; c1[j] = sweep; c2[j] = slot; c3[j] = kDomColour0; }
+#pragma unroll
+        for (int r = 0; r < 10; ++r) {
+#pragma unroll
+            for (int j = 0; j < ILP; ++j) {
+                const uint32_t hi0 = __umulhi(kPhiloxM0, c0[j]), lo0 = kPhiloxM0 * c0[j];
+                const uint32_t hi1 = __umulhi(kPhiloxM1, c2[j]), lo1 = kPhiloxM1 * c2[j];
+                const uint32_t n0 = hi1 ^ c1[j] ^ rk.k[2 * r], n2 = hi0 ^ c3[j] ^ rk.k[2 * r + 1];
+                c1[j] = lo1; c3[j] = lo0; c0[j] = n0; c2[j] = n2;
+            }
+        }
+#pragma unroll
+        for (int j = 0; j < ILP; ++j) acc ^= c0[j] ^ c1[j] ^ c2[j] ^ c3[j];
+        base += gridDim.x * blockDim.x * ILP;
     }
     out[blockIdx.x * blockDim.x + threadIdx.x] = acc;
 }
@@ -1095,9 +1114,15 @@ int rfim_pt_bench_philox(void* stream, int calls_per_thread, double* ms, double*
     const int blocks = sms * 8, threads = 256;
     uint32_t* out = reinterpret_cast<uint32_t*>(dev_alloc((size_t)blocks * threads * 4));
     if (!out) return RFIM_ENOMEM;
-    int rc = time_launch(s, [&] { k_bench_philox<<<blocks, threads, 0, s>>>(out, calls_per_thread, 7u, 3u); }, ms);
+    BenchKeys rk;
+    {
+        uint32_t k0 = 0x9E3779B9u, k1 = 0x1234567u;
+        for (int r = 0; r < 10; ++r) { rk.k[2 * r] = k0; rk.k[2 * r + 1] = k1; k0 += kPhiloxW0; k1 += kPhiloxW1; }
+    }
+    const int calls = (calls_per_thread + 3) / 4 * 4;
+    int rc = time_launch(s, [&] { k_bench_philox<<<blocks, threads, 0, s>>>(out, calls, rk, 7u, 3u); }, ms);
     dev_free(out);
-    *attempts = 4.0 * (double)blocks * threads * calls_per_thread;
+    *attempts = 4.0 * (double)blocks * threads * calls;
     return rc;
 }
 
