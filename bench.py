@@ -148,7 +148,7 @@ def main():
     import numpy as np
     import torch
     import torch.distributed as dist
-    from paper_1508_06268_b200 import binding
+    from paper_1508_06268_b200 import binding, sharding
 
     if not torch.cuda.is_available():
         raise SystemExit("bench.py needs a CUDA device: the product has no CPU fallback")
@@ -162,7 +162,7 @@ def main():
         torch.cuda.synchronize()
 
     k = wl.exchange_every
-    seeds = [s + rank for s in wl.seeds]           # each rank: its own disorder realisation(s)
+    seeds = sharding.rank_seeds(wl.seeds, rank)    # each rank: its own disorder realisation(s)
     if wl.D == 1:
         g = binding.RfimPT(wl.L, wl.R, wl.J, wl.h, wl.field_kind, seed=seeds[0])
     else:
@@ -204,11 +204,8 @@ def main():
     clocks = sampler.stop()
     total_ms = float(sum(ms))
     total_ms_sweep = float(sum(ms_sweep))
-    if world > 1:
-        tt = torch.tensor([total_ms, total_ms_sweep], device="cuda", dtype=torch.float64)
-        dist.all_reduce(tt, op=dist.ReduceOp.MAX)
-        total_ms, total_ms_sweep = float(tt[0]), float(tt[1])
-    value = attempts_per_step * args.steps * world / (total_ms * 1e6)
+    total_ms, total_ms_sweep = sharding.max_over_ranks([total_ms, total_ms_sweep], device="cuda")
+    value = sharding.whole_job_rate(attempts_per_step * args.steps, world, total_ms)
     sweep_rate = attempts_per_step * args.steps / (total_ms_sweep * 1e6)      # per GPU
 
     # the two candidate bounds, measured in this run on this GPU (north_star)
@@ -261,10 +258,7 @@ def main():
             E, M, _ = g.observables()
         barrier()
         dt = time.perf_counter() - t0
-        if world > 1:
-            tt = torch.tensor([dt], device="cuda", dtype=torch.float64)
-            dist.all_reduce(tt, op=dist.ReduceOp.MAX)
-            dt = float(tt[0])
+        dt = sharding.max_over_ranks([dt], device="cuda")[0]
         obs_bytes = 2 * 8 * wl.D * wl.R
         line["e2e"] = {"value": attempts_per_step * n_e2e * world / (dt * 1e9), "unit": UNIT,
                        "h2d_bytes_per_step": int(host.nbytes), "d2h_bytes_per_step": int(host.nbytes + obs_bytes),
@@ -276,9 +270,12 @@ def main():
         cores = os.cpu_count() or 1
         threads = max(1, min(cores, 16))
         r_s = min(wl.R, 4 * threads)
-        v, ms_b, r_used = oracle_sample(wl, threads, r_s, k, 1, 0, wl.seeds[0])
+        v0, ms0, r_used = oracle_sample(wl, threads, r_s, k, 1, 0, wl.seeds[0])      # one step, to size the sample
+        n_b = int(max(2, min(200, 12e3 / max(ms0, 1.0))))                            # about 12 s of oracle work
+        v, ms_b, r_used = oracle_sample(wl, threads, r_s, k, n_b, 0, wl.seeds[0])
         line["cpu_baseline"] = {"value": v, "unit": UNIT, "cores": threads, "kind": "oracle",
-                                "sample": f"{r_used} of {wl.R} replicas x {k} sweeps + 1 exchange step, L={wl.L} ({ms_b / 1e3:.1f} s wall)"}
+                                "sample": f"{r_used} of {wl.R} replicas x {n_b} steps of ({k} sweeps + 1 exchange step), L={wl.L} "
+                                          f"({ms_b * n_b / 1e3:.1f} s wall, oracle as it stands, {threads} OpenMP threads over replicas)"}
     if rank == 0:
         print(json.dumps(line), flush=True)
     g.close()
