@@ -206,10 +206,12 @@ __device__ __noinline__ void res_wait_slow(const int* s_done, int eb, int b_zp, 
 // one 16-site piece of a row: own word, same-row words of the other colour, and ns = SP * (number of up neighbours)
 struct ResPiece { uint32_t me[4], cw[4], ns[4]; };
 
+// rem: where the rows of a z-neighbour plane that lives in another CTA are found in global memory (boundary tasks only)
+struct ResRemote { const uint8_t* spins; uint32_t off_p, off_m; bool any, p, m; };
+
 template <int K>
 __device__ __forceinline__ ResPiece res_load_piece(const uint8_t* smem, uint32_t a_x, uint32_t a_yp, uint32_t a_ym, uint32_t a_zp,
-                                                   uint32_t a_zm, uint32_t a_me, int k, int dir, bool remote_p, bool remote_m,
-                                                   const uint8_t* g_zp, const uint8_t* g_zm) {
+                                                   uint32_t a_zm, uint32_t a_me, int k, int dir, const ResRemote& rem) {
     constexpr int ARR = ResGeom<K>::ARR;
     const uint4 x = *reinterpret_cast<const uint4*>(smem + a_x + k * ARR);
     const uint4 yp = *reinterpret_cast<const uint4*>(smem + a_yp + k * ARR);
@@ -217,13 +219,15 @@ __device__ __forceinline__ ResPiece res_load_piece(const uint8_t* smem, uint32_t
     uint4 zp = *reinterpret_cast<const uint4*>(smem + a_zp + k * ARR);
     uint4 zm = *reinterpret_cast<const uint4*>(smem + a_zm + k * ARR);
     const uint4 m = *reinterpret_cast<const uint4*>(smem + a_me + k * ARR);
-    if (remote_p) {
-        zp = ld_cg16(g_zp + 16 * k);
-        zp.x *= kResSP; zp.y *= kResSP; zp.z *= kResSP; zp.w *= kResSP;
-    }
-    if (remote_m) {
-        zm = ld_cg16(g_zm + 16 * k);
-        zm.x *= kResSP; zm.y *= kResSP; zm.z *= kResSP; zm.w *= kResSP;
+    if (rem.any) {                                  // warp-uniform: only boundary tasks come here
+        if (rem.p) {
+            zp = ld_cg16(rem.spins + (size_t)(rem.off_p + 16u * k));
+            zp.x *= kResSP; zp.y *= kResSP; zp.z *= kResSP; zp.w *= kResSP;
+        }
+        if (rem.m) {
+            zm = ld_cg16(rem.spins + (size_t)(rem.off_m + 16u * k));
+            zm.x *= kResSP; zm.y *= kResSP; zm.z *= kResSP; zm.w *= kResSP;
+        }
     }
     // the word holding the far x-neighbour of the piece's edge byte (periodic in x)
     uint32_t edge;
@@ -429,21 +433,38 @@ __global__ void __launch_bounds__(THREADS, 1) k_sweep_res(const View v, const Re
             __threadfence_block();
         }
 
+        // per-task constants; everything class-dependent below is an offset from these
+        const uint32_t e16 = (uint32_t)e * 16u, p16 = (uint32_t)(e - i) * 16u;      // my row / first row of my plane
+        const uint32_t zp16 = (uint32_t)e_zp * 16u, zm16 = (uint32_t)e_zm * 16u;
+        const uint32_t base_c = (uint32_t)(c * 2 * K) * ARR, base_oc = (uint32_t)(oc * 2 * K) * ARR;
+        const uint32_t slot = (uint32_t)rr->slot;
+        const uint32_t tab_addr = tab0 + (uint32_t)pi.rep * kResTabBytes;
+        const float band = rr->band;
+        const uint32_t q00 = (uint32_t)W * (uint32_t)(2 * i + L * z);
+        const uint32_t row00 = (uint32_t)(z * L + 2 * i) * ROWB;
+        const uint32_t fblk0 = ((d2 + (uint32_t)c) * L + (uint32_t)z) * 2u;                // field block of (colour, plane, class 0)
+        const float4* fp0 = reinterpret_cast<const float4*>(rp.fielda_res) + (size_t)(fblk0 * (W * LH) + (uint32_t)i);
+        const uint4* fq0 = reinterpret_cast<const uint4*>(rp.fieldb_res) + (size_t)(fblk0 * (K * LH) + (uint32_t)i);
+        ResRemote rem;
+        rem.spins = v.spins; rem.any = btask; rem.p = remote_p; rem.m = remote_m;
+
         long long m_eb = 0, m_ef = 0, m_ms = 0;
 #pragma unroll 1
         for (int s = 0; s < 2; ++s) {
-            const int ys = (s + z) & 1, y = 2 * i + ys;
+            const int ys = (s + z) & 1;
             const int dir = (s + c) & 1;              // 0: second x-neighbour at xh-1, 1: at xh+1 (warp-uniform)
             // row addresses: shared arrays [colour][class][piece][row]
-            const int e0 = e - i;                     // first row of my plane
-            const int i_yp = ys ? ((i + 1) & (LH - 1)) : i, i_ym = ys ? i : ((i - 1) & (LH - 1));
-            const uint32_t a_x = A(oc, s, 0, e), a_me = A(c, s, 0, e);
-            const uint32_t o_t = A(oc, 1 - s, 0, 0);
-            const uint32_t a_yp = o_t + (uint32_t)(e0 + i_yp) * 16u, a_ym = o_t + (uint32_t)(e0 + i_ym) * 16u;
-            const uint32_t a_zp = o_t + (uint32_t)e_zp * 16u, a_zm = o_t + (uint32_t)e_zm * 16u;
-            const uint32_t rowoff = (uint32_t)(z * L + y) * ROWB;               // byte offset of the row inside a colour array
-            const uint8_t* g_zp = v.spins + (size_t)((ds2 + oc) * nh32 + (uint32_t)(zq_p * L + y) * ROWB);
-            const uint8_t* g_zm = v.spins + (size_t)((ds2 + oc) * nh32 + (uint32_t)(zq_m * L + y) * ROWB);
+            const uint32_t sK = s ? (uint32_t)(K * ARR) : 0u, tK = (uint32_t)(K * ARR) - sK;
+            const uint32_t i_yp = ys ? (uint32_t)((i + 1) & (LH - 1)) : (uint32_t)i, i_ym = ys ? (uint32_t)i : (uint32_t)((i - 1) & (LH - 1));
+            const uint32_t a_x = base_oc + sK + e16, a_me = base_c + sK + e16;
+            const uint32_t o_t = base_oc + tK;
+            const uint32_t a_yp = o_t + p16 + i_yp * 16u, a_ym = o_t + p16 + i_ym * 16u;
+            const uint32_t a_zp = o_t + zp16, a_zm = o_t + zm16;
+            const uint32_t rowoff = row00 + (ys ? ROWB : 0);                    // byte offset of the row inside a colour array
+            if (btask) {
+                rem.off_p = (ds2 + oc) * nh32 + (uint32_t)(zq_p * L + 2 * i + ys) * ROWB;
+                rem.off_m = (ds2 + oc) * nh32 + (uint32_t)(zq_m * L + 2 * i + ys) * ROWB;
+            }
 
             // per-row constants
             uint32_t rk[20];
@@ -457,13 +478,9 @@ __global__ void __launch_bounds__(THREADS, 1) k_sweep_res(const View v, const Re
                     rk[4 * j] = q4.x; rk[4 * j + 1] = q4.y; rk[4 * j + 2] = q4.z; rk[4 * j + 3] = q4.w;
                 }
             }
-            const uint32_t slot = (uint32_t)rr->slot;
-            const uint32_t tab_addr = tab0 + (uint32_t)pi.rep * kResTabBytes;
-            const float band = rr->band;
-            const uint32_t q0 = (uint32_t)W * (uint32_t)(y + L * z);
-            const uint32_t blk = ((d2 + (uint32_t)c) * L + (uint32_t)z) * 2u + (uint32_t)s;   // field block of this (colour, plane, class)
-            const float4* fp = reinterpret_cast<const float4*>(rp.fielda_res) + (size_t)(blk * (W * LH) + (uint32_t)i);
-            const uint4* fq = reinterpret_cast<const uint4*>(rp.fieldb_res) + (size_t)(blk * (K * LH) + (uint32_t)i);
+            const uint32_t q0 = q00 + (ys ? W : 0);
+            const float4* fp = fp0 + (s ? W * LH : 0);
+            const uint4* fq = fq0 + (s ? K * LH : 0);
 
 #pragma unroll
             for (int k = 0; k < K; ++k) {             // one 16-site piece of the row at a time
@@ -475,7 +492,7 @@ __global__ void __launch_bounds__(THREADS, 1) k_sweep_res(const View v, const Re
 #pragma unroll
                     for (int w = 0; w < 4; ++w) fa[w] = __ldg(fp + (4 * k + w) * LH);
                 }
-                ResPiece pc = res_load_piece<K>(smem, a_x, a_yp, a_ym, a_zp, a_zm, a_me, k, dir, remote_p, remote_m, g_zp, g_zm);
+                ResPiece pc = res_load_piece<K>(smem, a_x, a_yp, a_ym, a_zp, a_zm, a_me, k, dir, rem);
                 const uint32_t fw[4] = {fb.x, fb.y, fb.z, fb.w};
                 uint32_t idx8[4];
 #pragma unroll
