@@ -10,7 +10,7 @@ import os
 import numpy as np
 
 _HERE = os.path.dirname(os.path.abspath(__file__))
-_LIB_PATH = os.path.join(_HERE, "librfimpt.so")
+_LIB_PATH = os.environ.get("RFIM_PT_LIB") or os.path.join(_HERE, "librfimpt.so")   # RFIM_PT_LIB: another build of the same library (A/B timing)
 _lib = None
 _alloc_refs = {}
 

@@ -289,6 +289,135 @@ __device__ __noinline__ int3 res_measure_piece(uint4 mev, uint4 idx8v, uint4 fbv
     return r;
 }
 
+// Per-task lane constants of the row update: shared-memory byte offsets of class 0 (class 1 = + K * ARR, an
+// immediate), everything else the two rows of a task share.
+struct ResLane {
+    uint32_t me, x;              // my row in my colour / in the other colour, class 0
+    uint32_t ya, yb, yc;         // rows i+1, i, i-1 of my plane in the other colour, class 0 (periodic in y)
+    uint32_t zp, zm;             // row i of the z-neighbour planes in the other colour, class 0
+    uint32_t q00;                // Philox counter word of (y = 2i, xh = 0)
+    uint32_t slot, tab_addr;
+    float band;
+    uint32_t zpar;               // z & 1
+    const float4* fp0;           // Gaussian field of (colour, plane, class 0), row i
+    const uint4* fq0;            // bimodal field, same place
+    uint32_t grow0;              // BND / rare path: byte offset of row y = 2i of colour c inside the slot's lattice
+    uint32_t ds2, d2;
+};
+
+// One row (L/2 same-colour sites) of one checkerboard class S: K pieces of 16 sites.  DIR (warp-uniform): the
+// second x-neighbour sits at xh-1 (0) or xh+1 (1).  BND: a z-neighbour plane lives in another CTA (rows read from and
+// published to global memory); MEAS: also measure; RAGGED: lanes past the last row redo it and do not store.
+template <int KIND, int K, bool NEVER, bool UNI, bool BND, bool MEAS, bool RAGGED>
+__device__ __forceinline__ void res_row(const View& v, const ResParams& rp, uint8_t* smem, const ResLane& ln, const int s, const int c, const int DIR,
+                                        const uint32_t sweep, const uint32_t dom, const ResRep* rr, const bool valid,
+                                        const bool remote_p, const bool remote_m, const uint32_t roff_p, const uint32_t roff_m,
+                                        long long& m_eb, long long& m_ef, long long& m_ms) {
+    using G = ResGeom<K>;
+    constexpr int L = G::L, LH = G::LH, ROWB = G::ROWB, W = G::W, ARR = G::ARR;
+    const uint32_t ys = (uint32_t)s ^ ln.zpar;
+    const uint32_t sK = s ? (uint32_t)(K * ARR) : 0u, tK = (uint32_t)(K * ARR) - sK;
+    const uint32_t a_me = ln.me + sK, a_x = ln.x + sK;
+    const uint32_t a_yp = (ys ? ln.ya : ln.yb) + tK, a_ym = (ys ? ln.yb : ln.yc) + tK;
+    const uint32_t a_zp = ln.zp + tK, a_zm = ln.zm + tK;
+    const uint32_t q0 = ln.q00 + (ys ? W : 0);
+    const float4* fp = ln.fp0 + (s ? W * LH : 0);
+    const uint4* fq = ln.fq0 + (s ? K * LH : 0);
+    const uint32_t grow = ln.grow0 + (ys ? ROWB : 0);          // only BND and the rare exact path use it
+    ResRemote rem;
+    rem.spins = v.spins; rem.any = BND; rem.p = BND && remote_p; rem.m = BND && remote_m;
+    rem.off_p = roff_p + (ys ? ROWB : 0); rem.off_m = roff_m + (ys ? ROWB : 0);
+
+    uint32_t rk[20];
+    if (UNI) {
+#pragma unroll
+        for (int j = 0; j < 20; ++j) rk[j] = rp.rk0[j];
+    } else {
+#pragma unroll
+        for (int j = 0; j < 5; ++j) {
+            const uint4 q4 = reinterpret_cast<const uint4*>(rr->rk)[j];
+            rk[4 * j] = q4.x; rk[4 * j + 1] = q4.y; rk[4 * j + 2] = q4.z; rk[4 * j + 3] = q4.w;
+        }
+    }
+
+#pragma unroll
+    for (int k = 0; k < K; ++k) {             // one 16-site piece of the row at a time
+        // field of the piece: issued first, consumed last
+        float4 fa[4];
+        uint4 fb = make_uint4(0u, 0u, 0u, 0u);
+        if (KIND == 0) fb = __ldg(fq + k * LH);
+        else {
+#pragma unroll
+            for (int w = 0; w < 4; ++w) fa[w] = __ldg(fp + (4 * k + w) * LH);
+        }
+        ResPiece pc = res_load_piece<K>(smem, a_x, a_yp, a_ym, a_zp, a_zm, a_me, k, DIR, rem);
+        const uint32_t fw[4] = {fb.x, fb.y, fb.z, fb.w};
+        uint32_t idx8[4];
+#pragma unroll
+        for (int w = 0; w < 4; ++w) idx8[w] = pc.ns[w] + (pc.me[w] << 3) + (KIND == 0 ? fw[w] : 0u);
+
+        // ---- the four words of the piece ---------------------------------------------------------------
+        float mn = 3.0e38f;                   // smallest |d| of the piece (Gaussian)
+#pragma unroll
+        for (int w = 0; w < 4; ++w) {
+            const Words4 r = philox_rkreg(rk, q0 + (uint32_t)(4 * k + w), sweep, ln.slot, dom);
+            const uint32_t u[4] = {r.w0, r.w1, r.w2, r.w3};
+            if (KIND == 0) {
+                uint32_t flips = 0;
+#pragma unroll
+                for (int j = 0; j < 4; ++j) {
+                    const uint2 ent = lds64(__byte_perm(idx8[w], ln.tab_addr, 0x7650 + j));
+                    bool acc = u[j] <= ent.x;
+                    if (NEVER) acc = acc && ent.y == 0u;
+                    if (acc) flips |= kResSP << (8 * j);
+                }
+                pc.me[w] ^= flips;
+            } else {
+                const float a[4] = {fa[w].x, fa[w].y, fa[w].z, fa[w].w};
+                float d[4];
+#pragma unroll
+                for (int j = 0; j < 4; ++j) d[j] = res_gauss_diff(idx8[w], j, ln.tab_addr, a[j], u[j]);
+                mn = fminf(fminf(mn, fminf(fabsf(d[0]), fabsf(d[1]))), fminf(fabsf(d[2]), fabsf(d[3])));
+                // sign bytes of the four differences -> 0xFF where d < 0 (accept)
+                const uint32_t m01 = prmt(__float_as_uint(d[0]), __float_as_uint(d[1]), 0x00FBu);
+                const uint32_t m23 = prmt(__float_as_uint(d[2]), __float_as_uint(d[3]), 0xFB00u);
+                pc.me[w] ^= prmt(m01, m23, 0x7610u) & (kResSP * 0x01010101u);
+            }
+        }
+        uint4 nw = make_uint4(pc.me[0], pc.me[1], pc.me[2], pc.me[3]);
+        if (KIND == 1 && mn < ln.band)          // rare: some site needs the exact binary64 rule
+            nw = res_gauss_piece_fix(v, make_uint4(idx8[0], idx8[1], idx8[2], idx8[3]), ln.tab_addr, ln.band, fp + 4 * k * LH, LH,
+                                     v.fieldg + (size_t)((ln.d2 + (uint32_t)c) * (uint32_t)v.Nh + grow + 16u * k), rr, q0 + 4u * k, sweep, dom);
+
+        // ---- write back ---------------------------------------------------------------------------------
+        if (!RAGGED || valid) {
+            *reinterpret_cast<uint4*>(smem + a_me + k * ARR) = nw;
+            if (BND && (remote_p || remote_m))
+                *reinterpret_cast<uint4*>(v.spins + (size_t)((ln.ds2 + (uint32_t)c) * (uint32_t)v.Nh + grow + 16u * k)) =
+                    make_uint4(nw.x >> 3, nw.y >> 3, nw.z >> 3, nw.w >> 3);
+            if (MEAS) {
+                const float4 z4 = make_float4(0.f, 0.f, 0.f, 0.f);
+                const int3 m3 = res_measure_piece<KIND>(nw, make_uint4(idx8[0], idx8[1], idx8[2], idx8[3]), fb,
+                                                        KIND ? fa[0] : z4, KIND ? fa[1] : z4, KIND ? fa[2] : z4, KIND ? fa[3] : z4, c);
+                m_eb += m3.x; m_ef += m3.y; m_ms += m3.z;
+            }
+        }
+    }
+}
+
+// both rows (classes) of a task, one after the other through the same code (the loop body must stay inside the
+// instruction cache: two unrolled copies of it were measured 15 % slower)
+template <int KIND, int K, bool NEVER, bool UNI, bool BND, bool MEAS, bool RAGGED>
+__device__ __forceinline__ void res_task_rows(const View& v, const ResParams& rp, uint8_t* smem, const ResLane& ln, const int c,
+                                              const uint32_t sweep, const uint32_t dom, const ResRep* rr, const bool valid,
+                                              const bool remote_p, const bool remote_m, const uint32_t roff_p, const uint32_t roff_m,
+                                              long long& m_eb, long long& m_ef, long long& m_ms) {
+#pragma unroll 1
+    for (int s = 0; s < 2; ++s)
+        res_row<KIND, K, NEVER, UNI, BND, MEAS, RAGGED>(v, rp, smem, ln, s, c, (s + c) & 1, sweep, dom, rr, valid, remote_p, remote_m, roff_p, roff_m,
+                                                        m_eb, m_ef, m_ms);
+}
+
 // K = 16-byte pieces per row per colour (L = 32 K); UNI: one member, round keys come from the constant bank
 template <int KIND, int K, bool NEVER, bool UNI, int THREADS>
 __global__ void __launch_bounds__(THREADS, 1) k_sweep_res(const View v, const ResParams rp) {
@@ -396,6 +525,7 @@ __global__ void __launch_bounds__(THREADS, 1) k_sweep_res(const View v, const Re
     const uint32_t nh32 = (uint32_t)v.Nh;
 
     // ---- the task flow ------------------------------------------------------------------------------
+    constexpr bool RAGGED = (LH % 32) != 0;
     int p_cur = 0, base_cur = 0;                      // phase of this warp's current task number (numbers only grow)
     for (;;) {
         int g = 0;
@@ -411,16 +541,14 @@ __global__ void __launch_bounds__(THREADS, 1) k_sweep_res(const View v, const Re
         const int eb = s_order[bidx];
         const bool btask = bidx < n_bblocks;
         const int e_raw = eb * 32 + lane;
-        const bool valid = e_raw < E;
+        const bool valid = !RAGGED || e_raw < E;
         const int e = valid ? e_raw : E - 1;
         const int pl = e / LH, i = e % LH;
         const ResPlane pi = s_plane[pl];
         const ResRep* rr = s_rep + pi.rep;
         const int z = pi.z;
-        const uint32_t ds2 = (uint32_t)rr->ds * 2u, d2 = (uint32_t)rr->d * 2u;
         const bool remote_p = pi.zp_pl < 0, remote_m = pi.zm_pl < 0;
         const int e_zp = remote_p ? 0 : pi.zp_pl * LH + i, e_zm = remote_m ? 0 : pi.zm_pl * LH + i;
-        const int zq_p = (z + 1) & (L - 1), zq_m = (z - 1) & (L - 1);
 
         // dependencies: the blocks of my plane and of its z-neighbours have finished phase p-1;
         // remote neighbour planes: their owners have published phase p-1
@@ -433,118 +561,40 @@ __global__ void __launch_bounds__(THREADS, 1) k_sweep_res(const View v, const Re
             __threadfence_block();
         }
 
-        // per-task constants; everything class-dependent below is an offset from these
-        const uint32_t e16 = (uint32_t)e * 16u, p16 = (uint32_t)(e - i) * 16u;      // my row / first row of my plane
-        const uint32_t zp16 = (uint32_t)e_zp * 16u, zm16 = (uint32_t)e_zm * 16u;
-        const uint32_t base_c = (uint32_t)(c * 2 * K) * ARR, base_oc = (uint32_t)(oc * 2 * K) * ARR;
-        const uint32_t slot = (uint32_t)rr->slot;
-        const uint32_t tab_addr = tab0 + (uint32_t)pi.rep * kResTabBytes;
-        const float band = rr->band;
-        const uint32_t q00 = (uint32_t)W * (uint32_t)(2 * i + L * z);
-        const uint32_t row00 = (uint32_t)(z * L + 2 * i) * ROWB;
-        const uint32_t fblk0 = ((d2 + (uint32_t)c) * L + (uint32_t)z) * 2u;                // field block of (colour, plane, class 0)
-        const float4* fp0 = reinterpret_cast<const float4*>(rp.fielda_res) + (size_t)(fblk0 * (W * LH) + (uint32_t)i);
-        const uint4* fq0 = reinterpret_cast<const uint4*>(rp.fieldb_res) + (size_t)(fblk0 * (K * LH) + (uint32_t)i);
-        ResRemote rem;
-        rem.spins = v.spins; rem.any = btask; rem.p = remote_p; rem.m = remote_m;
+        // per-task lane constants; everything class-dependent is an immediate offset from these
+        ResLane ln;
+        {
+            const uint32_t e16 = (uint32_t)e * 16u, p16 = (uint32_t)(e - i) * 16u;      // my row / first row of my plane
+            const uint32_t base_c = (uint32_t)(c * 2 * K) * ARR, base_oc = (uint32_t)(oc * 2 * K) * ARR;
+            ln.me = base_c + e16; ln.x = base_oc + e16;
+            ln.ya = base_oc + p16 + (uint32_t)((i + 1) & (LH - 1)) * 16u;
+            ln.yb = ln.x;
+            ln.yc = base_oc + p16 + (uint32_t)((i - 1) & (LH - 1)) * 16u;
+            ln.zp = base_oc + (uint32_t)e_zp * 16u; ln.zm = base_oc + (uint32_t)e_zm * 16u;
+            ln.q00 = (uint32_t)W * (uint32_t)(2 * i + L * z);
+            ln.slot = (uint32_t)rr->slot;
+            ln.tab_addr = tab0 + (uint32_t)pi.rep * kResTabBytes;
+            ln.band = rr->band;
+            ln.zpar = (uint32_t)z & 1u;
+            ln.ds2 = (uint32_t)rr->ds * 2u; ln.d2 = (uint32_t)rr->d * 2u;
+            const uint32_t fblk0 = ((ln.d2 + (uint32_t)c) * L + (uint32_t)z) * 2u;        // field block of (colour, plane, class 0)
+            ln.fp0 = reinterpret_cast<const float4*>(rp.fielda_res) + (size_t)(fblk0 * (W * LH) + (uint32_t)i);
+            ln.fq0 = reinterpret_cast<const uint4*>(rp.fieldb_res) + (size_t)(fblk0 * (K * LH) + (uint32_t)i);
+            ln.grow0 = (uint32_t)(z * L + 2 * i) * ROWB;
+        }
 
         long long m_eb = 0, m_ef = 0, m_ms = 0;
-#pragma unroll 1
-        for (int s = 0; s < 2; ++s) {
-            const int ys = (s + z) & 1;
-            const int dir = (s + c) & 1;              // 0: second x-neighbour at xh-1, 1: at xh+1 (warp-uniform)
-            // row addresses: shared arrays [colour][class][piece][row]
-            const uint32_t sK = s ? (uint32_t)(K * ARR) : 0u, tK = (uint32_t)(K * ARR) - sK;
-            const uint32_t i_yp = ys ? (uint32_t)((i + 1) & (LH - 1)) : (uint32_t)i, i_ym = ys ? (uint32_t)i : (uint32_t)((i - 1) & (LH - 1));
-            const uint32_t a_x = base_oc + sK + e16, a_me = base_c + sK + e16;
-            const uint32_t o_t = base_oc + tK;
-            const uint32_t a_yp = o_t + p16 + i_yp * 16u, a_ym = o_t + p16 + i_ym * 16u;
-            const uint32_t a_zp = o_t + zp16, a_zm = o_t + zm16;
-            const uint32_t rowoff = row00 + (ys ? ROWB : 0);                    // byte offset of the row inside a colour array
-            if (btask) {
-                rem.off_p = (ds2 + oc) * nh32 + (uint32_t)(zq_p * L + 2 * i + ys) * ROWB;
-                rem.off_m = (ds2 + oc) * nh32 + (uint32_t)(zq_m * L + 2 * i + ys) * ROWB;
-            }
-
-            // per-row constants
-            uint32_t rk[20];
-            if (UNI) {
-#pragma unroll
-                for (int j = 0; j < 20; ++j) rk[j] = rp.rk0[j];
-            } else {
-#pragma unroll
-                for (int j = 0; j < 5; ++j) {
-                    const uint4 q4 = reinterpret_cast<const uint4*>(rr->rk)[j];
-                    rk[4 * j] = q4.x; rk[4 * j + 1] = q4.y; rk[4 * j + 2] = q4.z; rk[4 * j + 3] = q4.w;
-                }
-            }
-            const uint32_t q0 = q00 + (ys ? W : 0);
-            const float4* fp = fp0 + (s ? W * LH : 0);
-            const uint4* fq = fq0 + (s ? K * LH : 0);
-
-#pragma unroll
-            for (int k = 0; k < K; ++k) {             // one 16-site piece of the row at a time
-                // field of the piece: issued first, consumed last
-                float4 fa[4];
-                uint4 fb = make_uint4(0u, 0u, 0u, 0u);
-                if (KIND == 0) fb = __ldg(fq + k * LH);
-                else {
-#pragma unroll
-                    for (int w = 0; w < 4; ++w) fa[w] = __ldg(fp + (4 * k + w) * LH);
-                }
-                ResPiece pc = res_load_piece<K>(smem, a_x, a_yp, a_ym, a_zp, a_zm, a_me, k, dir, rem);
-                const uint32_t fw[4] = {fb.x, fb.y, fb.z, fb.w};
-                uint32_t idx8[4];
-#pragma unroll
-                for (int w = 0; w < 4; ++w) idx8[w] = pc.ns[w] + (pc.me[w] << 3) + (KIND == 0 ? fw[w] : 0u);
-
-                // ---- the four words of the piece ---------------------------------------------------------------
-                float mn = 3.0e38f;                   // smallest |d| of the piece (Gaussian)
-#pragma unroll
-                for (int w = 0; w < 4; ++w) {
-                    const Words4 r = philox_rkreg(rk, q0 + (uint32_t)(4 * k + w), sweep, slot, dom);
-                    const uint32_t u[4] = {r.w0, r.w1, r.w2, r.w3};
-                    if (KIND == 0) {
-                        uint32_t flips = 0;
-#pragma unroll
-                        for (int j = 0; j < 4; ++j) {
-                            const uint2 ent = lds64(__byte_perm(idx8[w], tab_addr, 0x7650 + j));
-                            bool acc = u[j] <= ent.x;
-                            if (NEVER) acc = acc && ent.y == 0u;
-                            if (acc) flips |= kResSP << (8 * j);
-                        }
-                        pc.me[w] ^= flips;
-                    } else {
-                        const float a[4] = {fa[w].x, fa[w].y, fa[w].z, fa[w].w};
-                        float d[4];
-#pragma unroll
-                        for (int j = 0; j < 4; ++j) d[j] = res_gauss_diff(idx8[w], j, tab_addr, a[j], u[j]);
-                        mn = fminf(fminf(mn, fminf(fabsf(d[0]), fabsf(d[1]))), fminf(fabsf(d[2]), fabsf(d[3])));
-                        // sign bytes of the four differences -> 0xFF where d < 0 (accept)
-                        const uint32_t m01 = prmt(__float_as_uint(d[0]), __float_as_uint(d[1]), 0x00FBu);
-                        const uint32_t m23 = prmt(__float_as_uint(d[2]), __float_as_uint(d[3]), 0xFB00u);
-                        pc.me[w] ^= prmt(m01, m23, 0x7610u) & (kResSP * 0x01010101u);
-                    }
-                }
-                uint4 nw = make_uint4(pc.me[0], pc.me[1], pc.me[2], pc.me[3]);
-                if (KIND == 1 && mn < band)             // rare: some site needs the exact binary64 rule
-                    nw = res_gauss_piece_fix(v, make_uint4(idx8[0], idx8[1], idx8[2], idx8[3]), tab_addr, band, fp + 4 * k * LH, LH,
-                                             v.fieldg + (size_t)((d2 + (uint32_t)c) * nh32 + rowoff + 16u * k), rr, q0 + 4u * k, sweep, dom);
-
-                // ---- write back ---------------------------------------------------------------------------------
-                if (valid) {
-                    *reinterpret_cast<uint4*>(smem + a_me + k * ARR) = nw;
-                    if (remote_p || remote_m)
-                        *reinterpret_cast<uint4*>(v.spins + (size_t)((ds2 + (uint32_t)c) * nh32 + rowoff + 16u * k)) =
-                            make_uint4(nw.x >> 3, nw.y >> 3, nw.z >> 3, nw.w >> 3);
-                    if (meas) {
-                        const float4 z4 = make_float4(0.f, 0.f, 0.f, 0.f);
-                        const int3 m3 = res_measure_piece<KIND>(nw, make_uint4(idx8[0], idx8[1], idx8[2], idx8[3]), fb,
-                                                                KIND ? fa[0] : z4, KIND ? fa[1] : z4, KIND ? fa[2] : z4, KIND ? fa[3] : z4, c);
-                        m_eb += m3.x; m_ef += m3.y; m_ms += m3.z;
-                    }
-                }
-            }
+        if (!btask && !meas) {
+            res_task_rows<KIND, K, NEVER, UNI, false, false, RAGGED>(v, rp, smem, ln, c, sweep, dom, rr, valid, false, false, 0u, 0u, m_eb, m_ef, m_ms);
+        } else {
+            // rows of a z-neighbour plane that lives in another CTA: read from global memory (class 0; class 1 = + ROWB)
+            const int zq_p = (z + 1) & (L - 1), zq_m = (z - 1) & (L - 1);
+            const uint32_t roff_p = (ln.ds2 + (uint32_t)oc) * nh32 + (uint32_t)(zq_p * L + 2 * i) * ROWB;
+            const uint32_t roff_m = (ln.ds2 + (uint32_t)oc) * nh32 + (uint32_t)(zq_m * L + 2 * i) * ROWB;
+            if (btask && !meas)
+                res_task_rows<KIND, K, NEVER, UNI, true, false, RAGGED>(v, rp, smem, ln, c, sweep, dom, rr, valid, remote_p, remote_m, roff_p, roff_m, m_eb, m_ef, m_ms);
+            else
+                res_task_rows<KIND, K, NEVER, UNI, true, true, RAGGED>(v, rp, smem, ln, c, sweep, dom, rr, valid, remote_p && btask, remote_m && btask, roff_p, roff_m, m_eb, m_ef, m_ms);
         }
 
         if (meas) {
