@@ -51,12 +51,6 @@ namespace rfim {
 #ifndef RFIM_RES_THREADS
 #define RFIM_RES_THREADS 512
 #endif
-#ifndef RFIM_RES_SWP
-#define RFIM_RES_SWP 0
-#endif
-#ifndef RFIM_RES_FD
-#define RFIM_RES_FD 0
-#endif
 constexpr int kResThreads = RFIM_RES_THREADS;
 constexpr uint32_t kResSP = 8;                  // shared-memory spin coding: 0 / SP
 constexpr int kResTabBytes = 256;               // per-replica acceptance table slot (256-byte aligned)
@@ -319,7 +313,7 @@ __device__ __forceinline__ void res_row(const View& v, const ResParams& rp, uint
                                         const bool remote_p, const bool remote_m, const uint32_t roff_p, const uint32_t roff_m,
                                         long long& m_eb, long long& m_ef, long long& m_ms) {
     using G = ResGeom<K>;
-    constexpr int L = G::L, LH = G::LH, ROWB = G::ROWB, W = G::W, ARR = G::ARR;
+    constexpr int LH = G::LH, ROWB = G::ROWB, W = G::W, ARR = G::ARR;
     const uint32_t ys = (uint32_t)s ^ ln.zpar;
     const uint32_t sK = s ? (uint32_t)(K * ARR) : 0u, tK = (uint32_t)(K * ARR) - sK;
     const uint32_t a_me = ln.me + sK, a_x = ln.x + sK;
@@ -348,19 +342,8 @@ __device__ __forceinline__ void res_row(const View& v, const ResParams& rp, uint
     uint4 xr[K];
 #pragma unroll
     for (int k = 0; k < K; ++k) xr[k] = *reinterpret_cast<const uint4*>(smem + a_x + k * ARR);
-#if RFIM_RES_SWP
-    Words4 R[4], Rn[4];
-#pragma unroll
-    for (int w = 0; w < 4; ++w) R[w] = philox_rkreg(rk, q0 + (uint32_t)w, sweep, ln.slot, dom);
-#endif
 #pragma unroll
     for (int k = 0; k < K; ++k) {             // one 16-site piece of the row at a time
-#if RFIM_RES_SWP
-        if (k + 1 < K) {
-#pragma unroll
-            for (int w = 0; w < 4; ++w) Rn[w] = philox_rkreg(rk, q0 + (uint32_t)(4 * (k + 1) + w), sweep, ln.slot, dom);
-        }
-#endif
         // field of the piece: issued first, consumed last
         float4 fa[4];
         uint4 fb = make_uint4(0u, 0u, 0u, 0u);
@@ -377,27 +360,9 @@ __device__ __forceinline__ void res_row(const View& v, const ResParams& rp, uint
 
         // ---- the four words of the piece ---------------------------------------------------------------
         float mn = 3.0e38f;                   // smallest |d| of the piece (Gaussian)
-#if RFIM_RES_FD > 0
-        uint32_t fdep[4];
-#endif
 #pragma unroll
         for (int w = 0; w < 4; ++w) {
-#if RFIM_RES_SWP
-            const Words4 r = R[w];
-#else
-            uint32_t qw = q0 + (uint32_t)(4 * k + w);
-#if RFIM_RES_FD > 0
-            if (w >= RFIM_RES_FD) asm volatile("" : "+r"(qw) : "r"(fdep[w - RFIM_RES_FD]));   // at most RFIM_RES_FD calls in flight
-#endif
-#if RFIM_HACK_NOPHILOX          /* timing experiment only: results are wrong */
-            Words4 r; r.w0 = qw * 0x9E3779B9u ^ sweep; r.w1 = r.w0 * 0x85EBCA6Bu; r.w2 = r.w1 ^ (r.w0 >> 7); r.w3 = r.w2 * 0xC2B2AE35u;
-#else
-            const Words4 r = philox_rkreg(rk, qw, sweep, ln.slot, dom);
-#endif
-#if RFIM_RES_FD > 0
-            fdep[w] = r.w0;
-#endif
-#endif
+            const Words4 r = philox_rkreg(rk, q0 + (uint32_t)(4 * k + w), sweep, ln.slot, dom);
             const uint32_t u[4] = {r.w0, r.w1, r.w2, r.w3};
             if (KIND == 0) {
                 uint32_t flips = 0;
@@ -413,11 +378,7 @@ __device__ __forceinline__ void res_row(const View& v, const ResParams& rp, uint
                 const float a[4] = {fa[w].x, fa[w].y, fa[w].z, fa[w].w};
                 float d[4];
 #pragma unroll
-#if RFIM_HACK_NOFLOAT           /* timing experiment only: results are wrong */
-                for (int j = 0; j < 4; ++j) d[j] = __uint_as_float(u[j] ^ idx8[w]) + a[j];
-#else
                 for (int j = 0; j < 4; ++j) d[j] = res_gauss_diff(idx8[w], j, ln.tab_addr, a[j], u[j]);
-#endif
                 mn = fminf(fminf(mn, fminf(fabsf(d[0]), fabsf(d[1]))), fminf(fabsf(d[2]), fabsf(d[3])));
                 // sign bytes of the four differences -> 0xFF where d < 0 (accept)
                 const uint32_t m01 = prmt(__float_as_uint(d[0]), __float_as_uint(d[1]), 0x00FBu);
@@ -430,12 +391,6 @@ __device__ __forceinline__ void res_row(const View& v, const ResParams& rp, uint
             nw = res_gauss_piece_fix(v, make_uint4(idx8[0], idx8[1], idx8[2], idx8[3]), ln.tab_addr, ln.band, fp + 4 * k * LH, LH,
                                      v.fieldg + (size_t)((ln.d2 + (uint32_t)c) * (uint32_t)v.Nh + grow + 16u * k), rr, q0 + 4u * k, sweep, dom);
 
-#if RFIM_RES_SWP
-        if (k + 1 < K) {
-#pragma unroll
-            for (int w = 0; w < 4; ++w) R[w] = Rn[w];
-        }
-#endif
         // ---- write back ---------------------------------------------------------------------------------
         if (!RAGGED || valid) {
             *reinterpret_cast<uint4*>(smem + a_me + k * ARR) = nw;
