@@ -308,14 +308,16 @@ int ensure_stage(rfim_pt* h, size_t bytes) {
 bool flow_supported(const rfim_pt* h) { return h->L == 32 || h->L == 64; }
 
 // the resident kernel's partition of the D*n*L planes over the grid, and whether the largest run fits in shared memory
-struct ResPlan { int grid, total, q, rem, cap_planes, cap_reps; size_t smem; bool ok; };
-ResPlan res_plan(const rfim_pt* h) {
+struct ResPlan { int grid, total, q, rem, cap_planes, cap_reps, nd, groups; size_t smem; bool ok; };
+// plan for `nd` members per launch
+ResPlan res_plan_nd(const rfim_pt* h, int nd) {
     ResPlan p{};
     p.ok = false;
+    p.nd = nd; p.groups = (h->D + nd - 1) / nd;
     if (!flow_supported(h) || h->n < 1 || h->sm_count < 1) return p;
     p.grid = std::min(h->sm_count, kResMaxGrid);
     if (h->res_grid_limit > 0) p.grid = std::min(p.grid, h->res_grid_limit);
-    const long long total = (long long)h->D * h->n * h->L;
+    const long long total = (long long)nd * h->n * h->L;
     if (total > (long long)p.grid * 32767) return p;
     p.total = (int)total;
     p.q = p.total / p.grid; p.rem = p.total % p.grid;
@@ -325,6 +327,18 @@ ResPlan res_plan(const rfim_pt* h) {
     if (p.cap_reps > 255) return p;
     p.smem = res_smem_bytes(h->L, p.cap_reps);
     p.ok = p.smem <= (size_t)h->smem_optin;
+    return p;
+}
+// A batch whose planes do not all fit in the shared memory of the grid is swept in the fewest equal groups of members
+// that do (members are independent; config 5 = 2 launches of 16 members).
+ResPlan res_plan(const rfim_pt* h) {
+    ResPlan p{};
+    for (int groups = 1; groups <= h->D; ++groups) {
+        const int nd = (h->D + groups - 1) / groups;
+        if (groups > 1 && (h->D + nd - 1) / nd != groups) continue;
+        p = res_plan_nd(h, nd);
+        if (p.ok || groups >= 8) break;
+    }
     return p;
 }
 
@@ -406,39 +420,51 @@ int launch_res_t(rfim_pt* h, const ResPlan& pl, const ResParams& rp) {
 
 template <int KIND, int K, bool NEVER>
 int launch_res_u(rfim_pt* h, const ResPlan& pl, const ResParams& rp) {
-    return h->D == 1 ? launch_res_t<KIND, K, NEVER, true>(h, pl, rp) : launch_res_t<KIND, K, NEVER, false>(h, pl, rp);
+    return pl.nd == 1 ? launch_res_t<KIND, K, NEVER, true>(h, pl, rp) : launch_res_t<KIND, K, NEVER, false>(h, pl, rp);
 }
 
-// `sweeps` (<= 127) sweeps of every active replica of every member in one cooperative launch
+template <int KIND, int K, bool NEVER>
+int launch_res_k(rfim_pt* h, const ResPlan& pl, const ResParams& rp) { return launch_res_u<KIND, K, NEVER>(h, pl, rp); }
+
+// `sweeps` (<= 127) sweeps of every active replica of every member: one cooperative launch per group of members
 int launch_res(rfim_pt* h, int sweeps, bool measure, bool* exchanged) {
-    const ResPlan pl = res_plan(h);
-    if (!pl.ok) return fail(h, RFIM_EINVAL, "resident kernel: the planes of one CTA do not fit in shared memory");
-    ResParams rp{};
-    rp.phases = 2 * sweeps;
-    rp.measure = measure ? 1 : 0;
-    rp.exchange = (measure && h->D <= kResFusedExchangeMaxD) ? 1 : 0;
-    rp.nact = pl.q > 0 ? pl.grid : pl.rem;
-    rp.xstep = (uint32_t)h->xstep;
-    rp.xrow = h->series_steps;
-    rp.ticket = h->res_prog + kResMaxGrid;       // the word after the progress words (zeroed at create, left at zero)
-    *exchanged = rp.exchange != 0;
-    rp.sweep0 = (uint32_t)h->sweep_g;
-    rp.epoch = ++h->res_epoch;
-    rp.prog = h->res_prog;
-    rp.total_planes = pl.total; rp.q = pl.q; rp.rem = pl.rem;
-    rp.cap_reps = pl.cap_reps;
-    rp.fielda_res = h->fielda_res; rp.fieldb_res = h->fieldb_res;
-    rp.diag = h->v.diag;
-    {
-        uint32_t k0 = (uint32_t)(h->seeds[0] & 0xFFFFFFFFull), k1 = (uint32_t)(h->seeds[0] >> 32);
-        for (int r = 0; r < 10; ++r) { rp.rk0[2 * r] = k0; rp.rk0[2 * r + 1] = k1; k0 += kPhiloxW0; k1 += kPhiloxW1; }
+    const ResPlan pl0 = res_plan(h);
+    if (!pl0.ok) return fail(h, RFIM_EINVAL, "resident kernel: the planes of one CTA do not fit in shared memory");
+    *exchanged = measure && pl0.groups == 1 && h->D <= kResFusedExchangeMaxD;
+    for (int d0 = 0; d0 < h->D; d0 += pl0.nd) {
+        const int nd = std::min(pl0.nd, h->D - d0);
+        const ResPlan pl = nd == pl0.nd ? pl0 : res_plan_nd(h, nd);
+        if (!pl.ok) return fail(h, RFIM_EINVAL, "resident kernel: the last member group does not fit");
+        ResParams rp{};
+        rp.phases = 2 * sweeps;
+        rp.measure = measure ? 1 : 0;
+        rp.exchange = *exchanged ? 1 : 0;
+        rp.nact = pl.q > 0 ? pl.grid : pl.rem;
+        rp.xstep = (uint32_t)h->xstep;
+        rp.xrow = h->series_steps;
+        rp.ticket = h->res_prog + kResMaxGrid;       // the word after the progress words (zeroed at create, left at zero)
+        rp.sweep0 = (uint32_t)h->sweep_g;
+        rp.epoch = ++h->res_epoch;
+        rp.prog = h->res_prog;
+        rp.total_planes = pl.total; rp.q = pl.q; rp.rem = pl.rem;
+        rp.cap_reps = pl.cap_reps;
+        rp.d0 = d0;
+        rp.fielda_res = h->fielda_res; rp.fieldb_res = h->fieldb_res;
+        rp.diag = h->v.diag;
+        {
+            uint32_t k0 = (uint32_t)(h->seeds[d0] & 0xFFFFFFFFull), k1 = (uint32_t)(h->seeds[d0] >> 32);
+            for (int r = 0; r < 10; ++r) { rp.rk0[2 * r] = k0; rp.rk0[2 * r + 1] = k1; k0 += kPhiloxW0; k1 += kPhiloxW1; }
+        }
+        int rc;
+        if (h->kind == RFIM_FIELD_BIMODAL) {
+            if (h->L == 64) rc = h->has_never ? launch_res_k<0, 2, true>(h, pl, rp) : launch_res_k<0, 2, false>(h, pl, rp);
+            else rc = h->has_never ? launch_res_k<0, 1, true>(h, pl, rp) : launch_res_k<0, 1, false>(h, pl, rp);
+        } else {
+            rc = h->L == 64 ? launch_res_k<1, 2, false>(h, pl, rp) : launch_res_k<1, 1, false>(h, pl, rp);
+        }
+        if (rc) return rc;
     }
-    if (h->kind == RFIM_FIELD_BIMODAL) {
-        if (h->L == 64) return h->has_never ? launch_res_u<0, 2, true>(h, pl, rp) : launch_res_u<0, 2, false>(h, pl, rp);
-        return h->has_never ? launch_res_u<0, 1, true>(h, pl, rp) : launch_res_u<0, 1, false>(h, pl, rp);
-    }
-    if (h->L == 64) return launch_res_u<1, 2, false>(h, pl, rp);
-    return launch_res_u<1, 1, false>(h, pl, rp);
+    return RFIM_OK;
 }
 
 int launch_reduce(rfim_pt* h) {

@@ -84,6 +84,7 @@ struct ResParams {
     int total_planes;            // D * n * L
     int q, rem;                  // run of CTA b: start = b*q + min(b, rem), count = q + (b < rem)
     int cap_reps;                // replicas a run can touch -- same carve for every CTA
+    int d0;                      // first member of this launch's group (plane P = ((d - d0) * n + t) * L + z)
     const float* fielda_res;     // Gaussian: [D][2][L][2][4K][L/2] float4 (task order), (float)g_i (exact)
     const uint8_t* fieldb_res;   // bimodal:  [D][2][L][2][K][L/2] uint4, 0x80 where h_i = +1
     unsigned long long* diag;
@@ -466,7 +467,7 @@ __global__ void __launch_bounds__(THREADS, 1) k_sweep_res(const View v, const Re
         s_plane[p] = pi;
     }
     for (int r = tid; r < nrep; r += THREADS) {
-        const int dt = dt0 + r, d = dt / v.n, t = dt % v.n;
+        const int dt = dt0 + r, d = rp.d0 + dt / v.n, t = dt % v.n;
         ResRep rr;
         rr.d = d; rr.tr = d * v.R + t; rr.slot = v.t2r[rr.tr]; rr.ds = d * v.R + rr.slot;
         rr.band = KIND == 0 ? 0.f : v.band[rr.tr];
@@ -480,7 +481,7 @@ __global__ void __launch_bounds__(THREADS, 1) k_sweep_res(const View v, const Re
     // acceptance tables, 8-byte entries at byte offset SP*n1 + 8*SP*s (+ 16*SP*hb): Gaussian {x, y}, bimodal {thr-1, never}
     for (int i = tid; i < nrep * 32; i += THREADS) {
         const int r = i >> 5, idx = i & 31;
-        const int dt = dt0 + r, d = dt / v.n, t = dt % v.n, tr = d * v.R + t;
+        const int dt = dt0 + r, d = rp.d0 + dt / v.n, t = dt % v.n, tr = d * v.R + t;
         uint2 ent = make_uint2(0u, 0u);
         if (KIND == 0) {
             ent.x = v.etab[(long long)tr * 32 + idx];
