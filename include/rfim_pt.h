@@ -91,7 +91,13 @@ typedef void* (*rfim_pt_alloc_fn)(size_t bytes);
 typedef void (*rfim_pt_free_fn)(void* device_ptr);
 int rfim_pt_set_allocator(rfim_pt_alloc_fn alloc, rfim_pt_free_fn release);
 const char* rfim_pt_last_error(rfim_pt* h);
-/* 8 = one byte per spin (default), 1 = bit-packed.  Converts the stored lattices in place. */
+/* Storage of the lattices in device memory (BASELINE.json config 5 "spins bit-packed").
+ * 8 = one byte per spin (default), 1 = one bit per spin (bit j & 7 of byte j >> 3, j the same colour-separated
+ * site index as in the byte layout): an eighth of the footprint, every result identical to the byte layout
+ * ("int8 == bit-packed").  The call converts the stored lattices (synchronises; both buffers
+ * exist during the conversion).  Bit-packed lattices are read by the resident kernel only: RFIM_EINVAL unless
+ * L is 32 or 64 and the kernel variant is 0 or 4; a later sweep fails with RFIM_EINVAL if the active planes do
+ * not fit in shared memory.  Getters/setters keep their int8 +-1 interface in both modes. */
 int rfim_pt_set_packing(rfim_pt* h, int bits);
 /* which sweep implementation runs: 0 = automatic (default), 1 site, 2 word, 3 flow, 4 resident. */
 int rfim_pt_set_kernel_variant(rfim_pt* h, int variant);

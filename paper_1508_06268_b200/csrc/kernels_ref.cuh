@@ -167,28 +167,64 @@ __global__ void k_init_spins(View v) {
     }
 }
 
-// ---- natural-order +-1 int8  <->  colour-separated 0/1 bytes, slots [first, first+count) --------
+// ---- natural-order +-1 int8  <->  colour-separated 0/1 bytes (or bits), slots [first, first+count) --------
 __global__ void k_export_spins(View v, int first, int8_t* __restrict__ out) {
     const int ds = first + blockIdx.y;     // linear d*R + slot
     const int L = v.L, Lh = v.Lh;
-    const uint8_t* base = v.spins + (long long)ds * 2 * v.Nh;
+    const long long b0 = (long long)ds * 2 * v.Nh;
     int8_t* o = out + (long long)blockIdx.y * v.N;
     for (long long i = (long long)blockIdx.x * blockDim.x + threadIdx.x; i < v.N; i += (long long)gridDim.x * blockDim.x) {
         const int x = (int)(i % L), y = (int)((i / L) % L), z = (int)(i / ((long long)L * L));
         const int c = (x + y + z) & 1;
-        o[i] = base[(long long)c * v.Nh + (x >> 1) + (long long)Lh * (y + (long long)L * z)] ? 1 : -1;
+        const long long j = b0 + (long long)c * v.Nh + (x >> 1) + (long long)Lh * (y + (long long)L * z);
+        const int up = v.packed ? (v.spins[j >> 3] >> (j & 7)) & 1 : v.spins[j];
+        o[i] = up ? 1 : -1;
     }
 }
 
 __global__ void k_import_spins(View v, int first, const int8_t* __restrict__ in) {
     const int ds = first + blockIdx.y;
     const int L = v.L, Lh = v.Lh;
-    uint8_t* base = v.spins + (long long)ds * 2 * v.Nh;
     const int8_t* src = in + (long long)blockIdx.y * v.N;
+    if (v.packed) {                        // one thread per packed byte: eight same-colour sites
+        uint8_t* base = v.spins + (long long)ds * (v.N >> 3);
+        for (long long b = (long long)blockIdx.x * blockDim.x + threadIdx.x; b < (v.N >> 3); b += (long long)gridDim.x * blockDim.x) {
+            const int c = (int)(b / (v.Nh >> 3));
+            const long long j0 = (b % (v.Nh >> 3)) * 8;
+            uint32_t bits = 0;
+            for (int t = 0; t < 8; ++t) {
+                const long long j = j0 + t;
+                const int xh = (int)(j % Lh), y = (int)((j / Lh) % L), z = (int)(j / ((long long)Lh * L));
+                const int x = 2 * xh + ((y + z + c) & 1);
+                if (src[x + (long long)L * (y + (long long)L * z)] > 0) bits |= 1u << t;
+            }
+            base[b] = (uint8_t)bits;
+        }
+        return;
+    }
+    uint8_t* base = v.spins + (long long)ds * 2 * v.Nh;
     for (long long i = (long long)blockIdx.x * blockDim.x + threadIdx.x; i < v.N; i += (long long)gridDim.x * blockDim.x) {
         const int x = (int)(i % L), y = (int)((i / L) % L), z = (int)(i / ((long long)L * L));
         const int c = (x + y + z) & 1;
         base[(long long)c * v.Nh + (x >> 1) + (long long)Lh * (y + (long long)L * z)] = src[i] > 0 ? 1 : 0;
+    }
+}
+
+// ---- whole-buffer conversion between the byte and the bit layout (same index j, eight spins per byte) ----------
+__global__ void k_pack_bits(const uint8_t* __restrict__ bytes, uint8_t* __restrict__ bits, long long nbits_bytes) {
+    for (long long b = (long long)blockIdx.x * blockDim.x + threadIdx.x; b < nbits_bytes; b += (long long)gridDim.x * blockDim.x) {
+        const uint2 w = *reinterpret_cast<const uint2*>(bytes + 8 * b);
+        const uint32_t lo = ((w.x & 0x01010101u) * 0x01020408u) >> 24, hi = ((w.y & 0x01010101u) * 0x01020408u) >> 24;
+        bits[b] = (uint8_t)((lo & 0xFu) | ((hi & 0xFu) << 4));
+    }
+}
+__global__ void k_unpack_bits(const uint8_t* __restrict__ bits, uint8_t* __restrict__ bytes, long long nbits_bytes) {
+    for (long long b = (long long)blockIdx.x * blockDim.x + threadIdx.x; b < nbits_bytes; b += (long long)gridDim.x * blockDim.x) {
+        const uint32_t q = bits[b];
+        uint2 w;
+        w.x = ((q & 0xFu) * 0x00204081u) & 0x01010101u;
+        w.y = ((q >> 4) * 0x00204081u) & 0x01010101u;
+        *reinterpret_cast<uint2*>(bytes + 8 * b) = w;
     }
 }
 

@@ -48,6 +48,7 @@ struct rfim_pt {
     View v{};
     std::vector<void*> owned;         // every device allocation, released in destroy
     int8_t* stage = nullptr;          // device staging for spin import/export
+    uint8_t* unpacked = nullptr;      // packed mode: byte-layout scratch for the stand-alone reduction (allocated on first use)
     size_t stage_bytes = 0;
     uint64_t sweep_g = 0, xstep = 0;
     long long series_steps = 0, series_cap = 0;
@@ -343,6 +344,7 @@ ResPlan res_plan(const rfim_pt* h) {
 }
 
 int chosen_variant(const rfim_pt* h) {
+    if (h->packing == 1) return 4;              // only the resident kernel reads the bit layout
     if (h->variant != 0) return h->variant;
     if (res_plan(h).ok) return 4;
     if (flow_supported(h)) return 3;
@@ -468,8 +470,18 @@ int launch_res(rfim_pt* h, int sweeps, bool measure, bool* exchanged) {
 }
 
 int launch_reduce(rfim_pt* h) {
-    if (h->v.W > 0) k_reduce_word<<<grid_for(h->Nh / 4, h->D * h->n), 256, 0, h->stream>>>(h->v);
-    else k_reduce_site<<<grid_for(h->Nh, h->D * h->n), 256, 0, h->stream>>>(h->v);
+    View v = h->v;
+    if (h->packing == 1) {
+        // the stand-alone reduction reads the byte layout: unpack into scratch first (only the getters come here in
+        // packed mode; the sweep path measures inside the resident kernel)
+        const size_t DR = (size_t)h->D * h->R;
+        if (!h->unpacked) { int rc = alloc_into(h, &h->unpacked, DR * (size_t)h->N); if (rc) return rc; }
+        k_unpack_bits<<<grid_for((long long)(DR * (size_t)h->N / 8), 1), 256, 0, h->stream>>>(h->v.spins, h->unpacked, (long long)(DR * (size_t)h->N / 8));
+        h->launches += 1;
+        v.spins = h->unpacked; v.packed = 0;
+    }
+    if (v.W > 0) k_reduce_word<<<grid_for(h->Nh / 4, h->D * h->n), 256, 0, h->stream>>>(v);
+    else k_reduce_site<<<grid_for(h->Nh, h->D * h->n), 256, 0, h->stream>>>(v);
     h->launches += 1;
     CU(cudaGetLastError());
     return RFIM_OK;
@@ -722,13 +734,41 @@ int rfim_pt_synchronize(rfim_pt* h) {
 
 int rfim_pt_set_packing(rfim_pt* h, int bits) {
     if (!h) return RFIM_EINVAL;
-    if (bits == 8) { h->packing = 8; return RFIM_OK; }
-    return fail(h, RFIM_EINVAL, "packing must be 8 (bit-packed storage is not built yet)");
+    if (bits != 8 && bits != 1) return fail(h, RFIM_EINVAL, "packing must be 8 (one byte per spin) or 1 (one bit per spin)");
+    if (bits == h->packing) return RFIM_OK;
+    const size_t DR = (size_t)h->D * h->R, nbits_bytes = DR * (size_t)h->N / 8;
+    if (bits == 1) {
+        if (h->variant != 0 && h->variant != 4) return fail(h, RFIM_EINVAL, "bit-packed storage is read by the resident kernel only (variant 0 or 4)");
+        if (!flow_supported(h) || (h->have_T && !res_plan(h).ok))
+            return fail(h, RFIM_EINVAL, "bit-packed storage needs the resident kernel (L = 32 or 64, planes resident in shared memory)");
+        uint8_t* bitsbuf = nullptr;
+        int rc = alloc_into(h, &bitsbuf, nbits_bytes);
+        if (rc) return rc;
+        k_pack_bits<<<grid_for((long long)nbits_bytes, 1), 256, 0, h->stream>>>(h->v.spins, bitsbuf, (long long)nbits_bytes);
+        h->launches += 1;
+        CU(cudaGetLastError());
+        CU(cudaStreamSynchronize(h->stream));
+        release(h, h->v.spins);
+        h->v.spins = bitsbuf; h->v.packed = 1; h->packing = 1;
+    } else {
+        uint8_t* bytes = nullptr;
+        int rc = alloc_into(h, &bytes, DR * (size_t)h->N);
+        if (rc) return rc;
+        k_unpack_bits<<<grid_for((long long)nbits_bytes, 1), 256, 0, h->stream>>>(h->v.spins, bytes, (long long)nbits_bytes);
+        h->launches += 1;
+        CU(cudaGetLastError());
+        CU(cudaStreamSynchronize(h->stream));
+        release(h, h->v.spins);
+        if (h->unpacked) { release(h, h->unpacked); h->unpacked = nullptr; }
+        h->v.spins = bytes; h->v.packed = 0; h->packing = 8;
+    }
+    return RFIM_OK;
 }
 
 int rfim_pt_set_kernel_variant(rfim_pt* h, int variant) {
     if (!h) return RFIM_EINVAL;
     if (variant < 0 || variant > 4) return fail(h, RFIM_EINVAL, "unknown kernel variant");
+    if (h->packing == 1 && variant != 0 && variant != 4) return fail(h, RFIM_EINVAL, "bit-packed storage is read by the resident kernel only");
     if (variant == 4 && !flow_supported(h)) return fail(h, RFIM_EINVAL, "resident kernel needs L = 32 or 64");
     if (variant == 2 && h->v.W == 0) return fail(h, RFIM_EINVAL, "word kernel needs L % 8 == 0");
     if (variant == 3 && !flow_supported(h)) return fail(h, RFIM_EINVAL, "flow kernel needs L = 32 or 64");
@@ -813,8 +853,9 @@ int rfim_pt_adapt_temperatures(rfim_pt* h, int64_t trial_sweeps) {
             } else {
                 slot = next_slot++;
                 const int src = t2r[(size_t)d * R + p.copy_of[j]];
-                CU(cudaMemcpyAsync(h->v.spins + ((size_t)d * R + slot) * h->N, h->v.spins + ((size_t)d * R + src) * h->N,
-                                   (size_t)h->N, cudaMemcpyDeviceToDevice, h->stream));
+                const size_t lat = (size_t)h->N / (h->packing == 1 ? 8 : 1);      // bytes per lattice
+                CU(cudaMemcpyAsync(h->v.spins + ((size_t)d * R + slot) * lat, h->v.spins + ((size_t)d * R + src) * lat,
+                                   lat, cudaMemcpyDeviceToDevice, h->stream));
             }
             new_t2r[(size_t)d * R + j] = slot;
             h->T[(size_t)d * R + j] = p.T[j];

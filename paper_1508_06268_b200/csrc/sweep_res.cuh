@@ -141,6 +141,34 @@ __device__ __forceinline__ uint32_t prmt(uint32_t a, uint32_t b, uint32_t sel) {
 
 __device__ __forceinline__ int lds_volatile(const int* p) { return *reinterpret_cast<const volatile int*>(p); }
 
+// ---- one 16-site piece between its global form (16 bytes of 0/1, or 16 bits when View::packed) and the shared-memory
+// form (16 bytes of 0/SP).  `off` is the piece's index in spins (a multiple of 16).
+__device__ __forceinline__ uint32_t res_nibble_to_word(uint32_t nib) { return ((nib & 0xFu) * 0x00204081u) & 0x01010101u; }
+__device__ __forceinline__ uint32_t res_word_to_nibble(uint32_t w01) { return (((w01 & 0x01010101u) * 0x01020408u) >> 24) & 0xFu; }
+__device__ __forceinline__ uint4 res_piece_from_global(const uint8_t* spins, size_t off, int packed) {
+    uint4 x;
+    if (packed) {
+#if defined(__CUDA_ARCH__)
+        const uint32_t q = __ldcg(reinterpret_cast<const unsigned short*>(spins + (off >> 3)));
+#else
+        const uint32_t q = 0;
+#endif
+        x.x = res_nibble_to_word(q); x.y = res_nibble_to_word(q >> 4); x.z = res_nibble_to_word(q >> 8); x.w = res_nibble_to_word(q >> 12);
+    } else {
+        x = ld_cg16(spins + off);
+    }
+    x.x *= kResSP; x.y *= kResSP; x.z *= kResSP; x.w *= kResSP;
+    return x;
+}
+__device__ __forceinline__ void res_piece_to_global(uint8_t* spins, size_t off, int packed, uint4 x) {
+    x.x >>= 3; x.y >>= 3; x.z >>= 3; x.w >>= 3;
+    if (packed)
+        *reinterpret_cast<unsigned short*>(spins + (off >> 3)) = (unsigned short)(res_word_to_nibble(x.x) | (res_word_to_nibble(x.y) << 4) |
+                                                                                  (res_word_to_nibble(x.z) << 8) | (res_word_to_nibble(x.w) << 12));
+    else
+        *reinterpret_cast<uint4*>(spins + off) = x;
+}
+
 __device__ __forceinline__ Words4 philox_rkreg(const uint32_t (&rk)[20], uint32_t c0, uint32_t c1, uint32_t c2, uint32_t c3) {
 #pragma unroll
     for (int r = 0; r < 10; ++r) {
@@ -208,7 +236,7 @@ __device__ __noinline__ void res_wait_slow(const int* s_done, int eb, int b_zp, 
 struct ResPiece { uint32_t me[4], cw[4], ns[4]; };
 
 // rem: where the rows of a z-neighbour plane that lives in another CTA are found in global memory (boundary tasks only)
-struct ResRemote { const uint8_t* spins; uint32_t off_p, off_m; bool any, p, m; };
+struct ResRemote { const uint8_t* spins; uint32_t off_p, off_m; bool any, p, m; int packed; };
 
 // xr: the row's words of the other colour (all K pieces, loaded once per row: the far x-neighbour of a piece's edge
 // byte is a word of the neighbouring piece, periodic in x)
@@ -223,14 +251,8 @@ __device__ __forceinline__ ResPiece res_load_piece(const uint8_t* smem, const ui
     uint4 zm = *reinterpret_cast<const uint4*>(smem + a_zm + k * ARR);
     const uint4 m = *reinterpret_cast<const uint4*>(smem + a_me + k * ARR);
     if (rem.any) {                                  // warp-uniform: only boundary tasks come here
-        if (rem.p) {
-            zp = ld_cg16(rem.spins + (size_t)(rem.off_p + 16u * k));
-            zp.x *= kResSP; zp.y *= kResSP; zp.z *= kResSP; zp.w *= kResSP;
-        }
-        if (rem.m) {
-            zm = ld_cg16(rem.spins + (size_t)(rem.off_m + 16u * k));
-            zm.x *= kResSP; zm.y *= kResSP; zm.z *= kResSP; zm.w *= kResSP;
-        }
+        if (rem.p) zp = res_piece_from_global(rem.spins, (size_t)(rem.off_p + 16u * k), rem.packed);
+        if (rem.m) zm = res_piece_from_global(rem.spins, (size_t)(rem.off_m + 16u * k), rem.packed);
     }
     const uint32_t edge = dir == 0 ? xr[(k + K - 1) % K].w : xr[(k + 1) % K].x;
     ResPiece pc;
@@ -325,7 +347,7 @@ __device__ __forceinline__ void res_row(const View& v, const ResParams& rp, uint
     const uint4* fq = ln.fq0 + (s ? K * LH : 0);
     const uint32_t grow = ln.grow0 + (ys ? ROWB : 0);          // only BND and the rare exact path use it
     ResRemote rem;
-    rem.spins = v.spins; rem.any = BND; rem.p = BND && remote_p; rem.m = BND && remote_m;
+    rem.spins = v.spins; rem.any = BND; rem.p = BND && remote_p; rem.m = BND && remote_m; rem.packed = v.packed;
     rem.off_p = roff_p + (ys ? ROWB : 0); rem.off_m = roff_m + (ys ? ROWB : 0);
 
     uint32_t rk[20];
@@ -396,8 +418,7 @@ __device__ __forceinline__ void res_row(const View& v, const ResParams& rp, uint
         if (!RAGGED || valid) {
             *reinterpret_cast<uint4*>(smem + a_me + k * ARR) = nw;
             if (BND && (remote_p || remote_m))
-                *reinterpret_cast<uint4*>(v.spins + (size_t)((ln.ds2 + (uint32_t)c) * (uint32_t)v.Nh + grow + 16u * k)) =
-                    make_uint4(nw.x >> 3, nw.y >> 3, nw.z >> 3, nw.w >> 3);
+                res_piece_to_global(v.spins, (size_t)((ln.ds2 + (uint32_t)c) * (uint32_t)v.Nh + grow + 16u * k), v.packed, nw);
             if (MEAS) {
                 const float4 z4 = make_float4(0.f, 0.f, 0.f, 0.f);
                 const int3 m3 = res_measure_piece<KIND>(nw, make_uint4(idx8[0], idx8[1], idx8[2], idx8[3]), fb,
@@ -515,9 +536,7 @@ __global__ void __launch_bounds__(THREADS, 1) k_sweep_res(const View v, const Re
             const int k = u % K, y = (u / K) % L, col = (u / (K * L)) & 1, p = u / (2 * K * L);
             const ResPlane pi = s_plane[p];
             const int ds = s_rep[pi.rep].ds, z = pi.z;
-            const uint8_t* src = v.spins + ((long long)ds * 2 + col) * v.Nh + ((long long)z * L + y) * ROWB + 16 * k;
-            uint4 x = ld_cg16(src);
-            x.x *= kResSP; x.y *= kResSP; x.z *= kResSP; x.w *= kResSP;
+            const uint4 x = res_piece_from_global(v.spins, (size_t)(((long long)ds * 2 + col) * v.Nh + ((long long)z * L + y) * ROWB + 16 * k), v.packed);
             *reinterpret_cast<uint4*>(smem + A(col, (y + z) & 1, k, p * LH + (y >> 1))) = x;
         }
     }
@@ -644,9 +663,8 @@ __global__ void __launch_bounds__(THREADS, 1) k_sweep_res(const View v, const Re
             const int k = u % K, y = (u / K) % L, col = (u / (K * L)) & 1, p = u / (2 * K * L);
             const ResPlane pi = s_plane[p];
             const int ds = s_rep[pi.rep].ds, z = pi.z;
-            uint4 x = *reinterpret_cast<const uint4*>(smem + A(col, (y + z) & 1, k, p * LH + (y >> 1)));
-            x.x >>= 3; x.y >>= 3; x.z >>= 3; x.w >>= 3;
-            *reinterpret_cast<uint4*>(v.spins + ((long long)ds * 2 + col) * v.Nh + ((long long)z * L + y) * ROWB + 16 * k) = x;
+            const uint4 x = *reinterpret_cast<const uint4*>(smem + A(col, (y + z) & 1, k, p * LH + (y >> 1)));
+            res_piece_to_global(v.spins, (size_t)(((long long)ds * 2 + col) * v.Nh + ((long long)z * L + y) * ROWB + 16 * k), v.packed, x);
         }
         if (rp.measure)
             for (int r = tid; r < nrep * 3; r += THREADS)

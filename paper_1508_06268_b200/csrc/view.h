@@ -36,6 +36,7 @@ struct View {
     long long* series;             // [capacity][D][R(rank)][3]
     unsigned long long* diag;      // [4], see rfim_pt_get_diagnostics
     double J, hs;                  // hs = h (bimodal) or h * 2^-20 (Gaussian)
+    int packed;                    // != 0: `spins` holds one BIT per spin (bit j & 7 of byte j >> 3, same index j as the byte layout)
 };
 
 }  // namespace rfim

@@ -1,0 +1,106 @@
+"""-m gpu: bit-packed storage (rfim_pt_set_packing(1), SURVEY.md 8(b)/(c) "int8 == bit-packed").
+
+One bit per spin in device memory; the resident kernel expands a run into shared memory at load and packs it at
+store (boundary rows are published packed too).  Every result -- spins, integer energies, permutation, time series --
+must equal the oracle's, hence the byte layout's, bit for bit.
+"""
+import numpy as np
+import pytest
+
+from parity_util import assert_same_series, assert_same_state, make_pair
+from paper_1508_06268_b200.workloads import geometric_ladder, linear_ladder
+
+pytestmark = pytest.mark.gpu
+
+BIMODAL, GAUSSIAN = 0, 1
+
+
+@pytest.mark.parametrize("L,R,grid", [(32, 5, 0), (32, 5, 7), (64, 3, 0), (64, 3, 5)])
+@pytest.mark.parametrize("kind,h", [(BIMODAL, 2.0), (GAUSSIAN, 1.5)])
+def test_packed_storage_bit_exact(L, R, grid, kind, h):
+    """pack at the start, sweep with exchanges in several launch shapes, compare everything with the oracle."""
+    T = geometric_ladder(0.9, 5.5, R)
+    g, o = make_pair(L, R, 1.0, h, kind, 23, T)
+    g.set_packing(1)
+    if grid:
+        g.set_tuning(1, grid)
+    for r in range(R):                       # the conversion kept the initial state
+        assert np.array_equal(g.get_spins_slot(r), o.get_spins_slot(r))
+    for n, k in ((3, 0), (10, 5), (7, 2)):
+        g.sweep(n, k); o.sweep(n, k)
+        assert_same_state(g, o, what=f"packed L={L} grid={grid} after sweep({n},{k})")
+    assert_same_series(g, o)
+    assert g.diagnostics()["ulp_ambiguous"] == 0
+    g.close()
+
+
+@pytest.mark.parametrize("kind", [BIMODAL, GAUSSIAN])
+def test_packing_roundtrip_set_get_and_mixed_modes(kind):
+    """8 -> 1 -> 8 keeps every spin; set/get work in packed mode; sweeping packed then unpacked follows the oracle."""
+    L, R = 32, 4
+    T = linear_ladder(1.0, 5.0, R)
+    g, o = make_pair(L, R, 1.0, 1.5, kind, 5, T)
+    rng = np.random.default_rng(7)
+    lat = (rng.integers(0, 2, size=(R, L ** 3)) * 2 - 1).astype(np.int8)
+    g.set_packing(1)
+    for r in range(R):
+        g.set_spins_slot(r, lat[r]); o.set_spins_slot(r, lat[r])
+        assert np.array_equal(g.get_spins_slot(r), lat[r])
+    g.sweep(6, 3); o.sweep(6, 3)
+    assert_same_state(g, o, what="packed segment")
+    g.set_packing(8)
+    assert_same_state(g, o, what="after unpacking")
+    g.sweep(5, 5); o.sweep(5, 5)
+    assert_same_state(g, o, what="byte segment")
+    g.set_packing(1)
+    allspins = g.get_spins_all()
+    for r in range(R):
+        assert np.array_equal(allspins[0, r], o.get_spins_slot(r))
+    g.set_spins_all(allspins)
+    g.sweep(4, 2); o.sweep(4, 2)
+    assert_same_state(g, o, what="packed again")
+    g.close()
+
+
+def test_packed_batch_and_adaptation():
+    """batch members and the growing adaptation (copy of a lattice into a pool slot) in packed mode."""
+    import oracle
+    from paper_1508_06268_b200 import binding
+    L, R, n = 32, 8, 5
+    seeds = [101, 102, 103]
+    T = geometric_ladder(1.0, 5.0, n)
+    g = binding.RfimPT(L, R, 1.0, 1.5, GAUSSIAN, seeds=seeds)
+    g.set_packing(1)
+    g.set_temperatures(T)
+    g.set_adapt_params(5, 2)
+    g.adapt_temperatures(20)
+    g.sweep(10, 5)
+    for d, seed in enumerate(seeds):
+        o = oracle.Oracle(L, R, 1.0, 1.5, GAUSSIAN, seed)
+        o.set_temperatures(T)
+        o.set_adapt_params(5, 2)
+        o.adapt_temperatures(20)
+        o.sweep(10, 5)
+        assert np.array_equal(g.get_temperatures(d=d), o.get_temperatures())
+        assert_same_state(g, o, d=d, what=f"packed batch member {d}")
+    g.close()
+
+
+def test_packing_errors():
+    from paper_1508_06268_b200 import binding
+    g = binding.RfimPT(16, 4, 1.0, 1.0, BIMODAL, seed=1)
+    with pytest.raises(binding.RfimPtError) as e:
+        g.set_packing(1)                     # L = 16: no resident kernel
+    assert e.value.code == binding.EINVAL
+    with pytest.raises(binding.RfimPtError):
+        g.set_packing(4)
+    g.close()
+    g = binding.RfimPT(32, 4, 1.0, 1.0, BIMODAL, seed=1)
+    g.set_kernel_variant(3)
+    with pytest.raises(binding.RfimPtError):
+        g.set_packing(1)                     # the flow kernel reads bytes
+    g.set_kernel_variant(0)
+    g.set_packing(1)
+    with pytest.raises(binding.RfimPtError):
+        g.set_kernel_variant(2)
+    g.close()
