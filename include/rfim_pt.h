@@ -49,6 +49,36 @@ int rfim_pt_create(rfim_pt** out, int L, int R, double J, double h, int field_ki
 int rfim_pt_create_batch(rfim_pt** out, int L, int R, double J, double h, int field_kind,
                          int D, const uint64_t* seeds);
 
+/* ---- replica distribution over several GPUs --------------------------
+ * One realisation, R replica slots dealt to G ranks in contiguous windows of nslots = ceil(R/G) (Eq. 6:
+ * m = ceil(M/D) replicas per GPU): the handle of rank g is created with slot0 = g * nslots and STORES only the
+ * lattices of slots [slot0, slot0 + nslots) (slots >= R of the last window are never active).  Field, temperatures,
+ * tables, the permutation t2r/r2t, exchange counters and the time series are replicated on every rank and stay
+ * identical, because every rank takes the same exchange decisions from the same counter-based random stream: lattices
+ * never move, only temperatures do.  The Philox counters are keyed on the global slot, so a sharded
+ * run is bit-identical to the single-handle run.
+ *
+ * Sweeps need no communication.  Before every exchange step (and in the energy getters) each rank holds the integer
+ * energy terms (Eb, Ef, Msum: 3 x int64 = 24 bytes per slot) of its own slots only; the library then calls the
+ * gather function, which must complete the array on every rank -- an all-gather of local_bytes per rank:
+ *   terms_device     device pointer, int64[rows][3], rows = G * nslots (padded), the same array on every call
+ *   local_offset     byte offset of this rank's rows (= slot0 * 24),  local_bytes = nslots * 24
+ *   total_bytes      rows * 24
+ *   stream           the handle's CUDA stream (cudaStream_t): the collective must be ordered after the work already
+ *                    enqueued on it and before work enqueued later (e.g. ncclAllGather on that stream, in place)
+ * returning 0 on success.  The pointer stays owned by the library.  Restrictions: D = 1; slot0 a multiple of nslots;
+ * only the resident kernel visits a slot window (L = 32 or 64); an adaptation step that INSERTS replicas would copy a
+ * lattice to another rank and returns RFIM_EINVAL (the fixed-count, rank-preserving mode works: no lattice moves);
+ * rfim_pt_get/set_spins_slot accept the stored slots only and rfim_pt_get/set_spins_all move the nslots stored
+ * lattices. */
+typedef int (*rfim_pt_gather_fn)(void* user, void* terms_device, size_t local_offset, size_t local_bytes,
+                                 size_t total_bytes, void* stream);
+int rfim_pt_create_shard(rfim_pt** out, int L, int R, double J, double h, int field_kind, uint64_t seed,
+                         int slot0, int nslots);
+int rfim_pt_set_gather(rfim_pt* h, rfim_pt_gather_fn fn, void* user);
+/* slot window and the energy-term array the gather function completes (any output pointer may be NULL) */
+int rfim_pt_get_shard(rfim_pt* h, int* slot0, int* nslots, void** terms_device, size_t* terms_bytes);
+
 int rfim_pt_destroy(rfim_pt* h);
 
 /* PAPER.md:67 (step 1) + step 3's X_i <- beta_i: T[0..n) strictly ascending, > 0, 1 <= n <= R.

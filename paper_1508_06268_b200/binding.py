@@ -24,6 +24,8 @@ _i8p = ctypes.POINTER(ctypes.c_int8)
 _i32p = ctypes.POINTER(ctypes.c_int32)
 _i64p = ctypes.POINTER(ctypes.c_int64)
 _u64p = ctypes.POINTER(ctypes.c_uint64)
+_GATHER_FN = ctypes.CFUNCTYPE(ctypes.c_int, ctypes.c_void_p, ctypes.c_void_p, ctypes.c_size_t, ctypes.c_size_t, ctypes.c_size_t,
+                              ctypes.c_void_p)
 _ALLOC_FN = ctypes.CFUNCTYPE(ctypes.c_void_p, ctypes.c_size_t)
 _FREE_FN = ctypes.CFUNCTYPE(None, ctypes.c_void_p)
 
@@ -33,6 +35,10 @@ SIGNATURES = {
                                       ctypes.c_int, ctypes.c_uint64]),
     "rfim_pt_create_batch": (ctypes.c_int, [ctypes.POINTER(_vp), ctypes.c_int, ctypes.c_int, ctypes.c_double,
                                             ctypes.c_double, ctypes.c_int, ctypes.c_int, _u64p]),
+    "rfim_pt_create_shard": (ctypes.c_int, [ctypes.POINTER(_vp), ctypes.c_int, ctypes.c_int, ctypes.c_double, ctypes.c_double,
+                                            ctypes.c_int, ctypes.c_uint64, ctypes.c_int, ctypes.c_int]),
+    "rfim_pt_set_gather": (ctypes.c_int, [_vp, _GATHER_FN, _vp]),
+    "rfim_pt_get_shard": (ctypes.c_int, [_vp, _ip, _ip, ctypes.POINTER(_vp), ctypes.POINTER(ctypes.c_size_t)]),
     "rfim_pt_destroy": (ctypes.c_int, [_vp]),
     "rfim_pt_set_temperatures": (ctypes.c_int, [_vp, _dp, ctypes.c_int]),
     "rfim_pt_sweep": (ctypes.c_int, [_vp, ctypes.c_int64, ctypes.c_int]),
@@ -97,6 +103,8 @@ def use_torch_allocator():
     """Route the library's device allocations through PyTorch's CUDA caching allocator."""
     import torch
     lib = load()
+    if "alloc" in _alloc_refs:            # installed once per process (handles may be created from several threads)
+        return
 
     def _alloc(nbytes):
         try:
@@ -125,7 +133,7 @@ def _p(a, t):
 class RfimPT:
     """Handle on D realisations x R replica slots of an L^3 lattice (see include/rfim_pt.h)."""
 
-    def __init__(self, L, R, J, h, field_kind, seed=None, seeds=None, torch_allocator=True, torch_stream=True):
+    def __init__(self, L, R, J, h, field_kind, seed=None, seeds=None, torch_allocator=True, torch_stream=True, shard=None):
         lib = load()
         if torch_allocator:
             import torch
@@ -134,7 +142,12 @@ class RfimPT:
             torch.cuda.init()
             use_torch_allocator()
         self._h = _vp()
-        if seeds is None:
+        self.shard = shard
+        self._gather_ref = None
+        if shard is not None:             # (slot0, nslots): this handle stores that window of the R slots
+            rc = lib.rfim_pt_create_shard(ctypes.byref(self._h), L, R, J, h, field_kind, int(seed), int(shard[0]), int(shard[1]))
+            self.D = 1
+        elif seeds is None:
             rc = lib.rfim_pt_create(ctypes.byref(self._h), L, R, J, h, field_kind, int(seed))
             self.D = 1
         else:
@@ -145,6 +158,7 @@ class RfimPT:
             raise RfimPtError(rc, "rfim_pt_create failed (bad argument, no CUDA device, or out of memory)")
         self.L, self.R, self.J, self.h, self.kind = L, R, J, h, field_kind
         self.N = L ** 3
+        self.stored_slots = R if shard is None else int(shard[1])     # lattices this handle keeps in device memory
         self._torch_stream = torch_stream
         if torch_stream:
             self.use_current_torch_stream()
@@ -206,6 +220,25 @@ class RfimPT:
         return out
 
     # -- extensions ------------------------------------------------------------------------------
+    def set_gather(self, fn):
+        """fn(terms_device_ptr, local_offset, local_bytes, total_bytes, stream_ptr) -> None: completes the energy-term
+        array across ranks (include/rfim_pt.h, replica distribution).  Exceptions become a non-zero return code."""
+        def _thunk(user, terms, off, nloc, ntot, stream):
+            try:
+                fn(terms, off, nloc, ntot, stream)
+                return 0
+            except Exception:                       # must not unwind through the C library
+                import traceback
+                traceback.print_exc()
+                return 1
+        self._gather_ref = _GATHER_FN(_thunk)       # keep the thunk alive as long as the handle
+        self._ck(load().rfim_pt_set_gather(self._h, self._gather_ref, None))
+
+    def get_shard(self):
+        a, b, ptr, nb = ctypes.c_int(), ctypes.c_int(), _vp(), ctypes.c_size_t()
+        self._ck(load().rfim_pt_get_shard(self._h, ctypes.byref(a), ctypes.byref(b), ctypes.byref(ptr), ctypes.byref(nb)))
+        return a.value, b.value, ptr.value, nb.value
+
     def set_packing(self, bits):
         self._ck(load().rfim_pt_set_packing(self._h, bits))
 
@@ -230,12 +263,12 @@ class RfimPT:
 
     def get_spins_all(self, out=None):
         if out is None:
-            out = np.zeros((self.D, self.R, self.N), dtype=np.int8)
+            out = np.zeros((self.D, self.stored_slots, self.N), dtype=np.int8)
         self._ck(load().rfim_pt_get_spins_all(self._h, _p(out, _i8p)))
         return out
 
     def set_spins_all(self, s):
-        assert s.dtype == np.int8 and s.size == self.D * self.R * self.N and s.flags.c_contiguous
+        assert s.dtype == np.int8 and s.size == self.D * self.stored_slots * self.N and s.flags.c_contiguous
         self._ck(load().rfim_pt_set_spins_all(self._h, _p(s, _i8p)))
 
     def get_field(self, d=0):

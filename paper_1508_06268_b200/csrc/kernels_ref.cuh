@@ -154,10 +154,10 @@ __global__ void k_sweep_word(View v, int colour, uint32_t sweep) {
 
 // ---- initial spins (S2, domain 3): one thread per site in natural order ---------------
 __global__ void k_init_spins(View v) {
-    const int d = blockIdx.y / v.R, slot = blockIdx.y % v.R;
+    const int d = blockIdx.y / v.Rs, slot = v.slot0 + blockIdx.y % v.Rs;      // grid.y = D * (stored slots per member)
     const uint32_t k0 = v.keys[2 * d], k1 = v.keys[2 * d + 1];
     const int L = v.L, Lh = v.Lh;
-    uint8_t* base = v.spins + (long long)(d * v.R + slot) * 2 * v.Nh;
+    uint8_t* base = v.spins + (long long)blockIdx.y * 2 * v.Nh;
     for (long long i = (long long)blockIdx.x * blockDim.x + threadIdx.x; i < v.N; i += (long long)gridDim.x * blockDim.x) {
         const Words4 w = philox4x32_10(k0, k1, (uint32_t)(i >> 2), 0u, (uint32_t)slot, kDomInitSpins);
         const uint32_t bit = pick_word(w, (uint32_t)(i & 3)) >> 31;
@@ -241,8 +241,9 @@ __device__ __forceinline__ long long warp_sum(long long x) {
 __global__ void k_reduce_site(View v) {
     const int d = blockIdx.y / v.n, t = blockIdx.y % v.n;
     const int slot = v.t2r[d * v.R + t];
+    if (slot < v.slot0 || slot >= v.slot0 + v.Rs) return;                     // a replica shard reduces the slots it stores
     const long long Nh = v.Nh;
-    const uint8_t* c0 = v.spins + (long long)(d * v.R + slot) * 2 * Nh;
+    const uint8_t* c0 = v.spins + (long long)(d * v.Rs + slot - v.slot0) * 2 * Nh;
     const uint8_t* c1 = c0 + Nh;
     const long long f0 = (long long)d * 2 * Nh, f1 = f0 + Nh;
     const int L = v.L, Lh = v.Lh;

@@ -48,6 +48,11 @@ struct rfim_pt {
     View v{};
     std::vector<void*> owned;         // every device allocation, released in destroy
     int8_t* stage = nullptr;          // device staging for spin import/export
+    int slot0 = 0, Rs = 0;            // stored slot window (replica shard: [slot0, slot0 + Rs) of R; else 0, R)
+    bool shard = false;
+    rfim_pt_gather_fn gather = nullptr;   // shard: completes View::acc across ranks before an exchange step
+    void* gather_user = nullptr;
+    size_t acc_rows = 0;              // rows of View::acc (>= R; padded to a whole number of shards)
     uint8_t* unpacked = nullptr;      // packed mode: byte-layout scratch for the stand-alone reduction (allocated on first use)
     size_t stage_bytes = 0;
     uint64_t sweep_g = 0, xstep = 0;
@@ -264,7 +269,7 @@ int reset_statistics(rfim_pt* h) {
     const size_t DR = (size_t)h->D * h->R;
     CU(cudaMemsetAsync(h->v.att, 0, DR * 8, h->stream));
     CU(cudaMemsetAsync(h->v.accn, 0, DR * 8, h->stream));
-    CU(cudaMemsetAsync(h->v.acc, 0, DR * 3 * 8, h->stream));
+    CU(cudaMemsetAsync(h->v.acc, 0, (size_t)h->D * h->acc_rows * 24, h->stream));
     h->series_steps = 0;
     return RFIM_OK;
 }
@@ -309,16 +314,22 @@ int ensure_stage(rfim_pt* h, size_t bytes) {
 bool flow_supported(const rfim_pt* h) { return h->L == 32 || h->L == 64; }
 
 // the resident kernel's partition of the D*n*L planes over the grid, and whether the largest run fits in shared memory
+// replicas one sweep of this handle visits: every active rank, or the active slots a shard stores (active slots are 0 .. n-1)
+int iterated(const rfim_pt* h) {
+    if (!h->shard) return h->n;
+    return std::max(0, std::min(h->n, h->slot0 + h->Rs) - h->slot0);
+}
+
 struct ResPlan { int grid, total, q, rem, cap_planes, cap_reps, nd, groups; size_t smem; bool ok; };
 // plan for `nd` members per launch
 ResPlan res_plan_nd(const rfim_pt* h, int nd) {
     ResPlan p{};
     p.ok = false;
     p.nd = nd; p.groups = (h->D + nd - 1) / nd;
-    if (!flow_supported(h) || h->n < 1 || h->sm_count < 1) return p;
+    if (!flow_supported(h) || h->n < 1 || iterated(h) < 1 || h->sm_count < 1) return p;
     p.grid = std::min(h->sm_count, kResMaxGrid);
     if (h->res_grid_limit > 0) p.grid = std::min(p.grid, h->res_grid_limit);
-    const long long total = (long long)nd * h->n * h->L;
+    const long long total = (long long)nd * iterated(h) * h->L;
     if (total > (long long)p.grid * 32767) return p;
     p.total = (int)total;
     p.q = p.total / p.grid; p.rem = p.total % p.grid;
@@ -344,7 +355,7 @@ ResPlan res_plan(const rfim_pt* h) {
 }
 
 int chosen_variant(const rfim_pt* h) {
-    if (h->packing == 1) return 4;              // only the resident kernel reads the bit layout
+    if (h->packing == 1 || h->shard) return 4;  // only the resident kernel reads the bit layout / visits a slot window
     if (h->variant != 0) return h->variant;
     if (res_plan(h).ok) return 4;
     if (flow_supported(h)) return 3;
@@ -430,9 +441,10 @@ int launch_res_k(rfim_pt* h, const ResPlan& pl, const ResParams& rp) { return la
 
 // `sweeps` (<= 127) sweeps of every active replica of every member: one cooperative launch per group of members
 int launch_res(rfim_pt* h, int sweeps, bool measure, bool* exchanged) {
+    if (h->shard && iterated(h) == 0) { *exchanged = false; return RFIM_OK; }      // this shard stores no active slot
     const ResPlan pl0 = res_plan(h);
     if (!pl0.ok) return fail(h, RFIM_EINVAL, "resident kernel: the planes of one CTA do not fit in shared memory");
-    *exchanged = measure && pl0.groups == 1 && h->D <= kResFusedExchangeMaxD;
+    *exchanged = measure && pl0.groups == 1 && h->D <= kResFusedExchangeMaxD && !h->shard;
     for (int d0 = 0; d0 < h->D; d0 += pl0.nd) {
         const int nd = std::min(pl0.nd, h->D - d0);
         const ResPlan pl = nd == pl0.nd ? pl0 : res_plan_nd(h, nd);
@@ -469,12 +481,23 @@ int launch_res(rfim_pt* h, int sweeps, bool measure, bool* exchanged) {
     return RFIM_OK;
 }
 
+// replica shard: every rank now holds the energy terms of the slots it stores; the caller-supplied collective fills in
+// the rows of the other ranks (an all-gather of 24 bytes per slot) so that every rank takes the same
+// exchange decisions.  Runs on the handle's stream.
+int gather_terms(rfim_pt* h) {
+    if (!h->shard) return RFIM_OK;
+    if (!h->gather) return fail(h, RFIM_ESTATE, "replica shard: no gather function set (rfim_pt_set_gather)");
+    const int rc = h->gather(h->gather_user, h->v.acc, (size_t)h->slot0 * 24, (size_t)h->Rs * 24, h->acc_rows * 24, h->stream);
+    if (rc) return fail(h, RFIM_ECUDA, "replica shard: the gather function failed");
+    return RFIM_OK;
+}
+
 int launch_reduce(rfim_pt* h) {
     View v = h->v;
     if (h->packing == 1) {
         // the stand-alone reduction reads the byte layout: unpack into scratch first (only the getters come here in
         // packed mode; the sweep path measures inside the resident kernel)
-        const size_t DR = (size_t)h->D * h->R;
+        const size_t DR = (size_t)h->D * h->Rs;
         if (!h->unpacked) { int rc = alloc_into(h, &h->unpacked, DR * (size_t)h->N); if (rc) return rc; }
         k_unpack_bits<<<grid_for((long long)(DR * (size_t)h->N / 8), 1), 256, 0, h->stream>>>(h->v.spins, h->unpacked, (long long)(DR * (size_t)h->N / 8));
         h->launches += 1;
@@ -523,6 +546,7 @@ int do_sweeps(rfim_pt* h, int64_t n_sweeps, int k) {
         left -= chunk;
         if (step_after) {
             if (variant != 4 && (rc = launch_reduce(h))) return rc;
+            if ((rc = gather_terms(h))) return rc;
             if (!exchanged && (rc = launch_exchange(h))) return rc;
             h->series_steps += 1;
             h->xstep += 1;
@@ -534,14 +558,15 @@ int do_sweeps(rfim_pt* h, int64_t n_sweeps, int k) {
 // current integer terms of every active replica, by rank: out [D][n][3]; also returns t2r [D][R]
 int measure_now(rfim_pt* h, std::vector<long long>& terms, std::vector<int32_t>& t2r) {
     const size_t DR = (size_t)h->D * h->R;
-    CU(cudaMemsetAsync(h->v.acc, 0, DR * 3 * 8, h->stream));
+    CU(cudaMemsetAsync(h->v.acc, 0, (size_t)h->D * h->acc_rows * 24, h->stream));
     int rc = launch_reduce(h);
     if (rc) return rc;
+    if ((rc = gather_terms(h))) return rc;
     std::vector<long long> acc(DR * 3);
     t2r.assign(DR, -1);
     CU(cudaMemcpyAsync(acc.data(), h->v.acc, DR * 3 * 8, cudaMemcpyDeviceToHost, h->stream));
     CU(cudaMemcpyAsync(t2r.data(), h->v.t2r, DR * 4, cudaMemcpyDeviceToHost, h->stream));
-    CU(cudaMemsetAsync(h->v.acc, 0, DR * 3 * 8, h->stream));
+    CU(cudaMemsetAsync(h->v.acc, 0, (size_t)h->D * h->acc_rows * 24, h->stream));
     CU(cudaStreamSynchronize(h->stream));
     terms.assign((size_t)h->D * h->n * 3, 0);
     for (int d = 0; d < h->D; ++d)
@@ -558,7 +583,7 @@ int check_member(rfim_pt* h, int d) {
     return RFIM_OK;
 }
 
-int create_impl(rfim_pt** out, int L, int R, double J, double hh, int kind, int D, const uint64_t* seeds) {
+int create_impl(rfim_pt** out, int L, int R, double J, double hh, int kind, int D, const uint64_t* seeds, int slot0 = 0, int nslots = -1) {
     if (!out) return RFIM_EINVAL;
     *out = nullptr;
     if (L < 2 || (L & 1) || L > 1024 || R < 1 || R > 4096 || D < 1 || D > 4096 || !seeds) return RFIM_EINVAL;
@@ -566,8 +591,12 @@ int create_impl(rfim_pt** out, int L, int R, double J, double hh, int kind, int 
     if (!std::isfinite(J) || !std::isfinite(hh)) return RFIM_EINVAL;
     int ndev = 0;
     if (cudaGetDeviceCount(&ndev) != cudaSuccess || ndev < 1) return RFIM_ECUDA;   // no CPU fallback
+    const bool shard = nslots >= 0;
+    if (shard && (D != 1 || slot0 < 0 || nslots < 1 || slot0 >= R || slot0 % nslots != 0)) return RFIM_EINVAL;
     rfim_pt* h = new rfim_pt();
     h->L = L; h->R = R; h->D = D; h->kind = kind; h->J = J; h->h = hh;
+    h->shard = shard; h->slot0 = shard ? slot0 : 0; h->Rs = shard ? nslots : R;
+    h->acc_rows = shard ? (size_t)((R + nslots - 1) / nslots) * nslots : (size_t)R;
     h->N = (long long)L * L * L; h->Nh = h->N / 2;
     h->seeds.assign(seeds, seeds + D);
     h->field_nat.assign((size_t)D * h->N, 0);
@@ -578,10 +607,11 @@ int create_impl(rfim_pt** out, int L, int R, double J, double hh, int kind, int 
     v.W = (L % 8 == 0) ? L / 8 : 0;
     v.N = h->N; v.Nh = h->Nh;
     v.J = J; v.hs = (kind == RFIM_FIELD_BIMODAL) ? hh : hh / kFieldScale;
+    v.shard = shard ? 1 : 0; v.slot0 = h->slot0; v.Rs = h->Rs; v.n_it = 0;
     const size_t DR = (size_t)D * R;
     int rc = RFIM_OK;
     auto A = [&](int r) { if (rc == RFIM_OK) rc = r; };
-    A(alloc_into(h, &v.spins, DR * (size_t)h->N));
+    A(alloc_into(h, &v.spins, (size_t)D * h->Rs * (size_t)h->N));
     if (kind == RFIM_FIELD_BIMODAL) {
         A(alloc_into(h, const_cast<uint8_t**>(&v.fieldb), (size_t)D * h->N));
         A(alloc_into(h, const_cast<uint32_t**>(&v.etab), DR * 32));
@@ -596,7 +626,7 @@ int create_impl(rfim_pt** out, int L, int R, double J, double hh, int kind, int 
     A(alloc_into(h, &v.t2r, DR));
     A(alloc_into(h, &v.r2t, DR));
     A(alloc_into(h, const_cast<uint32_t**>(&v.keys), (size_t)D * 2));
-    A(alloc_into(h, &v.acc, DR * 3));
+    A(alloc_into(h, &v.acc, (size_t)D * h->acc_rows * 3));
     A(alloc_into(h, &v.ework, DR));
     A(alloc_into(h, &v.att, DR));
     A(alloc_into(h, &v.accn, DR));
@@ -631,7 +661,7 @@ int create_impl(rfim_pt** out, int L, int R, double J, double hh, int kind, int 
             generate_field_host(h, d);
             if ((r2 = upload_field(h, d))) return r2;
         }
-        k_init_spins<<<grid_for(h->N, D * R), 256, 0, h->stream>>>(v);
+        k_init_spins<<<grid_for(h->N, D * h->Rs), 256, 0, h->stream>>>(v);
         h->launches += 1;
         CU(cudaGetLastError());
         CU(cudaStreamSynchronize(h->stream));
@@ -709,6 +739,26 @@ int rfim_pt_create_batch(rfim_pt** out, int L, int R, double J, double hh, int f
     return create_impl(out, L, R, J, hh, field_kind, D, seeds);
 }
 
+int rfim_pt_create_shard(rfim_pt** out, int L, int R, double J, double hh, int field_kind, uint64_t seed, int slot0, int nslots) {
+    return create_impl(out, L, R, J, hh, field_kind, 1, &seed, slot0, nslots);
+}
+
+int rfim_pt_set_gather(rfim_pt* h, rfim_pt_gather_fn fn, void* user) {
+    if (!h) return RFIM_EINVAL;
+    if (!h->shard) return fail(h, RFIM_EINVAL, "not a replica shard");
+    h->gather = fn; h->gather_user = user;
+    return RFIM_OK;
+}
+
+int rfim_pt_get_shard(rfim_pt* h, int* slot0, int* nslots, void** terms_device, size_t* terms_bytes) {
+    if (!h) return RFIM_EINVAL;
+    if (slot0) *slot0 = h->slot0;
+    if (nslots) *nslots = h->Rs;
+    if (terms_device) *terms_device = h->v.acc;
+    if (terms_bytes) *terms_bytes = (size_t)h->D * h->acc_rows * 24;
+    return RFIM_OK;
+}
+
 int rfim_pt_destroy(rfim_pt* h) {
     if (!h) return RFIM_OK;
     cudaStreamSynchronize(h->stream);
@@ -736,7 +786,7 @@ int rfim_pt_set_packing(rfim_pt* h, int bits) {
     if (!h) return RFIM_EINVAL;
     if (bits != 8 && bits != 1) return fail(h, RFIM_EINVAL, "packing must be 8 (one byte per spin) or 1 (one bit per spin)");
     if (bits == h->packing) return RFIM_OK;
-    const size_t DR = (size_t)h->D * h->R, nbits_bytes = DR * (size_t)h->N / 8;
+    const size_t DR = (size_t)h->D * h->Rs, nbits_bytes = DR * (size_t)h->N / 8;
     if (bits == 1) {
         if (h->variant != 0 && h->variant != 4) return fail(h, RFIM_EINVAL, "bit-packed storage is read by the resident kernel only (variant 0 or 4)");
         if (!flow_supported(h) || (h->have_T && !res_plan(h).ok))
@@ -797,7 +847,7 @@ int rfim_pt_set_temperatures(rfim_pt* h, const double* T, int n) {
         if (!(T[t] > 0.0) || !std::isfinite(T[t])) return fail(h, RFIM_EINVAL, "temperatures must be positive and finite");
         if (t > 0 && !(T[t] > T[t - 1])) return fail(h, RFIM_EINVAL, "temperatures must be strictly ascending");
     }
-    h->n = n; h->v.n = n;
+    h->n = n; h->v.n = n; h->v.n_it = iterated(h);
     std::vector<int32_t> t2r((size_t)h->D * h->R, -1);
     for (int d = 0; d < h->D; ++d)
         for (int t = 0; t < n; ++t) { h->T[(size_t)d * h->R + t] = T[t]; t2r[(size_t)d * h->R + t] = t; }
@@ -851,6 +901,7 @@ int rfim_pt_adapt_temperatures(rfim_pt* h, int64_t trial_sweeps) {
             } else if (p.keep_of[j] >= 0) {
                 slot = t2r[(size_t)d * R + p.keep_of[j]];
             } else {
+                if (h->shard) return fail(h, RFIM_EINVAL, "replica shard: adaptation that inserts replicas would copy lattices between ranks (use n = R)");
                 slot = next_slot++;
                 const int src = t2r[(size_t)d * R + p.copy_of[j]];
                 const size_t lat = (size_t)h->N / (h->packing == 1 ? 8 : 1);      // bytes per lattice
@@ -861,7 +912,7 @@ int rfim_pt_adapt_temperatures(rfim_pt* h, int64_t trial_sweeps) {
             h->T[(size_t)d * R + j] = p.T[j];
         }
     }
-    h->n = n_new; h->v.n = n_new;
+    h->n = n_new; h->v.n = n_new; h->v.n_it = iterated(h);
     if ((rc = upload_permutation(h, new_t2r))) return rc;
     if ((rc = upload_tables(h))) return rc;
     if ((rc = reset_statistics(h))) return rc;
@@ -905,8 +956,9 @@ int rfim_pt_get_spins_slot(rfim_pt* h, int d, int slot, int8_t* out) {
     int rc = check_member(h, d);
     if (rc) return rc;
     if (slot < 0 || slot >= h->R || !out) return fail(h, RFIM_EINVAL, "bad slot or null buffer");
+    if (slot < h->slot0 || slot >= h->slot0 + h->Rs) return fail(h, RFIM_EINVAL, "replica shard: this rank does not store that slot");
     if ((rc = ensure_stage(h, (size_t)h->N))) return rc;
-    k_export_spins<<<grid_for(h->N, 1), 256, 0, h->stream>>>(h->v, d * h->R + slot, h->stage);
+    k_export_spins<<<grid_for(h->N, 1), 256, 0, h->stream>>>(h->v, d * h->Rs + slot - h->slot0, h->stage);
     h->launches += 1;
     CU(cudaGetLastError());
     CU(cudaMemcpyAsync(out, h->stage, (size_t)h->N, cudaMemcpyDeviceToHost, h->stream));
@@ -933,9 +985,10 @@ int rfim_pt_set_spins_slot(rfim_pt* h, int d, int slot, const int8_t* in) {
     if (slot < 0 || slot >= h->R || !in) return fail(h, RFIM_EINVAL, "bad slot or null buffer");
     for (long long i = 0; i < h->N; ++i)
         if (in[i] != 1 && in[i] != -1) return fail(h, RFIM_EINVAL, "spins must be +1 or -1");
+    if (slot < h->slot0 || slot >= h->slot0 + h->Rs) return fail(h, RFIM_EINVAL, "replica shard: this rank does not store that slot");
     if ((rc = ensure_stage(h, (size_t)h->N))) return rc;
     CU(cudaMemcpyAsync(h->stage, in, (size_t)h->N, cudaMemcpyHostToDevice, h->stream));
-    k_import_spins<<<grid_for(h->N, 1), 256, 0, h->stream>>>(h->v, d * h->R + slot, h->stage);
+    k_import_spins<<<grid_for(h->N, 1), 256, 0, h->stream>>>(h->v, d * h->Rs + slot - h->slot0, h->stage);
     h->launches += 1;
     CU(cudaGetLastError());
     CU(cudaStreamSynchronize(h->stream));
@@ -944,7 +997,7 @@ int rfim_pt_set_spins_slot(rfim_pt* h, int d, int slot, const int8_t* in) {
 
 int rfim_pt_get_spins_all(rfim_pt* h, int8_t* out) {
     if (!h || !out) return RFIM_EINVAL;
-    const int DR = h->D * h->R;
+    const int DR = h->D * h->Rs;          // every stored lattice (a replica shard: its slot window)
     int rc = ensure_stage(h, (size_t)DR * h->N);
     if (rc) return rc;
     k_export_spins<<<grid_for(h->N, DR), 256, 0, h->stream>>>(h->v, 0, h->stage);
@@ -957,7 +1010,7 @@ int rfim_pt_get_spins_all(rfim_pt* h, int8_t* out) {
 
 int rfim_pt_set_spins_all(rfim_pt* h, const int8_t* in) {
     if (!h || !in) return RFIM_EINVAL;
-    const int DR = h->D * h->R;
+    const int DR = h->D * h->Rs;
     int rc = ensure_stage(h, (size_t)DR * h->N);
     if (rc) return rc;
     CU(cudaMemcpyAsync(h->stage, in, (size_t)DR * h->N, cudaMemcpyHostToDevice, h->stream));

@@ -2,7 +2,7 @@
 // one SM for a whole launch (all phases of an exchange period).  DESIGN.md section 6.
 //
 // Decomposition.  The D*n active replicas (by temperature rank) are stacked into one list of
-// D*n*L planes (plane P = (d*n + t)*L + z).  CTA b of a cooperative launch owns the contiguous run
+// D*n*L planes (plane P = (d*n + t)*L + z; a replica shard lists its stored slots instead of the ranks).  CTA b of a cooperative launch owns the contiguous run
 // [start_b, start_b + count_b) with counts differing by at most one, so 148 SMs hold 55 or 56 planes
 // each at L = 64, R = 128: no replica-granular imbalance (128 replicas do not divide over 148 SMs).
 // A run is loaded once, swept 2*sweeps phases (colour 0, colour 1, ...) in place, and stored once.
@@ -488,9 +488,12 @@ __global__ void __launch_bounds__(THREADS, 1) k_sweep_res(const View v, const Re
         s_plane[p] = pi;
     }
     for (int r = tid; r < nrep; r += THREADS) {
-        const int dt = dt0 + r, d = rp.d0 + dt / v.n, t = dt % v.n;
+        const int dt = dt0 + r, d = rp.d0 + dt / v.n_it, q = dt % v.n_it;
         ResRep rr;
-        rr.d = d; rr.tr = d * v.R + t; rr.slot = v.t2r[rr.tr]; rr.ds = d * v.R + rr.slot;
+        rr.d = d;
+        if (v.shard) { rr.slot = v.slot0 + q; rr.tr = d * v.R + v.r2t[d * v.R + rr.slot]; }      // visit stored slots
+        else { rr.tr = d * v.R + q; rr.slot = v.t2r[rr.tr]; }                                  // visit ranks
+        rr.ds = d * v.Rs + rr.slot - v.slot0;
         rr.band = KIND == 0 ? 0.f : v.band[rr.tr];
         rr.never = KIND == 0 ? v.never[rr.tr] : 0u;
         rr.beta = v.beta[rr.tr];
@@ -502,7 +505,8 @@ __global__ void __launch_bounds__(THREADS, 1) k_sweep_res(const View v, const Re
     // acceptance tables, 8-byte entries at byte offset SP*n1 + 8*SP*s (+ 16*SP*hb): Gaussian {x, y}, bimodal {thr-1, never}
     for (int i = tid; i < nrep * 32; i += THREADS) {
         const int r = i >> 5, idx = i & 31;
-        const int dt = dt0 + r, d = rp.d0 + dt / v.n, t = dt % v.n, tr = d * v.R + t;
+        const int dt = dt0 + r, d = rp.d0 + dt / v.n_it, q = dt % v.n_it;
+        const int tr = d * v.R + (v.shard ? v.r2t[d * v.R + v.slot0 + q] : q);
         uint2 ent = make_uint2(0u, 0u);
         if (KIND == 0) {
             ent.x = v.etab[(long long)tr * 32 + idx];
@@ -668,7 +672,7 @@ __global__ void __launch_bounds__(THREADS, 1) k_sweep_res(const View v, const Re
         }
         if (rp.measure)
             for (int r = tid; r < nrep * 3; r += THREADS)
-                atomicAdd(reinterpret_cast<unsigned long long*>(v.acc + (long long)s_rep[r / 3].ds * 3 + r % 3), (unsigned long long)s_acc[r]);
+                atomicAdd(reinterpret_cast<unsigned long long*>(v.acc + (long long)(s_rep[r / 3].d * v.R + s_rep[r / 3].slot) * 3 + r % 3), (unsigned long long)s_acc[r]);
     }
     if (rp.exchange) {
         // the CTA that arrives last has every replica's sums in View::acc (integer atomics at L2): it runs the exchange step

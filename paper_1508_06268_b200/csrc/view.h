@@ -37,6 +37,10 @@ struct View {
     unsigned long long* diag;      // [4], see rfim_pt_get_diagnostics
     double J, hs;                  // hs = h (bimodal) or h * 2^-20 (Gaussian)
     int packed;                    // != 0: `spins` holds one BIT per spin (bit j & 7 of byte j >> 3, same index j as the byte layout)
+    // Replica sharding: this handle STORES the slots [slot0, slot0 + Rs) of every member (all R of
+    // them when shard == 0) and a sweep visits n_it replicas: every rank t < n (shard == 0) or the active stored slots
+    // slot0 .. slot0 + n_it - 1 (shard != 0).  t2r, r2t, tables, acc, series stay global (indexed by rank / slot < R).
+    int shard, slot0, Rs, n_it;
 };
 
 }  // namespace rfim

@@ -1,8 +1,13 @@
-"""Rank sharding of the benchmark / batch drivers: independent disorder realisations per rank.
+"""Rank sharding.  No method arithmetic lives here.  One process per GPU.
 
-No method arithmetic lives here.  One process per GPU; rank r of W takes the realisations whose seeds are
-`rank_seeds(base_seeds, r)`; there is no data-path collective, only the reduction of timings (max over ranks)
-and, for drivers that want them, a gather of per-realisation observables.
+Two ways to use several GPUs:
+  * independent disorder realisations per rank: rank r of W takes the realisations whose seeds are
+    `rank_seeds(base_seeds, r)`; no data-path collective, only the reduction of timings (max over ranks) and, for
+    drivers that want them, a gather of per-realisation observables;
+  * ONE realisation, its R replica slots dealt to the ranks in contiguous windows (Eq. 6:
+    m = ceil(M/D) replicas per GPU): `replica_window` gives rank r's window and `make_terms_gather` builds the one
+    collective of the path, the all-gather of 24 bytes of integer energy terms per slot before every exchange step,
+    after which every rank takes the same exchange decisions (lattices never move).
 """
 from typing import Sequence
 
@@ -35,3 +40,43 @@ def gather_by_rank(x: torch.Tensor):
     out = [torch.empty_like(x) for _ in range(dist.get_world_size())]
     dist.all_gather(out, x)
     return out
+
+
+def replica_window(R: int, world: int, rank: int):
+    """(slot0, nslots) of rank `rank`: contiguous windows of m = ceil(R / world) slots (Eq. 6).  The last
+    windows may reach past R (padding, the paper's M' = D * m): those slots are never active."""
+    m = -(-int(R) // int(world))
+    if (world - 1) * m >= R:
+        raise ValueError(f"{world} ranks of {m} slots leave a rank without any of the {R} slots: use fewer ranks")
+    return rank * m, m
+
+
+def all_gather_rows(terms: torch.Tensor, rank: int, world: int, group=None):
+    """In-place all-gather of a [world * m, 3] int64 array whose rows [rank*m, (rank+1)*m) are valid on this rank.
+    Works on any device / backend (NCCL on CUDA tensors, gloo on CPU tensors); identity for world == 1."""
+    assert terms.dim() == 2 and terms.shape[0] % world == 0
+    if world == 1:
+        return terms
+    m = terms.shape[0] // world
+    mine = terms[rank * m:(rank + 1) * m].clone()          # the send buffer must not alias the receive buffer
+    flat = terms.view(-1)
+    dist.all_gather_into_tensor(flat, mine.view(-1), group=group)
+    return terms
+
+
+class _DevicePtr:
+    """Expose a raw device pointer to torch through __cuda_array_interface__ (no copy, no ownership)."""
+
+    def __init__(self, ptr: int, nbytes: int):
+        self.__cuda_array_interface__ = {"shape": (nbytes // 8,), "typestr": "<i8", "data": (int(ptr), False), "version": 3}
+
+
+def make_terms_gather(rank: int, world: int, group=None):
+    """The function to hand to RfimPT.set_gather: wraps the library's energy-term array (device memory the library
+    owns) in a tensor and all-gathers it in place over torch.distributed.  The handle must run on torch's current
+    stream (the binding's default), which is what orders the collective against the library's kernels."""
+    def gather(terms_ptr, local_offset, local_bytes, total_bytes, stream_ptr):
+        t = torch.as_tensor(_DevicePtr(terms_ptr, total_bytes), device="cuda").view(-1, 3)
+        assert local_offset == rank * local_bytes and total_bytes == world * local_bytes, "windows must be equal and ordered by rank"
+        all_gather_rows(t, rank, world, group)
+    return gather

@@ -78,3 +78,60 @@ def test_single_process_identities():
     assert sharding.max_over_ranks([1.5, 2.5]) == [1.5, 2.5]
     x = torch.arange(3)
     assert len(sharding.gather_by_rank(x)) == 1
+
+
+# ---- replica distribution: windows of slots per rank + the all-gather of energy terms -----------
+SH_L, SH_R, SH_K = 4, 6, 3
+
+
+def _shard_worker(rank, world, port, q):
+    """Each rank owns a window of the R replica slots.  The oracle stands in for the device library: every rank runs the
+    whole chain (cheap at this size) but only CONTRIBUTES the energy terms of its own window; after the all-gather every
+    rank must hold the full array and must take the same exchange decisions as a serial run fed with it."""
+    os.environ["MASTER_ADDR"] = "127.0.0.1"
+    os.environ["MASTER_PORT"] = str(port)
+    dist.init_process_group("gloo", rank=rank, world_size=world)
+    try:
+        import oracle
+        slot0, m = sharding.replica_window(SH_R, world, rank)
+        o = oracle.Oracle(SH_L, SH_R, 1.0, 1.0, BIMODAL, 99)
+        o.set_temperatures(linear_ladder(1.0, 4.0, SH_R))
+        rows_seen = []
+        for step in range(4):
+            o.sweep(SH_K, 0)                                             # sweeps need no communication
+            eb, ef, ms = o.get_energy_terms()                            # by rank; bring to slot order
+            perm = o.get_permutation()
+            full = np.zeros((world * m, 3), dtype=np.int64)
+            full[perm, 0], full[perm, 1], full[perm, 2] = eb, ef, ms
+            mine = torch.zeros((world * m, 3), dtype=torch.int64)
+            mine[slot0:slot0 + m] = torch.from_numpy(full[slot0:slot0 + m])   # only my window is valid before the gather
+            sharding.all_gather_rows(mine, rank, world)
+            assert np.array_equal(mine.numpy()[:SH_R], full[:SH_R]), (rank, step)
+            rows_seen.append(mine.numpy().copy())
+        dist.barrier()
+        if rank == 0:
+            q.put(rows_seen)
+    finally:
+        dist.destroy_process_group()
+
+
+def test_replica_windows_and_terms_all_gather():
+    assert sharding.replica_window(128, 8, 3) == (48, 16)
+    assert sharding.replica_window(5, 3, 2) == (4, 2)                     # last window reaches past R (padding)
+    try:
+        sharding.replica_window(6, 4, 0)
+        raise AssertionError("a rank without slots must be refused")
+    except ValueError:
+        pass
+    world = 2
+    ctx = mp.get_context("spawn")
+    q = ctx.Queue()
+    port = _free_port()
+    procs = [ctx.Process(target=_shard_worker, args=(r, world, port, q)) for r in range(world)]
+    for p in procs:
+        p.start()
+    rows = q.get(timeout=120)
+    for p in procs:
+        p.join(timeout=60)
+        assert p.exitcode == 0
+    assert len(rows) == 4 and all(r.shape == (6, 3) for r in rows)

@@ -1,0 +1,171 @@
+"""-m gpu: replica distribution (include/rfim_pt.h "replica distribution over several GPUs").
+
+The R slots of one realisation are dealt to G shard handles; each sweeps only the slots it stores, and before every
+exchange step the 24-byte energy terms per slot are all-gathered so that every shard takes the same exchange decisions.
+Only one GPU is available to the tests, so the G "ranks" are G handles of one process, each driven by its own host
+thread and its own CUDA stream (no kernel waits for another kernel: the host threads meet at a barrier inside the
+gather function and copy one another's rows).  A sharded run must equal the oracle -- hence the single-handle run --
+bit for bit: spins of every slot, permutation, energy terms, exchange counters, time series.
+"""
+import threading
+
+import numpy as np
+import pytest
+import torch
+
+from paper_1508_06268_b200.sharding import _DevicePtr, replica_window
+from paper_1508_06268_b200.workloads import geometric_ladder
+
+pytestmark = pytest.mark.gpu
+
+BIMODAL, GAUSSIAN = 0, 1
+_KEEP = []
+
+
+class LoopbackGather:
+    """All-gather among G handles of one process: every participant publishes its rows, waits for the others at a host
+    barrier, then copies their rows into its own array (device-to-device, on its own stream)."""
+
+    def __init__(self, world):
+        self.world = world
+        self.barrier = threading.Barrier(world)
+        self.rows = [None] * world
+
+    def make(self, rank):
+        def gather(terms_ptr, local_offset, local_bytes, total_bytes, stream_ptr):
+            t = torch.as_tensor(_DevicePtr(terms_ptr, total_bytes), device="cuda").view(self.world, -1)
+            torch.cuda.current_stream().synchronize()           # my rows are final
+            self.rows[rank] = t[rank]
+            self.barrier.wait()
+            for r in range(self.world):
+                if r != rank:
+                    t[r].copy_(self.rows[r])
+            torch.cuda.current_stream().synchronize()
+            self.barrier.wait()                                  # nobody overwrites rows a peer still reads
+        return gather
+
+
+def _run_sharded(L, R, n, kind, h, seed, T, world, program, packing=8):
+    """program(handle) runs on every shard in its own thread; returns the shard handles."""
+    from paper_1508_06268_b200 import binding
+    lg = LoopbackGather(world)
+    shards, errors = [None] * world, []
+    streams = [torch.cuda.Stream() for _ in range(world)]
+    _KEEP.append(streams)                                        # the handles keep using these streams after the threads end
+
+    def worker(rank):
+        try:
+            with torch.cuda.stream(streams[rank]):
+                g = binding.RfimPT(L, R, 1.0, h, kind, seed=seed, shard=replica_window(R, world, rank))
+                g.set_gather(lg.make(rank))
+                if packing != 8:
+                    g.set_packing(packing)
+                g.set_temperatures(T)
+                shards[rank] = g
+                program(g)
+                g.synchronize()
+        except Exception as e:                                   # a dead thread would leave the others at the barrier
+            errors.append(e)
+            lg.barrier.abort()
+
+    threads = [threading.Thread(target=worker, args=(r,)) for r in range(world)]
+    for t in threads:
+        t.start()
+    for t in threads:
+        t.join(timeout=300)
+    assert not errors, errors
+    return shards
+
+
+@pytest.mark.parametrize("L,R,n,world", [(32, 6, 6, 2), (32, 8, 7, 4), (64, 4, 4, 2), (32, 5, 5, 3)])
+@pytest.mark.parametrize("kind,h", [(BIMODAL, 2.0), (GAUSSIAN, 1.5)])
+def test_sharded_run_equals_oracle(L, R, n, world, kind, h):
+    import oracle
+    T = geometric_ladder(0.9, 5.0, n)
+    o = oracle.Oracle(L, R, 1.0, h, kind, 41)
+    o.set_temperatures(T)
+    calls = [(3, 0), (8, 2), (5, 5), (7, 3)]
+    for a, k in calls:
+        o.sweep(a, k)
+
+    def program(g):
+        for a, k in calls:
+            g.sweep(a, k)
+
+    shards = _run_sharded(L, R, n, kind, h, 41, T, world, program)
+    perm = o.get_permutation()
+    terms = o.get_energy_terms()
+    series = o.get_timeseries()
+    for rank, g in enumerate(shards):
+        slot0, m = replica_window(R, world, rank)
+        for slot in range(slot0, min(slot0 + m, n)):
+            assert np.array_equal(g.get_spins_slot(slot), o.get_spins_slot(slot)), (rank, slot)
+        assert np.array_equal(g.get_permutation(), perm), rank
+        assert g.get_counters() == o.get_counters()
+        for x, y in zip(g.get_exchange_counts(), o.get_exchange_counts()):
+            assert np.array_equal(x, y)
+        for x, y in zip(g.get_timeseries(), series):
+            assert np.array_equal(x, y)
+        assert g.diagnostics()["ulp_ambiguous"] == 0
+    # the energy getter gathers too: every rank must be inside it at the same time
+    got = [None] * world
+    lg = LoopbackGather(world)
+
+    def getter(rank):
+        shards[rank].set_gather(lg.make(rank))
+        got[rank] = shards[rank].get_energy_terms()
+
+    ts = [threading.Thread(target=getter, args=(r,)) for r in range(world)]
+    [t.start() for t in ts]
+    [t.join(timeout=120) for t in ts]
+    for rank in range(world):
+        for x, y in zip(got[rank], terms):
+            assert np.array_equal(x, y), rank
+    for g in shards:
+        g.close()
+
+
+def test_sharded_bit_packed_and_fixed_count_adaptation():
+    """shards with bit-packed storage; the fixed-count (rank-preserving) adaptation moves no lattice and works sharded."""
+    import oracle
+    L, R, world = 32, 6, 2
+    T = geometric_ladder(0.9, 5.0, R)
+    o = oracle.Oracle(L, R, 1.0, 1.5, GAUSSIAN, 77)
+    o.set_temperatures(T)
+    o.set_adapt_params(4, 2)
+    o.adapt_temperatures(40)
+    o.sweep(12, 4)
+
+    def program(g):
+        g.set_adapt_params(4, 2)
+        g.adapt_temperatures(40)
+        g.sweep(12, 4)
+
+    shards = _run_sharded(L, R, R, GAUSSIAN, 1.5, 77, T, world, program, packing=1)
+    for rank, g in enumerate(shards):
+        slot0, m = replica_window(R, world, rank)
+        assert np.array_equal(g.get_temperatures(), o.get_temperatures())
+        for slot in range(slot0, min(slot0 + m, R)):
+            assert np.array_equal(g.get_spins_slot(slot), o.get_spins_slot(slot)), (rank, slot)
+        assert np.array_equal(g.get_permutation(), o.get_permutation())
+        g.close()
+
+
+def test_shard_errors():
+    from paper_1508_06268_b200 import binding
+    with pytest.raises(binding.RfimPtError):
+        binding.RfimPT(32, 6, 1.0, 1.0, BIMODAL, seed=1, shard=(1, 3))     # window not aligned
+    with pytest.raises(binding.RfimPtError):
+        binding.RfimPT(32, 6, 1.0, 1.0, BIMODAL, seed=1, shard=(6, 3))     # window past R
+    g = binding.RfimPT(32, 6, 1.0, 1.0, BIMODAL, seed=1, shard=(3, 3))
+    g.set_temperatures(geometric_ladder(1.0, 4.0, 6))
+    with pytest.raises(binding.RfimPtError):
+        g.get_spins_slot(0)                                                # not stored here
+    with pytest.raises(binding.RfimPtError) as e:
+        g.sweep(2, 2)                                                      # exchange step without a gather function
+    assert e.value.code == binding.ESTATE
+    g.close()
+    g = binding.RfimPT(32, 6, 1.0, 1.0, BIMODAL, seed=1)
+    with pytest.raises(binding.RfimPtError):
+        g.set_gather(lambda *a: None)                                      # not a shard
+    g.close()
