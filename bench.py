@@ -36,6 +36,10 @@ def parse():
     ap.add_argument("--workload", default="cfg4")
     ap.add_argument("--variant", type=int, default=0, help="kernel variant (0 = automatic)")
     ap.add_argument("--packing", type=int, default=8)
+    ap.add_argument("--multi", default="realisations", choices=["realisations", "replicas"],
+                    help="N > 1: independent disorder realisations per rank (weak scaling, no collective; default) or the "
+                         "replicas of ONE realisation dealt to the ranks (PAPER.md:123-137; strong scaling, one all-gather "
+                         "of 24 B per replica per exchange step)")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-e2e", action="store_true")
     return ap.parse_args()
@@ -162,17 +166,24 @@ def main():
         torch.cuda.synchronize()
 
     k = wl.exchange_every
-    seeds = sharding.rank_seeds(wl.seeds, rank)    # each rank: its own disorder realisation(s)
-    if wl.D == 1:
-        g = binding.RfimPT(wl.L, wl.R, wl.J, wl.h, wl.field_kind, seed=seeds[0])
+    replicas = world > 1 and args.multi == "replicas" and wl.D == 1
+    if replicas:                                    # one realisation, its replica slots dealt to the ranks
+        g = binding.RfimPT(wl.L, wl.R, wl.J, wl.h, wl.field_kind, seed=wl.seeds[0], shard=sharding.replica_window(wl.R, world, rank))
+        g.set_gather(sharding.make_terms_gather(rank, world))
     else:
-        g = binding.RfimPT(wl.L, wl.R, wl.J, wl.h, wl.field_kind, seeds=seeds)
+        seeds = sharding.rank_seeds(wl.seeds, rank)    # each rank: its own disorder realisation(s)
+        if wl.D == 1:
+            g = binding.RfimPT(wl.L, wl.R, wl.J, wl.h, wl.field_kind, seed=seeds[0])
+        else:
+            g = binding.RfimPT(wl.L, wl.R, wl.J, wl.h, wl.field_kind, seeds=seeds)
     if args.packing != 8:
         g.set_packing(args.packing)
     if args.variant:
         g.set_kernel_variant(args.variant)
     g.set_temperatures(wl.temperatures())
-    attempts_per_step = float(wl.N) * wl.R * wl.D * k
+    attempts_per_step = float(wl.N) * wl.R * wl.D * k            # per rank (realisations) ...
+    if replicas:
+        attempts_per_step /= world                                  # ... or this rank's share of the one realisation
 
     flush = torch.empty(256 << 20, dtype=torch.uint8, device="cuda")   # > 126 MB L2
 
@@ -233,19 +244,20 @@ def main():
                 "whole_step_frac": (value / world) / bound}
 
     line = {"metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps, "warmup": max(args.warmup, 3),
-            "ms_per_step": total_ms / args.steps, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
+            "ms_per_step": total_ms / args.steps, "higher_is_better": True, "scaling": "strong" if replicas else "weak", "vs_baseline": None,
             "dtype": "u8" if args.packing == 8 else "u1", "data": "synthetic",
             "config": {"workload": f"{wl.name}: L={wl.L} R={wl.R} D={wl.D} {'Gaussian' if wl.field_kind else 'bimodal'} h={wl.h} "
                                    f"T {wl.ladder} [{wl.t_min},{wl.t_max}] exchange_every={k} seed={wl.seeds[0]}",
                        "step": f"{k} sweeps + energy reduction + 1 exchange step", "l2": "flushed between steps (256 MiB memset)",
                        "packing_bits": args.packing, "kernel_variant": args.variant,
-                       "parallelism": "1 GPU" if world == 1 else f"{world} independent realisations, one per GPU"},
+                       "parallelism": "1 GPU" if world == 1 else (f"replicas of one realisation over {world} GPUs, all-gather of energy terms per exchange step"
+                                                                     if replicas else f"{world} independent realisations, one per GPU")},
             "clocks": clocks, "gpu_launches": int(l1 - l0), "wall_s_timed_region": t_wall, "roofline": roofline}
 
     # end to end through the C ABI with HOST buffers: H2D of every lattice, the step, D2H of lattices + observables
     if not args.no_e2e:
         n_e2e = max(3, min(args.steps, 20))
-        host = torch.empty((wl.D, wl.R, wl.N), dtype=torch.int8).pin_memory().numpy()
+        host = torch.empty((wl.D, g.stored_slots, wl.N), dtype=torch.int8).pin_memory().numpy()
         g.get_spins_all(out=host)
         E = None
         for it in range(2 + n_e2e):
