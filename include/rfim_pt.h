@@ -160,6 +160,16 @@ int rfim_pt_get_energy_terms(rfim_pt* h, int d, int64_t* Eb, int64_t* Ef, int64_
 /* one row [rank] per exchange step since the last reset */
 int64_t rfim_pt_timeseries_steps(rfim_pt* h);
 int rfim_pt_get_timeseries(rfim_pt* h, int d, int64_t* Eb, int64_t* Ef, int64_t* Msum);
+/* thermal averages of the measurement series (one measurement per exchange step), per temperature
+ * rank, over the steps [skip, steps) recorded since the last set_temperatures / adapt call.
+ * rfim_pt_thermal_moments: out[n][5] = <e>, <e^2>, <|m|>, <m^2>, <m^4> of member d, e = E/N the energy per site,
+ * m = (1/V) sum_i s_i.  rfim_pt_thermal_observables: the observables of Eq. 11-13 averaged over the D disorder
+ * realisations of the handle, n values each (any pointer may be NULL): absM = [<|M|>] (Eq. 11),
+ * C = [N/T^2 (<e^2> - <e>^2)] (Eq. 12, each realisation with its own T), g = (3 - [<M^4>]/[<M^2>]^2)/2 (Eq. 13).
+ * Computed on the device from the integer series (fixed summation order: deterministic).  RFIM_ESTATE if no step has
+ * been recorded after `skip`.  Host arrays are caller-owned; the calls synchronise. */
+int rfim_pt_thermal_moments(rfim_pt* h, int d, int64_t skip, double* out);
+int rfim_pt_thermal_observables(rfim_pt* h, int64_t skip, double* absM, double* C, double* g);
 int rfim_pt_get_exchange_counts(rfim_pt* h, int d, uint64_t* attempted, uint64_t* accepted);
 /* device acceptance table entry as the 33-bit threshold of DESIGN.md S3 (bimodal only) */
 int rfim_pt_get_bimodal_threshold(rfim_pt* h, int d, int rank, int k, int b, uint64_t* thr);

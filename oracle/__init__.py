@@ -58,6 +58,7 @@ def lib():
             "oracle_site_threshold": (ctypes.c_uint64, [ctypes.c_void_p] + [ctypes.c_int] * 4),
             "oracle_bimodal_threshold": (ctypes.c_uint64, [ctypes.c_void_p] + [ctypes.c_int] * 3),
             "oracle_energy_from_terms": (ctypes.c_double, [ctypes.c_void_p, ctypes.c_int64, ctypes.c_int64]),
+            "oracle_thermal_moments": (ctypes.c_int, [ctypes.c_void_p, ctypes.c_int64, _dp]),
             "oracle_half_sweep": (ctypes.c_int, [ctypes.c_void_p, ctypes.c_int, ctypes.c_int, ctypes.c_uint64]),
             "oracle_exchange_step": (ctypes.c_int, [ctypes.c_void_p]),
             "oracle_last_error": (ctypes.c_char_p, [ctypes.c_void_p]),
@@ -171,6 +172,12 @@ class Oracle:
         assert f.size == self.N
         self._ck(lib().oracle_set_field(self._h, _ptr(f, _i32p)))
 
+    def thermal_moments(self, skip=0):
+        """[n][5]: <e>, <e^2>, <|m|>, <m^2>, <m^4> per temperature rank over measurement steps [skip, steps)."""
+        out = np.zeros((self.n, 5))
+        self._ck(lib().oracle_thermal_moments(self._h, int(skip), _ptr(out, _dp)))
+        return out
+
     def get_permutation(self):
         out = np.zeros(self.n, dtype=np.int32)
         self._ck(lib().oracle_get_permutation(self._h, _ptr(out, _i32p)))
@@ -230,3 +237,20 @@ class Oracle:
 
     def exchange_step(self):
         self._ck(lib().oracle_exchange_step(self._h))
+
+
+def thermal_observables(moments, T, N):
+    """PAPER.md:249-260, Eq. 11-13 from the thermal moments of D disorder realisations at the same n temperatures.
+
+    moments: [D][n][5] (Oracle.thermal_moments of each realisation), T: [D][n] or [n], N = L^3.
+    Returns ([<|M|>], [C], [g]) per temperature: [.] = plain mean over the realisations;
+    C_d = N / T^2 (<e^2> - <e>^2) per realisation (Eq. 12), g = (3 - [<M^4>] / [<M^2>]^2) / 2 (Eq. 13: the ratio is
+    taken of the disorder averages, "an average at the disorder realization level")."""
+    mom = np.asarray(moments, dtype=np.float64)
+    if mom.ndim == 2:
+        mom = mom[None]
+    T = np.broadcast_to(np.asarray(T, dtype=np.float64), mom.shape[:2])
+    absM = mom[:, :, 2].mean(axis=0)
+    C = ((N / (T * T)) * (mom[:, :, 1] - mom[:, :, 0] * mom[:, :, 0])).mean(axis=0)
+    g = 0.5 * (3.0 - mom[:, :, 4].mean(axis=0) / (mom[:, :, 3].mean(axis=0) ** 2))
+    return absM, C, g

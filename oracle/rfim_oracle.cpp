@@ -18,6 +18,7 @@
 //   temperature swap      two index arrays replica<->temperature          PAPER.md:131-137 (reading G2)
 //   adaptation            lowest-rate intervals get a midpoint T          PAPER.md:147-153 (readings G5,G6,G10)
 //   magnetisation         |1/V sum s_i|                                    PAPER.md:251 (Eq. 11)
+//   specific heat, Binder C = L^3/T^2 (<e^2>-<e>^2), g = (3 - [<M^4>]/[<M^2>]^2)/2  PAPER.md:253-260 (Eq. 12-13)
 // What the paper is silent on and north_star (BASELINE.json) fixes: Philox4x32-10
 // random numbers keyed on (seed, replica, sweep, site), and the acceptance
 // thresholds floor(min(1, exp(-dE/T)) * 2^32) compared against one 32-bit word.
@@ -564,6 +565,29 @@ uint64_t oracle_bimodal_threshold(void* p, int rank, int k, int b) {
 double oracle_energy_from_terms(void* p, int64_t Eb, int64_t Ef) {
     Measurement m{Eb, Ef, 0};
     return ((Oracle*)p)->energy_of(m);
+}
+// Thermal moments of the measurement series (one measurement per parallel-tempering step), per temperature
+// rank, over the steps [skip, steps): out[t][0..4] = <e>, <e^2>, <|m|>, <m^2>, <m^4> with e = E/N the energy per site
+// ("E is the average energy per site") and m = (1/V) sum_i s_i (Eq. 11).  Plain running sums
+// in step order.  The observables of Eq. 11-13 follow from these (oracle/__init__.py: thermal_observables).
+int oracle_thermal_moments(void* p, int64_t skip, double* out) {
+    Oracle* o = (Oracle*)p;
+    const int64_t steps = o->series_steps;
+    if (skip < 0 || skip >= steps || !out) return -1;
+    const int n = o->n;
+    const double cnt = (double)(steps - skip);
+    for (int t = 0; t < n; ++t) {
+        double se = 0, se2 = 0, sa = 0, sm2 = 0, sm4 = 0;
+        for (int64_t q = skip; q < steps; ++q) {
+            const Measurement& ms = o->series[(size_t)q * n + t];
+            const double e = o->energy_of(ms) / (double)o->N;
+            const double m = (double)ms.Msum / (double)o->N;
+            se += e; se2 += e * e; sa += std::fabs(m); sm2 += m * m; sm4 += (m * m) * (m * m);
+        }
+        out[5 * t + 0] = se / cnt; out[5 * t + 1] = se2 / cnt; out[5 * t + 2] = sa / cnt;
+        out[5 * t + 3] = sm2 / cnt; out[5 * t + 4] = sm4 / cnt;
+    }
+    return 0;
 }
 // run exactly one half-sweep / one exchange step (for invariants checked between them)
 int oracle_half_sweep(void* p, int slot, int colour, uint64_t sweep_index) {

@@ -69,6 +69,8 @@ SIGNATURES = {
     "rfim_pt_get_energy_terms": (ctypes.c_int, [_vp, ctypes.c_int, _i64p, _i64p, _i64p]),
     "rfim_pt_timeseries_steps": (ctypes.c_int64, [_vp]),
     "rfim_pt_get_timeseries": (ctypes.c_int, [_vp, ctypes.c_int, _i64p, _i64p, _i64p]),
+    "rfim_pt_thermal_moments": (ctypes.c_int, [_vp, ctypes.c_int, ctypes.c_int64, _dp]),
+    "rfim_pt_thermal_observables": (ctypes.c_int, [_vp, ctypes.c_int64, _dp, _dp, _dp]),
     "rfim_pt_get_exchange_counts": (ctypes.c_int, [_vp, ctypes.c_int, _u64p, _u64p]),
     "rfim_pt_get_bimodal_threshold": (ctypes.c_int, [_vp, ctypes.c_int, ctypes.c_int, ctypes.c_int, ctypes.c_int, _u64p]),
     "rfim_pt_get_diagnostics": (ctypes.c_int, [_vp, _u64p]),
@@ -290,6 +292,17 @@ class RfimPT:
         t2r = np.ascontiguousarray(t2r, dtype=np.int32)
         assert t2r.size == self.n
         self._ck(load().rfim_pt_set_permutation(self._h, d, _p(t2r, _i32p)))
+
+    def thermal_moments(self, skip=0, d=0):
+        out = np.zeros((self.n, 5))
+        self._ck(load().rfim_pt_thermal_moments(self._h, d, int(skip), _p(out, _dp)))
+        return out
+
+    def thermal_observables(self, skip=0):
+        n = self.n
+        absM, C, g = np.zeros(n), np.zeros(n), np.zeros(n)
+        self._ck(load().rfim_pt_thermal_observables(self._h, int(skip), _p(absM, _dp), _p(C, _dp), _p(g, _dp)))
+        return absM, C, g
 
     def get_temperatures(self, d=0):
         out = np.zeros(self.n)

@@ -324,4 +324,30 @@ __global__ void k_exchange(View v, uint32_t xstep, long long row, int record) {
     exchange_member(v, (int)blockIdx.x, xstep, row, record);
 }
 
+// ---- thermal moments of the measurement series (Eq. 11-13 are built from these on the host) ------
+// One CTA per (member d, rank t): out[(d*n + t)*5 + 0..4] = <e>, <e^2>, <|m|>, <m^2>, <m^4> over steps [skip, steps), with
+// e = E/N per site (E as in DESIGN.md S5) and m = Msum/N.  Each thread sums a strided subset in step order, then a fixed
+// shared-memory tree combines the 256 partial sums: deterministic, and within a few ulp of a sequential sum.
+__global__ void k_thermal_moments(View v, long long skip, long long steps, double* __restrict__ out) {
+    const int d = blockIdx.x / v.n, t = blockIdx.x % v.n;
+    __shared__ double part[5][256];
+    double a[5] = {0, 0, 0, 0, 0};
+    const double invN = 1.0 / (double)v.N;
+    for (long long q = skip + threadIdx.x; q < steps; q += blockDim.x) {
+        const long long* s = v.series + ((q * v.D + d) * v.R + t) * 3;
+        const double E = __dsub_rn(__dmul_rn(-v.J, (double)s[0]), __dmul_rn(v.hs, (double)s[1]));
+        const double e = E / (double)v.N, m = (double)s[2] / (double)v.N;
+        (void)invN;
+        a[0] += e; a[1] += e * e; a[2] += fabs(m); a[3] += m * m; a[4] += (m * m) * (m * m);
+    }
+    for (int j = 0; j < 5; ++j) part[j][threadIdx.x] = a[j];
+    __syncthreads();
+    for (int w = 128; w > 0; w >>= 1) {
+        if ((int)threadIdx.x < w)
+            for (int j = 0; j < 5; ++j) part[j][threadIdx.x] += part[j][threadIdx.x + w];
+        __syncthreads();
+    }
+    if (threadIdx.x < 5) out[(long long)blockIdx.x * 5 + threadIdx.x] = part[threadIdx.x][0] / (double)(steps - skip);
+}
+
 }  // namespace rfim

@@ -1123,6 +1123,60 @@ int rfim_pt_get_timeseries(rfim_pt* h, int d, int64_t* Eb, int64_t* Ef, int64_t*
     return RFIM_OK;
 }
 
+namespace {
+// [D][n][5] thermal moments of the series over steps [skip, steps), computed on the device
+int thermal_moments_all(rfim_pt* h, int64_t skip, std::vector<double>& mom) {
+    if (!h->have_T) return fail(h, RFIM_ESTATE, "temperatures not set");
+    if (skip < 0 || skip >= h->series_steps) return fail(h, RFIM_ESTATE, "no measurement steps after `skip` (sweep with exchange_every > 0 first)");
+    const size_t cnt = (size_t)h->D * h->n * 5;
+    double* dev = nullptr;
+    int rc = alloc_into(h, &dev, cnt);
+    if (rc) return rc;
+    k_thermal_moments<<<h->D * h->n, 256, 0, h->stream>>>(h->v, (long long)skip, h->series_steps, dev);
+    h->launches += 1;
+    mom.assign(cnt, 0.0);
+    cudaError_t e1 = cudaGetLastError();
+    cudaError_t e2 = cudaMemcpyAsync(mom.data(), dev, cnt * 8, cudaMemcpyDeviceToHost, h->stream);
+    cudaError_t e3 = cudaStreamSynchronize(h->stream);
+    release(h, dev);
+    CU(e1); CU(e2); CU(e3);
+    return RFIM_OK;
+}
+}  // namespace
+
+int rfim_pt_thermal_moments(rfim_pt* h, int d, int64_t skip, double* out) {
+    int rc = check_member(h, d);
+    if (rc) return rc;
+    if (!out) return fail(h, RFIM_EINVAL, "null buffer");
+    std::vector<double> mom;
+    if ((rc = thermal_moments_all(h, skip, mom))) return rc;
+    std::memcpy(out, mom.data() + (size_t)d * h->n * 5, (size_t)h->n * 5 * 8);
+    return RFIM_OK;
+}
+
+int rfim_pt_thermal_observables(rfim_pt* h, int64_t skip, double* absM, double* C, double* g) {
+    if (!h) return RFIM_EINVAL;
+    std::vector<double> mom;
+    int rc = thermal_moments_all(h, skip, mom);
+    if (rc) return rc;
+    const int D = h->D, n = h->n;
+    for (int t = 0; t < n; ++t) {
+        double sa = 0, sc = 0, s2 = 0, s4 = 0;
+        for (int d = 0; d < D; ++d) {
+            const double* m = mom.data() + ((size_t)d * n + t) * 5;
+            const double T = h->T[(size_t)d * h->R + t];
+            sa += m[2];
+            sc += ((double)h->N / (T * T)) * (m[1] - m[0] * m[0]);      // Eq. 12 per realisation
+            s2 += m[3]; s4 += m[4];
+        }
+        const double m2 = s2 / D, m4 = s4 / D;
+        if (absM) absM[t] = sa / D;                                     // Eq. 11
+        if (C) C[t] = sc / D;
+        if (g) g[t] = 0.5 * (3.0 - m4 / (m2 * m2));                     // Eq. 13: ratio of the disorder averages
+    }
+    return RFIM_OK;
+}
+
 int rfim_pt_get_exchange_counts(rfim_pt* h, int d, uint64_t* attempted, uint64_t* accepted) {
     int rc = check_member(h, d);
     if (rc) return rc;

@@ -32,3 +32,12 @@ def exact_averages(J, hs, field, T):
     H, p = boltzmann(st, J, hs, field, T)
     m = st.sum(axis=1) / 8.0
     return float((p * H).sum()), float((p * np.abs(m)).sum())
+
+
+def exact_moments(J, hs, field, T):
+    """Exact <e>, <e^2>, <|m|>, <m^2>, <m^4> of the 2x2x2 lattice (e = H/8 per site, m = mean spin)."""
+    st = all_states()
+    H, p = boltzmann(st, J, hs, field, T)
+    e = H / 8.0
+    m = st.sum(axis=1) / 8.0
+    return np.array([(p * e).sum(), (p * e * e).sum(), (p * np.abs(m)).sum(), (p * m ** 2).sum(), (p * m ** 4).sum()])
