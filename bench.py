@@ -234,7 +234,12 @@ def main():
     hbm_bound = hbm_peak / bytes_per_attempt                                  # attempts/ns if HBM were the limit
     bound = min(philox_bound, hbm_bound)
     roofline = {"bound": "alu", "achieved": sweep_rate, "peak": bound, "unit": UNIT, "frac": sweep_rate / bound,
-                "traffic": None,
+                # DRAM bytes of one launch of the dominant kernel from the committed `ncu --set full` capture of this
+                # command at config 4 (profiles/r1_res_sweep_full.md: 35.2 MB read + 2.2 MB written; the write-back of the
+                # run is still in L2 when the kernel ends); algorithmic = every int8 spin read once and written once per launch
+                "traffic": 37.45e6 if (wl.name == "cfg4" and args.packing == 8 and world == 1) else None,
+                "traffic_unit": "bytes per launch (ncu dram__bytes_read.sum + dram__bytes_write.sum)",
+                "algorithmic_bytes_per_launch": 2.0 * wl.N * wl.R * wl.D / (8 if args.packing == 1 else 1),
                 "kernel": "sweep (both colours), timed alone with CUDA events over the same steps",
                 "philox_bound_measured": philox_bound, "hbm_bound": hbm_bound,
                 "hbm_peak_gbs": hbm_peak, "hbm_peak_source": "MEASURED_PEAKS.json" if peaks else "fallback 6650 GB/s",
