@@ -290,7 +290,10 @@ def main():
         v0, ms0, r_used = oracle_sample(wl, threads, r_s, k, 1, 0, wl.seeds[0])      # one step, to size the sample
         n_b = int(max(2, min(200, 12e3 / max(ms0, 1.0))))                            # about 12 s of oracle work
         v, ms_b, r_used = oracle_sample(wl, threads, r_s, k, n_b, 0, wl.seeds[0])
+        v1, ms1, r1 = oracle_sample(wl, 1, 4, k, 2, 0, wl.seeds[0])                   # and on ONE core
         line["cpu_baseline"] = {"value": v, "unit": UNIT, "cores": threads, "kind": "oracle",
+                                "single_core": {"value": v1, "unit": UNIT, "cores": 1,
+                                                "sample": f"{r1} of {wl.R} replicas x 2 steps of ({k} sweeps + 1 exchange step), L={wl.L}"},
                                 "sample": f"{r_used} of {wl.R} replicas x {n_b} steps of ({k} sweeps + 1 exchange step), L={wl.L} "
                                           f"({ms_b * n_b / 1e3:.1f} s wall, oracle as it stands, {threads} OpenMP threads over replicas)"}
     if rank == 0:

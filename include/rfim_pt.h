@@ -114,6 +114,9 @@ int rfim_pt_get_spins(rfim_pt* h, int temp_rank, int8_t* out);
 
 /* cuda_stream: a cudaStream_t (e.g. torch.cuda.current_stream().cuda_stream); NULL = default. */
 int rfim_pt_set_stream(rfim_pt* h, void* cuda_stream);
+/* waits for the handle's stream.  RFIM_ESTATE if a persistent sweep kernel gave up a dependency wait (it never hangs the
+ * GPU: after ~2^22 polls it sets a flag and runs on; the lattices are then invalid).  rfim_pt_observables and
+ * rfim_pt_get_diagnostics report the same condition. */
 int rfim_pt_synchronize(rfim_pt* h);
 /* Process-wide device allocator used by handles created afterwards.  alloc returns a device
  * pointer or NULL; both NULL restores cudaMalloc/cudaFree. */

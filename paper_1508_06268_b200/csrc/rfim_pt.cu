@@ -556,6 +556,16 @@ int do_sweeps(rfim_pt* h, int64_t n_sweeps, int k) {
 }
 
 // current integer terms of every active replica, by rank: out [D][n][3]; also returns t2r [D][R]
+// The persistent kernels give up a dependency wait after ~2^22 polls instead of hanging the GPU and set diag[0]:
+// every synchronising getter reports that as an error (the lattices are then invalid).
+int check_wait_flag(rfim_pt* h) {
+    unsigned long long flag = 0;
+    CU(cudaMemcpyAsync(&flag, h->v.diag, 8, cudaMemcpyDeviceToHost, h->stream));
+    CU(cudaStreamSynchronize(h->stream));
+    if (flag != 0) return fail(h, RFIM_ESTATE, "a dependency wait of a persistent sweep kernel timed out: results are invalid");
+    return RFIM_OK;
+}
+
 int measure_now(rfim_pt* h, std::vector<long long>& terms, std::vector<int32_t>& t2r) {
     const size_t DR = (size_t)h->D * h->R;
     CU(cudaMemsetAsync(h->v.acc, 0, (size_t)h->D * h->acc_rows * 24, h->stream));
@@ -778,8 +788,7 @@ int rfim_pt_set_stream(rfim_pt* h, void* s) {
 
 int rfim_pt_synchronize(rfim_pt* h) {
     if (!h) return RFIM_EINVAL;
-    CU(cudaStreamSynchronize(h->stream));
-    return RFIM_OK;
+    return check_wait_flag(h);
 }
 
 int rfim_pt_set_packing(rfim_pt* h, int bits) {
@@ -926,6 +935,7 @@ int rfim_pt_observables(rfim_pt* h, double* E, double* M, double* rate) {
     std::vector<long long> terms; std::vector<int32_t> t2r;
     int rc = measure_now(h, terms, t2r);
     if (rc) return rc;
+    if ((rc = check_wait_flag(h))) return rc;
     const int D = h->D, n = h->n, R = h->R;
     for (int d = 0; d < D; ++d)
         for (int t = 0; t < n; ++t) {
@@ -1207,7 +1217,7 @@ int rfim_pt_get_diagnostics(rfim_pt* h, uint64_t diag[4]) {
     unsigned long long d4[4];
     CU(cudaMemcpyAsync(d4, h->v.diag, 32, cudaMemcpyDeviceToHost, h->stream));
     CU(cudaStreamSynchronize(h->stream));
-    if (d4[0] != 0) return fail(h, RFIM_ESTATE, "a flow-kernel dependency wait timed out: results are invalid");
+    if (d4[0] != 0) return fail(h, RFIM_ESTATE, "a dependency wait of a persistent sweep kernel timed out: results are invalid");
     diag[0] = h->launches; diag[1] = d4[1]; diag[2] = d4[2]; diag[3] = d4[3];
     return RFIM_OK;
 }
