@@ -259,27 +259,35 @@ def main():
                                                                      if replicas else f"{world} independent realisations, one per GPU")},
             "clocks": clocks, "gpu_launches": int(l1 - l0), "wall_s_timed_region": t_wall, "roofline": roofline}
 
-    # end to end through the C ABI with HOST buffers: H2D of every lattice, the step, D2H of lattices + observables
+    # end to end through the C ABI with HOST buffers, every step: H2D of every lattice (the step's input state) from pinned
+    # memory, the step, D2H of every lattice and of the observables (the step's result).  Timed twice: with the bit-packed
+    # host format (1 bit per spin, rfim_pt_*_spins_all_bits: the headline e2e) and with the int8 +-1 format (8x the bytes).
     if not args.no_e2e:
         n_e2e = max(3, min(args.steps, 20))
-        host = torch.empty((wl.D, g.stored_slots, wl.N), dtype=torch.int8).pin_memory().numpy()
-        g.get_spins_all(out=host)
-        E = None
-        for it in range(2 + n_e2e):
-            if it == 2:
-                barrier()
-                t0 = time.perf_counter()
-            g.set_spins_all(host)
-            g.sweep(k, k)
-            g.get_spins_all(out=host)
-            E, M, _ = g.observables()
-        barrier()
-        dt = time.perf_counter() - t0
-        dt = sharding.max_over_ranks([dt], device="cuda")[0]
         obs_bytes = 2 * 8 * wl.D * wl.R
-        line["e2e"] = {"value": attempts_per_step * n_e2e * world / (dt * 1e9), "unit": UNIT,
-                       "h2d_bytes_per_step": int(host.nbytes), "d2h_bytes_per_step": int(host.nbytes + obs_bytes),
-                       "steps": n_e2e, "what": "rfim_pt_set_spins_all(host) + rfim_pt_sweep(k,k) + rfim_pt_get_spins_all(host) + rfim_pt_observables"}
+
+        def e2e_leg(host, put, get, what):
+            get(host)
+            for it in range(2 + n_e2e):
+                if it == 2:
+                    barrier()
+                    t0 = time.perf_counter()
+                put(host)
+                g.sweep(k, k)
+                get(host)
+                g.observables()
+            barrier()
+            dt = sharding.max_over_ranks([time.perf_counter() - t0], device="cuda")[0]
+            return {"value": attempts_per_step * n_e2e * world / (dt * 1e9), "unit": UNIT,
+                    "h2d_bytes_per_step": int(host.nbytes), "d2h_bytes_per_step": int(host.nbytes + obs_bytes),
+                    "steps": n_e2e, "what": what}
+
+        bits = torch.empty((wl.D, g.stored_slots, wl.N // 8), dtype=torch.uint8).pin_memory().numpy()
+        line["e2e"] = e2e_leg(bits, g.set_spins_all_bits, lambda h_: g.get_spins_all_bits(out=h_),
+                              "rfim_pt_set_spins_all_bits(host) + rfim_pt_sweep(k,k) + rfim_pt_get_spins_all_bits(host) + rfim_pt_observables")
+        host = torch.empty((wl.D, g.stored_slots, wl.N), dtype=torch.int8).pin_memory().numpy()
+        line["e2e_int8"] = e2e_leg(host, g.set_spins_all, lambda h_: g.get_spins_all(out=h_),
+                                   "rfim_pt_set_spins_all(host) + rfim_pt_sweep(k,k) + rfim_pt_get_spins_all(host) + rfim_pt_observables")
 
     d = g.diagnostics()
     line["diagnostics"] = d

@@ -150,6 +150,12 @@ int rfim_pt_set_spins_slot(rfim_pt* h, int d, int slot, const int8_t* in);
 /* all D*R slots at once, [d][slot][L^3]; the host buffers of the end-to-end benchmark */
 int rfim_pt_get_spins_all(rfim_pt* h, int8_t* out);
 int rfim_pt_set_spins_all(rfim_pt* h, const int8_t* in);
+/* the same with bit-packed HOST buffers (checkpoint format, an eighth of the PCIe traffic): [d][slot][L^3 / 8] bytes,
+ * bit (i & 7) of byte (i >> 3) = 1 iff s_i = +1, i = x + L (y + L z).  Independent of the device storage mode
+ * (rfim_pt_set_packing).  get synchronises; set is asynchronous on the handle's stream (`in` must stay valid and, for
+ * true asynchrony, pinned, until the stream has consumed it). */
+int rfim_pt_get_spins_all_bits(rfim_pt* h, uint8_t* out);
+int rfim_pt_set_spins_all_bits(rfim_pt* h, const uint8_t* in);
 /* field of member d in natural site order: bimodal +-1, Gaussian g_i in units of 2^-20 */
 int rfim_pt_get_field(rfim_pt* h, int d, int32_t* out);
 int rfim_pt_set_field(rfim_pt* h, int d, const int32_t* in);

@@ -59,6 +59,8 @@ SIGNATURES = {
     "rfim_pt_set_spins_slot": (ctypes.c_int, [_vp, ctypes.c_int, ctypes.c_int, _i8p]),
     "rfim_pt_get_spins_all": (ctypes.c_int, [_vp, _i8p]),
     "rfim_pt_set_spins_all": (ctypes.c_int, [_vp, _i8p]),
+    "rfim_pt_get_spins_all_bits": (ctypes.c_int, [_vp, ctypes.POINTER(ctypes.c_uint8)]),
+    "rfim_pt_set_spins_all_bits": (ctypes.c_int, [_vp, ctypes.POINTER(ctypes.c_uint8)]),
     "rfim_pt_get_field": (ctypes.c_int, [_vp, ctypes.c_int, _i32p]),
     "rfim_pt_set_field": (ctypes.c_int, [_vp, ctypes.c_int, _i32p]),
     "rfim_pt_get_permutation": (ctypes.c_int, [_vp, ctypes.c_int, _i32p]),
@@ -272,6 +274,17 @@ class RfimPT:
     def set_spins_all(self, s):
         assert s.dtype == np.int8 and s.size == self.D * self.stored_slots * self.N and s.flags.c_contiguous
         self._ck(load().rfim_pt_set_spins_all(self._h, _p(s, _i8p)))
+
+    def get_spins_all_bits(self, out=None):
+        """[D][stored slots][N/8] uint8: bit i&7 of byte i>>3 set iff s_i = +1 (natural site order)."""
+        if out is None:
+            out = np.zeros((self.D, self.stored_slots, self.N // 8), dtype=np.uint8)
+        self._ck(load().rfim_pt_get_spins_all_bits(self._h, _p(out, ctypes.POINTER(ctypes.c_uint8))))
+        return out
+
+    def set_spins_all_bits(self, bits):
+        assert bits.dtype == np.uint8 and bits.size == self.D * self.stored_slots * (self.N // 8) and bits.flags.c_contiguous
+        self._ck(load().rfim_pt_set_spins_all_bits(self._h, _p(bits, ctypes.POINTER(ctypes.c_uint8))))
 
     def get_field(self, d=0):
         out = np.zeros(self.N, dtype=np.int32)

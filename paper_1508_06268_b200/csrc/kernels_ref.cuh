@@ -210,6 +210,51 @@ __global__ void k_import_spins(View v, int first, const int8_t* __restrict__ in)
     }
 }
 
+// ---- the same with the HOST side bit-packed: bit (i & 7) of byte (i >> 3) of a lattice = 1 iff s_i = +1, i the natural
+// site index x + L (y + L z): an eighth of the PCIe traffic of the int8 interface.  N is a multiple of 8 (L is even).
+__global__ void k_export_bits(View v, int first, uint8_t* __restrict__ out) {
+    const int ds = first + blockIdx.y;
+    const int L = v.L, Lh = v.Lh;
+    const long long b0 = (long long)ds * 2 * v.Nh;
+    uint8_t* o = out + (long long)blockIdx.y * (v.N >> 3);
+    for (long long b = (long long)blockIdx.x * blockDim.x + threadIdx.x; b < (v.N >> 3); b += (long long)gridDim.x * blockDim.x) {
+        uint32_t bits = 0;
+        for (int t = 0; t < 8; ++t) {
+            const long long i = 8 * b + t;
+            const int x = (int)(i % L), y = (int)((i / L) % L), z = (int)(i / ((long long)L * L));
+            const int c = (x + y + z) & 1;
+            const long long j = b0 + (long long)c * v.Nh + (x >> 1) + (long long)Lh * (y + (long long)L * z);
+            const uint32_t up = v.packed ? (v.spins[j >> 3] >> (j & 7)) & 1u : v.spins[j];
+            bits |= up << t;
+        }
+        o[b] = (uint8_t)bits;
+    }
+}
+
+__global__ void k_import_bits(View v, int first, const uint8_t* __restrict__ in) {
+    const int ds = first + blockIdx.y;
+    const int L = v.L, Lh = v.Lh;
+    const uint8_t* src = in + (long long)blockIdx.y * (v.N >> 3);
+    // one thread per group of eight same-colour sites j0 .. j0+7 (one packed byte, or eight bytes of the byte layout)
+    for (long long b = (long long)blockIdx.x * blockDim.x + threadIdx.x; b < (v.N >> 3); b += (long long)gridDim.x * blockDim.x) {
+        const int c = (int)(b / (v.Nh >> 3));
+        const long long j0 = (b % (v.Nh >> 3)) * 8;
+        uint32_t bits = 0;
+        for (int t = 0; t < 8; ++t) {
+            const long long j = j0 + t;
+            const int xh = (int)(j % Lh), y = (int)((j / Lh) % L), z = (int)(j / ((long long)Lh * L));
+            const long long i = 2 * xh + ((y + z + c) & 1) + (long long)L * (y + (long long)L * z);
+            bits |= ((src[i >> 3] >> (i & 7)) & 1u) << t;
+        }
+        if (v.packed) {
+            v.spins[(long long)ds * (v.N >> 3) + b] = (uint8_t)bits;
+        } else {
+            uint8_t* dst = v.spins + (long long)ds * 2 * v.Nh + (long long)c * v.Nh + j0;
+            for (int t = 0; t < 8; ++t) dst[t] = (uint8_t)((bits >> t) & 1u);
+        }
+    }
+}
+
 // ---- whole-buffer conversion between the byte and the bit layout (same index j, eight spins per byte) ----------
 __global__ void k_pack_bits(const uint8_t* __restrict__ bytes, uint8_t* __restrict__ bits, long long nbits_bytes) {
     for (long long b = (long long)blockIdx.x * blockDim.x + threadIdx.x; b < nbits_bytes; b += (long long)gridDim.x * blockDim.x) {
@@ -289,6 +334,8 @@ __device__ __forceinline__ void exchange_member(const View& v, int d, uint32_t x
         long long* a = v.acc + (long long)(d * R + t2r[t]) * 3;
         const long long eb = __ldcg(a + 0), ef = __ldcg(a + 1), ms = __ldcg(a + 2);   // written by other CTAs' atomics: read at L2
         a[0] = 0; a[1] = 0; a[2] = 0;
+        long long* keep = v.last + (long long)(d * R + t2r[t]) * 3;
+        keep[0] = eb; keep[1] = ef; keep[2] = ms;
         if (record) {
             long long* s = v.series + ((row * v.D + d) * R + t) * 3;
             s[0] = eb; s[1] = ef; s[2] = ms;

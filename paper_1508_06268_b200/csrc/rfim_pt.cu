@@ -68,6 +68,7 @@ struct rfim_pt {
     uint8_t* fieldb_res = nullptr;
     uint32_t* res_prog = nullptr;     // [kResMaxGrid] progress words of the resident kernel
     uint32_t res_epoch = 0;
+    bool terms_fresh = false;         // View::last holds the energy terms of the CURRENT lattices (last call ended on an exchange step)
     int res_grid_limit = 0;           // 0 = one CTA per SM
     int sm_count = 0, smem_optin = 0;
     std::string err;
@@ -544,6 +545,7 @@ int do_sweeps(rfim_pt* h, int64_t n_sweeps, int k) {
         if (rc) return rc;
         h->sweep_g += (uint64_t)chunk;
         left -= chunk;
+        h->terms_fresh = step_after;                 // the lattices changed; an exchange step right now measures them
         if (step_after) {
             if (variant != 4 && (rc = launch_reduce(h))) return rc;
             if ((rc = gather_terms(h))) return rc;
@@ -568,16 +570,25 @@ int check_wait_flag(rfim_pt* h) {
 
 int measure_now(rfim_pt* h, std::vector<long long>& terms, std::vector<int32_t>& t2r) {
     const size_t DR = (size_t)h->D * h->R;
-    CU(cudaMemsetAsync(h->v.acc, 0, (size_t)h->D * h->acc_rows * 24, h->stream));
-    int rc = launch_reduce(h);
-    if (rc) return rc;
-    if ((rc = gather_terms(h))) return rc;
     std::vector<long long> acc(DR * 3);
     t2r.assign(DR, -1);
-    CU(cudaMemcpyAsync(acc.data(), h->v.acc, DR * 3 * 8, cudaMemcpyDeviceToHost, h->stream));
-    CU(cudaMemcpyAsync(t2r.data(), h->v.t2r, DR * 4, cudaMemcpyDeviceToHost, h->stream));
-    CU(cudaMemsetAsync(h->v.acc, 0, (size_t)h->D * h->acc_rows * 24, h->stream));
-    CU(cudaStreamSynchronize(h->stream));
+    int rc;
+    if (h->terms_fresh) {
+        // nothing has touched the lattices since the last exchange step measured them inside the sweep kernel: the terms
+        // it consumed (kept by slot; an exchange moves temperatures, not lattices) are the terms of the current state
+        CU(cudaMemcpyAsync(acc.data(), h->v.last, DR * 3 * 8, cudaMemcpyDeviceToHost, h->stream));
+        CU(cudaMemcpyAsync(t2r.data(), h->v.t2r, DR * 4, cudaMemcpyDeviceToHost, h->stream));
+        CU(cudaStreamSynchronize(h->stream));
+    } else {
+        CU(cudaMemsetAsync(h->v.acc, 0, (size_t)h->D * h->acc_rows * 24, h->stream));
+        rc = launch_reduce(h);
+        if (rc) return rc;
+        if ((rc = gather_terms(h))) return rc;
+        CU(cudaMemcpyAsync(acc.data(), h->v.acc, DR * 3 * 8, cudaMemcpyDeviceToHost, h->stream));
+        CU(cudaMemcpyAsync(t2r.data(), h->v.t2r, DR * 4, cudaMemcpyDeviceToHost, h->stream));
+        CU(cudaMemsetAsync(h->v.acc, 0, (size_t)h->D * h->acc_rows * 24, h->stream));
+        CU(cudaStreamSynchronize(h->stream));
+    }
     terms.assign((size_t)h->D * h->n * 3, 0);
     for (int d = 0; d < h->D; ++d)
         for (int t = 0; t < h->n; ++t) {
@@ -637,6 +648,7 @@ int create_impl(rfim_pt** out, int L, int R, double J, double hh, int kind, int 
     A(alloc_into(h, &v.r2t, DR));
     A(alloc_into(h, const_cast<uint32_t**>(&v.keys), (size_t)D * 2));
     A(alloc_into(h, &v.acc, (size_t)D * h->acc_rows * 3));
+    A(alloc_into(h, &v.last, DR * 3));
     A(alloc_into(h, &v.ework, DR));
     A(alloc_into(h, &v.att, DR));
     A(alloc_into(h, &v.accn, DR));
@@ -856,7 +868,7 @@ int rfim_pt_set_temperatures(rfim_pt* h, const double* T, int n) {
         if (!(T[t] > 0.0) || !std::isfinite(T[t])) return fail(h, RFIM_EINVAL, "temperatures must be positive and finite");
         if (t > 0 && !(T[t] > T[t - 1])) return fail(h, RFIM_EINVAL, "temperatures must be strictly ascending");
     }
-    h->n = n; h->v.n = n; h->v.n_it = iterated(h);
+    h->n = n; h->v.n = n; h->v.n_it = iterated(h); h->terms_fresh = false;
     std::vector<int32_t> t2r((size_t)h->D * h->R, -1);
     for (int d = 0; d < h->D; ++d)
         for (int t = 0; t < n; ++t) { h->T[(size_t)d * h->R + t] = T[t]; t2r[(size_t)d * h->R + t] = t; }
@@ -921,7 +933,7 @@ int rfim_pt_adapt_temperatures(rfim_pt* h, int64_t trial_sweeps) {
             h->T[(size_t)d * R + j] = p.T[j];
         }
     }
-    h->n = n_new; h->v.n = n_new; h->v.n_it = iterated(h);
+    h->n = n_new; h->v.n = n_new; h->v.n_it = iterated(h); h->terms_fresh = false;
     if ((rc = upload_permutation(h, new_t2r))) return rc;
     if ((rc = upload_tables(h))) return rc;
     if ((rc = reset_statistics(h))) return rc;
@@ -990,6 +1002,7 @@ int rfim_pt_get_spins_member(rfim_pt* h, int d, int temp_rank, int8_t* out) {
 int rfim_pt_get_spins(rfim_pt* h, int temp_rank, int8_t* out) { return rfim_pt_get_spins_member(h, 0, temp_rank, out); }
 
 int rfim_pt_set_spins_slot(rfim_pt* h, int d, int slot, const int8_t* in) {
+    if (h) h->terms_fresh = false;
     int rc = check_member(h, d);
     if (rc) return rc;
     if (slot < 0 || slot >= h->R || !in) return fail(h, RFIM_EINVAL, "bad slot or null buffer");
@@ -1019,12 +1032,41 @@ int rfim_pt_get_spins_all(rfim_pt* h, int8_t* out) {
 }
 
 int rfim_pt_set_spins_all(rfim_pt* h, const int8_t* in) {
+    if (h) h->terms_fresh = false;
     if (!h || !in) return RFIM_EINVAL;
     const int DR = h->D * h->Rs;
     int rc = ensure_stage(h, (size_t)DR * h->N);
     if (rc) return rc;
     CU(cudaMemcpyAsync(h->stage, in, (size_t)DR * h->N, cudaMemcpyHostToDevice, h->stream));
     k_import_spins<<<grid_for(h->N, DR), 256, 0, h->stream>>>(h->v, 0, h->stage);
+    h->launches += 1;
+    CU(cudaGetLastError());
+    return RFIM_OK;
+}
+
+int rfim_pt_get_spins_all_bits(rfim_pt* h, uint8_t* out) {
+    if (!h || !out) return RFIM_EINVAL;
+    const int DR = h->D * h->Rs;
+    const size_t bytes = (size_t)DR * (size_t)(h->N / 8);
+    int rc = ensure_stage(h, bytes);
+    if (rc) return rc;
+    k_export_bits<<<grid_for(h->N / 8, DR), 256, 0, h->stream>>>(h->v, 0, reinterpret_cast<uint8_t*>(h->stage));
+    h->launches += 1;
+    CU(cudaGetLastError());
+    CU(cudaMemcpyAsync(out, h->stage, bytes, cudaMemcpyDeviceToHost, h->stream));
+    CU(cudaStreamSynchronize(h->stream));
+    return RFIM_OK;
+}
+
+int rfim_pt_set_spins_all_bits(rfim_pt* h, const uint8_t* in) {
+    if (h) h->terms_fresh = false;
+    if (!h || !in) return RFIM_EINVAL;
+    const int DR = h->D * h->Rs;
+    const size_t bytes = (size_t)DR * (size_t)(h->N / 8);
+    int rc = ensure_stage(h, bytes);
+    if (rc) return rc;
+    CU(cudaMemcpyAsync(h->stage, in, bytes, cudaMemcpyHostToDevice, h->stream));
+    k_import_bits<<<grid_for(h->N / 8, DR), 256, 0, h->stream>>>(h->v, 0, reinterpret_cast<const uint8_t*>(h->stage));
     h->launches += 1;
     CU(cudaGetLastError());
     return RFIM_OK;
@@ -1039,6 +1081,7 @@ int rfim_pt_get_field(rfim_pt* h, int d, int32_t* out) {
 }
 
 int rfim_pt_set_field(rfim_pt* h, int d, const int32_t* in) {
+    if (h) h->terms_fresh = false;
     int rc = check_member(h, d);
     if (rc) return rc;
     if (!in) return fail(h, RFIM_EINVAL, "null buffer");
@@ -1063,6 +1106,7 @@ int rfim_pt_get_permutation(rfim_pt* h, int d, int32_t* t2r) {
 }
 
 int rfim_pt_set_permutation(rfim_pt* h, int d, const int32_t* t2r_in) {
+    if (h) h->terms_fresh = false;
     int rc = check_member(h, d);
     if (rc) return rc;
     if (!t2r_in || !h->have_T) return fail(h, RFIM_EINVAL, "null buffer or temperatures not set");

@@ -30,6 +30,7 @@ struct View {
     int32_t* r2t;                  // [D][R]
     const uint32_t* keys;          // [D][2]
     long long* acc;                // [D][R(slot)][3]: Eb, Ef, Msum accumulators of the reduction
+    long long* last;               // [D][R(slot)][3]: the terms the last exchange step consumed (acc is zeroed by it)
     double* ework;                 // [D][R(rank)] energies of the current exchange step
     unsigned long long* att;       // [D][R]
     unsigned long long* accn;      // [D][R]

@@ -104,3 +104,43 @@ def test_packing_errors():
     with pytest.raises(binding.RfimPtError):
         g.set_kernel_variant(2)
     g.close()
+
+
+def test_bit_packed_host_interface_roundtrip():
+    """rfim_pt_get/set_spins_all_bits: natural-order bits on the host, both device storage modes, against the int8 getters."""
+    from paper_1508_06268_b200 import binding
+    for L, packing in ((8, 8), (32, 8), (32, 1)):
+        g = binding.RfimPT(L, 3, 1.0, 1.0, BIMODAL, seeds=[5, 6])
+        if packing == 1:
+            g.set_packing(1)
+        ref = g.get_spins_all()                                   # [D][R][N] of +-1
+        bits = g.get_spins_all_bits()
+        assert bits.shape == (2, 3, L ** 3 // 8)
+        assert np.array_equal(np.unpackbits(bits, axis=-1, bitorder="little"), (ref > 0).astype(np.uint8))
+        rng = np.random.default_rng(L + packing)
+        new = rng.integers(0, 2, size=ref.shape, dtype=np.uint8)
+        g.set_spins_all_bits(np.ascontiguousarray(np.packbits(new, axis=-1, bitorder="little")))
+        assert np.array_equal(g.get_spins_all(), (2 * new.astype(np.int8) - 1))
+        assert np.array_equal(g.get_spins_all_bits(), np.packbits(new, axis=-1, bitorder="little"))
+        g.close()
+
+
+def test_observables_reuse_the_in_kernel_measurement():
+    """after a call that ends on an exchange step the getters return the terms measured inside the sweep kernel; after
+    anything that touches the lattices they reduce again: both must equal the oracle's recomputed Hamiltonian."""
+    T = geometric_ladder(1.0, 4.0, 4)
+    g, o = make_pair(32, 4, 1.0, 1.5, GAUSSIAN, 8, T)
+    g.sweep(10, 5); o.sweep(10, 5)                                 # ends on a step: cached terms
+    for a, b in zip(g.get_energy_terms(), o.get_energy_terms()):
+        assert np.array_equal(a, b)
+    E, M, _ = g.observables(); Eo, Mo, _ = o.observables()
+    assert np.array_equal(E, Eo) and np.array_equal(M, Mo)
+    g.sweep(3, 5); o.sweep(3, 5)                                   # does not end on a step: fresh reduction
+    for a, b in zip(g.get_energy_terms(), o.get_energy_terms()):
+        assert np.array_equal(a, b)
+    g.sweep(2, 5); o.sweep(2, 5)                                   # on a step again, then overwrite one lattice
+    s = -g.get_spins_slot(1)
+    g.set_spins_slot(1, s); o.set_spins_slot(1, s)
+    for a, b in zip(g.get_energy_terms(), o.get_energy_terms()):
+        assert np.array_equal(a, b)
+    g.close()
