@@ -117,6 +117,16 @@ __host__ __device__ inline size_t res_smem_bytes(int L, int cap_reps) {
     return (b + 15) & ~(size_t)15;
 }
 
+__device__ __forceinline__ uint32_t lds32(uint32_t saddr) {
+    uint32_t r;
+#if defined(__CUDA_ARCH__)
+    asm volatile("ld.shared.u32 %0, [%1];" : "=r"(r) : "r"(saddr));
+#else
+    r = 0;
+#endif
+    return r;
+}
+
 __device__ __forceinline__ uint2 lds64(uint32_t saddr) {
     uint2 r;
 #if defined(__CUDA_ARCH__)
@@ -391,7 +401,10 @@ __device__ __forceinline__ void res_row(const View& v, const ResParams& rp, uint
                 uint32_t flips = 0;
 #pragma unroll
                 for (int j = 0; j < 4; ++j) {
-                    const uint2 ent = lds64(__byte_perm(idx8[w], ln.tab_addr, 0x7650 + j));
+                    // without a zero threshold in the table only the first word of the entry is needed: one wavefront
+                    const uint32_t ea = __byte_perm(idx8[w], ln.tab_addr, 0x7650 + j);
+                    uint2 ent;
+                    if (NEVER) ent = lds64(ea); else { ent.x = lds32(ea); ent.y = 0u; }
                     bool acc = u[j] <= ent.x;
                     if (NEVER) acc = acc && ent.y == 0u;
                     if (acc) flips |= kResSP << (8 * j);
