@@ -255,7 +255,7 @@ int upload_tables(rfim_pt* h) {
                 const double aY = h->amax[d] * std::fabs(c);
                 const double Xmax = std::fabs(c) * std::fabs(h->J) * 6.0 + 32.0;
                 const double arg_err = std::ldexp(3.0 * aY + 2.0 * Xmax, -24);
-                const double eta = M_LN2 * arg_err + std::ldexp(1.0, -21) + std::ldexp(1.0, -23);
+                const double eta = M_LN2 * arg_err + std::ldexp(1.0, -21) + std::ldexp(1.0, -22);   // ex2.approx, float(u) (rounded down by the resident kernel: < 2^-23)
                 const double bd = 1.5 * eta * kTwo32 + 512.0;
                 band[(size_t)d * R + t] = (float)std::min(bd, 3.0e38);
             }
@@ -1371,3 +1371,9 @@ int rfim_pt_bench_stream(void* stream, size_t bytes, double* ms, double* bytes_m
 }
 
 }  // extern "C"
+
+#ifdef RFIM_RES_TIMING
+extern "C" int rfim_pt_debug_timing(unsigned long long* out /* [256][8] */) {
+    return cudaMemcpyFromSymbol(out, rfim::g_res_timing, sizeof(unsigned long long) * 256 * 8) == cudaSuccess ? 0 : -1;
+}
+#endif

@@ -3,7 +3,7 @@
 //
 // Decomposition.  The D*n active replicas (by temperature rank) are stacked into one list of
 // D*n*L planes (plane P = (d*n + t)*L + z; a replica shard lists its stored slots instead of the ranks).  CTA b of a cooperative launch owns the contiguous run
-// [start_b, start_b + count_b) with counts differing by at most one, so 148 SMs hold 55 or 56 planes
+// [start_b, start_b + count_b) with counts differing by at most one (the last CTAs take the longer runs), so 148 SMs hold 55 or 56 planes
 // each at L = 64, R = 128: no replica-granular imbalance (128 replicas do not divide over 148 SMs).
 // A run is loaded once, swept 2*sweeps phases (colour 0, colour 1, ...) in place, and stored once.
 // Only the planes at the ends of a run (and at a replica seam inside it) have a z-neighbour in
@@ -48,12 +48,21 @@
 
 namespace rfim {
 
+#ifdef RFIM_RES_TIMING
+__device__ unsigned long long g_res_timing[256][8];
+__device__ __forceinline__ unsigned long long res_now() { unsigned long long t; asm volatile("mov.u64 %0, %globaltimer;" : "=l"(t)); return t; }
+#define RES_STAMP(i) do { if (threadIdx.x == 0) g_res_timing[blockIdx.x][i] = res_now(); } while (0)
+#else
+#define RES_STAMP(i) do { } while (0)
+#endif
+
 #ifndef RFIM_RES_THREADS
 #define RFIM_RES_THREADS 512
 #endif
 constexpr int kResThreads = RFIM_RES_THREADS;
 constexpr uint32_t kResSP = 8;                  // shared-memory spin coding: 0 / SP
 constexpr int kResTabBytes = 256;               // per-replica acceptance table slot (256-byte aligned)
+constexpr int kResLoadDepth = 8;                // 16-byte loads a thread keeps in flight while the run is loaded
 
 // shared-memory geometry of the resident kernel for L = 32 K
 template <int K>
@@ -82,7 +91,7 @@ struct ResParams {
     uint32_t epoch;              // launch id: progress words hold (epoch << 8) | phases published
     uint32_t* prog;              // [grid]
     int total_planes;            // D * n * L
-    int q, rem;                  // run of CTA b: start = b*q + min(b, rem), count = q + (b < rem)
+    int q, rem;                  // run of CTA b: count = q, or q + 1 for the last rem CTAs of the grid
     int cap_reps;                // replicas a run can touch -- same carve for every CTA
     int d0;                      // first member of this launch's group (plane P = ((d - d0) * n + t) * L + z)
     const float* fielda_res;     // Gaussian: [D][2][L][2][4K][L/2] float4 (task order), (float)g_i (exact)
@@ -170,6 +179,26 @@ __device__ __forceinline__ uint4 res_piece_from_global(const uint8_t* spins, siz
     x.x *= kResSP; x.y *= kResSP; x.z *= kResSP; x.w *= kResSP;
     return x;
 }
+// raw form of a piece as it sits in global memory (16 bytes, or 16 bits in .x when packed) and its conversion
+__device__ __forceinline__ uint4 res_piece_raw(const uint8_t* spins, size_t off, int packed) {
+    uint4 x = make_uint4(0u, 0u, 0u, 0u);
+    if (packed) {
+#if defined(__CUDA_ARCH__)
+        x.x = __ldcg(reinterpret_cast<const unsigned short*>(spins + (off >> 3)));
+#endif
+    } else {
+        x = ld_cg16(spins + off);
+    }
+    return x;
+}
+__device__ __forceinline__ uint4 res_piece_expand(uint4 x, int packed) {
+    if (packed) {
+        const uint32_t q = x.x;
+        x.x = res_nibble_to_word(q); x.y = res_nibble_to_word(q >> 4); x.z = res_nibble_to_word(q >> 8); x.w = res_nibble_to_word(q >> 12);
+    }
+    x.x *= kResSP; x.y *= kResSP; x.z *= kResSP; x.w *= kResSP;
+    return x;
+}
 __device__ __forceinline__ void res_piece_to_global(uint8_t* spins, size_t off, int packed, uint4 x) {
     x.x >>= 3; x.y >>= 3; x.z >>= 3; x.w >>= 3;
     if (packed)
@@ -193,11 +222,23 @@ __device__ __forceinline__ Words4 philox_rkreg(const uint32_t (&rk)[20], uint32_
     return w;
 }
 
+// u as a float, rounded toward minus infinity: cvt.rm compiles to I2F.U32.RM, which runs on the XU pipe (the default
+// round-to-nearest conversion is I2FP on the ALU pipe, the pipe the Philox XORs already saturate).  Error < 2^-23 relative.
+__device__ __forceinline__ float res_u2f(uint32_t u) {
+#if defined(__CUDA_ARCH__)
+    float f;
+    asm("cvt.rm.f32.u32 %0, %1;" : "=f"(f) : "r"(u));
+    return f;
+#else
+    return (float)u;
+#endif
+}
+
 // the float path of one Gaussian attempt: d = float(u) - P~, P~ = 2^(g*y + x); accept iff d < 0 unless |d| < band
 __device__ __forceinline__ float res_gauss_diff(uint32_t idx8, int j, uint32_t tab_addr, float a, uint32_t u) {
     const uint2 ent = lds64(__byte_perm(idx8, tab_addr, 0x7650 + j));
     const float P = ex2_approx(fmaf(a, __uint_as_float(ent.y), __uint_as_float(ent.x)));
-    return __uint2float_rn(u) - P;
+    return res_u2f(u) - P;
 }
 
 // Rare path: some site of the piece fell inside the float path's guard band.  Redo the piece's four words: sites
@@ -464,8 +505,12 @@ __global__ void __launch_bounds__(THREADS, 1) k_sweep_res(const View v, const Re
 
     const int tid = threadIdx.x, lane = tid & 31;
     const int b = blockIdx.x;
-    const int start = b * rp.q + min(b, rp.rem);
-    const int count = rp.q + (b < rp.rem ? 1 : 0);
+    RES_STAMP(0);
+    // the last rp.rem CTAs own one plane more: they hold the hottest replicas, whose planes are slightly cheaper
+    // (fewer exact-rule fall-backs), so the longer runs do not also carry the dearer planes
+    const int nshort = (int)gridDim.x - rp.rem;                      // CTAs with rp.q planes
+    const int start = b * rp.q + max(0, b - nshort);
+    const int count = rp.q + (b >= nshort ? 1 : 0);
     if (count == 0) return;
     const int E = count * LH;                   // rows in use (per colour and class)
     const int nb = (E + 31) / 32;               // 32-row blocks
@@ -487,8 +532,8 @@ __global__ void __launch_bounds__(THREADS, 1) k_sweep_res(const View v, const Re
         const int P = start + p, dt = P / L, z = P % L;
         const int Pzp = dt * L + (z + 1 == L ? 0 : z + 1), Pzm = dt * L + (z == 0 ? L - 1 : z - 1);
         auto owner = [&](int Q) {
-            const int big = rp.rem * (rp.q + 1);
-            return Q < big ? Q / (rp.q + 1) : rp.rem + (Q - big) / rp.q;
+            const int small = nshort * rp.q;
+            return Q < small ? Q / rp.q : nshort + (Q - small) / (rp.q + 1);
         };
         ResPlane pi;
         const bool lp = Pzp >= start && Pzp < start + count, lm = Pzm >= start && Pzm < start + count;
@@ -531,33 +576,51 @@ __global__ void __launch_bounds__(THREADS, 1) k_sweep_res(const View v, const Re
         reinterpret_cast<uint2*>(s_tab + (size_t)r * kResTabBytes)[idx] = ent;
     }
     for (int i = tid; i < nb; i += THREADS) s_done[i] = 0;
+    if (tid == 0) { s_ctl[0] = 0; s_ctl[1] = 0; s_ctl[2] = 0; s_ctl[3] = 0; }
     __syncthreads();
-    if (tid == 0) {
-        int nbd = 0;
-        auto is_boundary = [&](int eb) {
-            const int p0 = (eb * 32) / LH, p1 = min((eb * 32 + 31) / LH, count - 1);
-            for (int p = p0; p <= p1; ++p)
-                if (s_plane[p].zp_pl < 0 || s_plane[p].zm_pl < 0) return true;
-            return false;
-        };
-        for (int eb = 0; eb < nb; ++eb) if (is_boundary(eb)) s_order[nbd++] = eb;
-        int k = nbd;
-        for (int eb = 0; eb < nb; ++eb) if (!is_boundary(eb)) s_order[k++] = eb;
-        s_ctl[0] = 0; s_ctl[1] = 0; s_ctl[2] = 0; s_ctl[3] = nbd;
+    // block order: blocks with a plane whose z-neighbour lives in another CTA first (any order among them)
+    {
+        bool bnd = false;
+        if (tid < nb) {
+            const int p0 = (tid * 32) / LH, p1 = min((tid * 32 + 31) / LH, count - 1);
+            for (int p = p0; p <= p1; ++p) bnd = bnd || s_plane[p].zp_pl < 0 || s_plane[p].zm_pl < 0;
+        }
+        if (tid < nb && bnd) s_order[atomicAdd(&s_ctl[3], 1)] = tid;
+        __syncthreads();
+        const int nbd = s_ctl[3];
+        if (tid < nb && !bnd) s_order[nbd + atomicAdd(&s_ctl[0], 1)] = tid;
+        __syncthreads();
+        if (tid == 0) s_ctl[0] = 0;
     }
 
+    RES_STAMP(1);
     // ---- load the run: global [colour][z][y][ROWB] (0/1) -> shared [colour][s][k][row] (0/SP) ------------------
+    // kResLoadDepth loads in flight per thread: the run comes from HBM (or L2) at full rate instead of one
+    // round trip per 16-byte piece
     {
         const int units = count * 2 * L * K;            // 16-byte pieces
-        for (int u = tid; u < units; u += THREADS) {
-            const int k = u % K, y = (u / K) % L, col = (u / (K * L)) & 1, p = u / (2 * K * L);
-            const ResPlane pi = s_plane[p];
-            const int ds = s_rep[pi.rep].ds, z = pi.z;
-            const uint4 x = res_piece_from_global(v.spins, (size_t)(((long long)ds * 2 + col) * v.Nh + ((long long)z * L + y) * ROWB + 16 * k), v.packed);
-            *reinterpret_cast<uint4*>(smem + A(col, (y + z) & 1, k, p * LH + (y >> 1))) = x;
+        for (int u0 = 0; u0 < units; u0 += THREADS * kResLoadDepth) {
+            uint4 raw[kResLoadDepth];
+            uint32_t dst[kResLoadDepth];
+#pragma unroll
+            for (int j = 0; j < kResLoadDepth; ++j) {
+                const int u = u0 + j * THREADS + tid;
+                dst[j] = 0xFFFFFFFFu;
+                if (u < units) {
+                    const int k = u % K, y = (u / K) % L, col = (u / (K * L)) & 1, p = u / (2 * K * L);
+                    const ResPlane pi = s_plane[p];
+                    const int ds = s_rep[pi.rep].ds, z = pi.z;
+                    raw[j] = res_piece_raw(v.spins, (size_t)(((long long)ds * 2 + col) * v.Nh + ((long long)z * L + y) * ROWB + 16 * k), v.packed);
+                    dst[j] = A(col, (y + z) & 1, k, p * LH + (y >> 1));
+                }
+            }
+#pragma unroll
+            for (int j = 0; j < kResLoadDepth; ++j)
+                if (dst[j] != 0xFFFFFFFFu) *reinterpret_cast<uint4*>(smem + dst[j]) = res_piece_expand(raw[j], v.packed);
         }
     }
     __syncthreads();
+    RES_STAMP(2);
     const int n_bblocks = s_ctl[3];
     const int total_tasks = nb * rp.phases;
     const uint32_t tab0 = (uint32_t)__cvta_generic_to_shared(s_tab);
@@ -573,7 +636,11 @@ __global__ void __launch_bounds__(THREADS, 1) k_sweep_res(const View v, const Re
         if (g >= total_tasks) break;
         while (g - base_cur >= nb) { base_cur += nb; ++p_cur; }
         const int p = p_cur, bidx = g - base_cur;
+        #ifdef RFIM_DBG_NOMEAS
+        const bool meas = false;
+#else
         const bool meas = rp.measure && p >= rp.phases - 2;   // the last two phases also measure their colour
+#endif
         const int c = p & 1, oc = 1 - c;
         const uint32_t sweep = rp.sweep0 + (uint32_t)(p >> 1);
         const uint32_t dom = c == 0 ? kDomColour0 : kDomColour1;
@@ -671,7 +738,9 @@ __global__ void __launch_bounds__(THREADS, 1) k_sweep_res(const View v, const Re
             atomicAdd(&s_done[eb], 1);
         }
     }
+    RES_STAMP(3);
     __syncthreads();
+    RES_STAMP(4);
 
     // ---- store the run back, hand the measurement over ------------------------------------------------------
     {
@@ -687,6 +756,8 @@ __global__ void __launch_bounds__(THREADS, 1) k_sweep_res(const View v, const Re
             for (int r = tid; r < nrep * 3; r += THREADS)
                 atomicAdd(reinterpret_cast<unsigned long long*>(v.acc + (long long)(s_rep[r / 3].d * v.R + s_rep[r / 3].slot) * 3 + r % 3), (unsigned long long)s_acc[r]);
     }
+    RES_STAMP(5);
+#ifndef RFIM_DBG_NOEXCH
     if (rp.exchange) {
         // the CTA that arrives last has every replica's sums in View::acc (integer atomics at L2): it runs the exchange step
         __threadfence();
@@ -702,6 +773,8 @@ __global__ void __launch_bounds__(THREADS, 1) k_sweep_res(const View v, const Re
             if (tid == 0) *rp.ticket = 0u;
         }
     }
+#endif
+    RES_STAMP(6);
 }
 
 }  // namespace rfim
