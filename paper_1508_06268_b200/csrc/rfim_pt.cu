@@ -66,6 +66,7 @@ struct rfim_pt {
     bool has_never = false;           // some reachable bimodal table entry has threshold 0
     float* fielda_res = nullptr;      // resident-kernel copies of the field (task order), L = 32 or 64
     uint8_t* fieldb_res = nullptr;
+    long long* gsum_res = nullptr;    // Gaussian: [D][L] sum of g_i over plane z (the resident kernel measures Ef = 2 * sum over up spins - this)
     uint32_t* res_prog = nullptr;     // [kResMaxGrid] progress words of the resident kernel
     uint32_t res_epoch = 0;
     bool terms_fresh = false;         // View::last holds the energy terms of the CURRENT lattices (last call ended on an exchange step)
@@ -194,6 +195,10 @@ int upload_field(rfim_pt* h, int d) {
             for (int z = 0; z < L; ++z) for (int y = 0; y < L; ++y) for (int x = 0; x < L; ++x)
                 fr[res_field_index(h, x, y, z)] = (float)f[x + (long long)L * (y + (long long)L * z)];
             CU(cudaMemcpyAsync(h->fielda_res + (long long)d * h->N, fr.data(), h->N * sizeof(float), cudaMemcpyHostToDevice, h->stream));
+            std::vector<long long> gs(L, 0);
+            for (int z = 0; z < L; ++z)
+                for (long long i = 0; i < (long long)L * L; ++i) gs[z] += f[(long long)z * L * L + i];
+            CU(cudaMemcpyAsync(h->gsum_res + (long long)d * L, gs.data(), (size_t)L * sizeof(long long), cudaMemcpyHostToDevice, h->stream));
             CU(cudaStreamSynchronize(h->stream));
         }
         CU(cudaStreamSynchronize(h->stream));
@@ -427,7 +432,13 @@ int launch_res_t(rfim_pt* h, const ResPlan& pl, const ResParams& rp) {
     auto kernel = k_sweep_res<KIND, K, NEVER, UNI, kResThreads>;
     CU(cudaFuncSetAttribute(kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)pl.smem));
     void* argv[] = {const_cast<void*>(static_cast<const void*>(&h->v)), const_cast<void*>(static_cast<const void*>(&rp))};
+#ifdef RFIM_DBG_PLAIN_LAUNCH
+    (void)argv;
+    kernel<<<dim3((unsigned)pl.grid), dim3(kResThreads), pl.smem, h->stream>>>(h->v, rp);
+    CU(cudaGetLastError());
+#else
     CU(cudaLaunchCooperativeKernel(reinterpret_cast<const void*>(kernel), dim3((unsigned)pl.grid), dim3(kResThreads), argv, pl.smem, h->stream));
+#endif
     h->launches += 1;
     return RFIM_OK;
 }
@@ -464,7 +475,7 @@ int launch_res(rfim_pt* h, int sweeps, bool measure, bool* exchanged) {
         rp.total_planes = pl.total; rp.q = pl.q; rp.rem = pl.rem;
         rp.cap_reps = pl.cap_reps;
         rp.d0 = d0;
-        rp.fielda_res = h->fielda_res; rp.fieldb_res = h->fieldb_res;
+        rp.fielda_res = h->fielda_res; rp.fieldb_res = h->fieldb_res; rp.gsum = h->gsum_res;
         rp.diag = h->v.diag;
         {
             uint32_t k0 = (uint32_t)(h->seeds[d0] & 0xFFFFFFFFull), k1 = (uint32_t)(h->seeds[d0] >> 32);
@@ -657,7 +668,7 @@ int create_impl(rfim_pt** out, int L, int R, double J, double hh, int kind, int 
     A(alloc_into(h, &h->res_prog, (size_t)kResMaxGrid + 1));
     if (flow_supported(h)) {
         if (kind == RFIM_FIELD_BIMODAL) A(alloc_into(h, &h->fieldb_res, (size_t)D * h->N));
-        else A(alloc_into(h, &h->fielda_res, (size_t)D * h->N));
+        else { A(alloc_into(h, &h->fielda_res, (size_t)D * h->N)); A(alloc_into(h, &h->gsum_res, (size_t)D * L)); }
     }
     {
         int dev = 0;

@@ -19,10 +19,10 @@
 // only ever waits for lower-numbered tasks, so the lowest outstanding task can always run: no
 // deadlock, no tail at the end of a phase.
 //
-// Measurement (S5) rides on the last two phases of the launch, from registers the update holds
-// anyway: each phase sums Msum and Ef of the colour it has just updated (the field copy stores g_i as
-// exact floats), and since every bond has exactly one colour-1 end the colour-1 phase also gives
-// Eb = sum over colour-1 sites of s_i' * (six-neighbour sum).  Sums go per replica to shared memory,
+// Measurement (S5) rides on the last phase of the launch (colour 1), from registers the update
+// holds anyway: Msum and Ef of the colour-1 words it has just updated and of the colour-0 words of the same
+// row (final since the phase before; only their field is loaded in addition), and since every bond has
+// exactly one colour-1 end, Eb = sum over colour-1 sites of s_i' * (six-neighbour sum).  Sums go per replica to shared memory,
 // then to View::acc with integer atomics (order-independent, hence deterministic).  The
 // CTA that finishes last then runs the exchange step itself (small batches), so a whole
 // parallel-tempering move is one launch.
@@ -96,6 +96,7 @@ struct ResParams {
     int d0;                      // first member of this launch's group (plane P = ((d - d0) * n + t) * L + z)
     const float* fielda_res;     // Gaussian: [D][2][L][2][4K][L/2] float4 (task order), (float)g_i (exact)
     const uint8_t* fieldb_res;   // bimodal:  [D][2][L][2][K][L/2] uint4, 0x80 where h_i = +1
+    const long long* gsum;       // Gaussian: [D][L] sum of g_i over plane z
     unsigned long long* diag;
     uint32_t rk0[20];            // Philox round keys of member 0 (used from the constant bank when D == 1)
 };
@@ -123,6 +124,7 @@ __host__ __device__ inline size_t res_smem_bytes(int L, int cap_reps) {
     b += nbcap * 2 * sizeof(int);                           // block order, block completion counters
     b += 16;                                                // counters
     b += (size_t)cap_reps * 3 * sizeof(long long);          // measurement accumulators
+    b += (size_t)(kResThreads / 32) * 4 * sizeof(long long); // per-warp measurement slots
     return (b + 15) & ~(size_t)15;
 }
 
@@ -323,11 +325,11 @@ __device__ __forceinline__ ResPiece res_load_piece(const uint8_t* smem, const ui
     return pc;
 }
 
-// Measurement of one piece, taken in the last two phases of a launch from what the update holds in registers:
+// Measurement of one piece, taken in the last phase of a launch from what the update holds in registers:
 // me = updated words of the piece, fb / f0..f3 = the piece's field (bimodal 0x80 flags / Gaussian g_i as floats, exact),
 // idx8 = table offsets before the update (bits 3..5 of a byte = SP * n1).  Returns {Eb, Ef, Msum} contributions of the
 // piece's 16 sites: Ef and Msum of this colour always, Eb (the six-neighbour form: every bond has one colour-1 end)
-// only when with_eb, i.e. in the colour-1 phase.  Ef fits an int: 16 terms below 2^23.
+// only when with_eb (the colour-1 words).  Both fit an int.
 template <int KIND>
 __device__ __noinline__ int3 res_measure_piece(uint4 mev, uint4 idx8v, uint4 fbv, float4 f0, float4 f1, float4 f2, float4 f3, int with_eb) {
     const uint32_t me[4] = {mev.x, mev.y, mev.z, mev.w};
@@ -348,18 +350,24 @@ __device__ __noinline__ int3 res_measure_piece(uint4 mev, uint4 idx8v, uint4 fbv
         for (int w = 0; w < 4; ++w) { hs0 += dot4(hb[w], me[w]); hh += dot4(hb[w], 0x01010101u); }
         r.y = 4 * (hs0 / 8) - 2 * hh - 2 * (s0 / 8) + 16;
     } else {
+        // SP * (sum of g_i over the up spins of the piece): |.| <= 16 * 2^23 * SP = 2^30.  Ef = 2 * (that / SP) - (sum of g_i over
+        // all sites), and the second term is a constant of the plane (ResParams::gsum), subtracted once when the sums are handed over
         const float gf[16] = {f0.x, f0.y, f0.z, f0.w, f1.x, f1.y, f1.z, f1.w, f2.x, f2.y, f2.z, f2.w, f3.x, f3.y, f3.z, f3.w};
         int ef = 0;
 #pragma unroll
         for (int w = 0; w < 4; ++w)
 #pragma unroll
-            for (int j = 0; j < 4; ++j) {
-                const int g = __float2int_rn(gf[4 * w + j]);
-                ef += ((me[w] >> (8 * j)) & kResSP) ? g : -g;
-            }
+            for (int j = 0; j < 4; ++j) ef += __float2int_rn(gf[4 * w + j]) * (int)__byte_perm(me[w], 0u, 0x4440 + j);
         r.y = ef;
     }
     return r;
+}
+
+__device__ __noinline__ void res_flush_sums(long long* s_acc, int rep, long long eb, long long ef, long long ms) {
+    if (rep < 0) return;
+    atomicAdd(reinterpret_cast<unsigned long long*>(s_acc + 3 * rep + 0), (unsigned long long)eb);
+    atomicAdd(reinterpret_cast<unsigned long long*>(s_acc + 3 * rep + 1), (unsigned long long)ef);
+    atomicAdd(reinterpret_cast<unsigned long long*>(s_acc + 3 * rep + 2), (unsigned long long)ms);
 }
 
 // Per-task lane constants of the row update: shared-memory byte offsets of class 0 (class 1 = + K * ARR, an
@@ -474,10 +482,21 @@ __device__ __forceinline__ void res_row(const View& v, const ResParams& rp, uint
             if (BND && (remote_p || remote_m))
                 res_piece_to_global(v.spins, (size_t)((ln.ds2 + (uint32_t)c) * (uint32_t)v.Nh + grow + 16u * k), v.packed, nw);
             if (MEAS) {
+                // the final phase (colour 1) measures both colours: its own updated words (with Eb: every bond has one
+                // colour-1 end) and the colour-0 words of the same row, xr[k], final since the phase before; their field
+                // sits one colour block (L planes x 2 classes) below this one
                 const float4 z4 = make_float4(0.f, 0.f, 0.f, 0.f);
                 const int3 m3 = res_measure_piece<KIND>(nw, make_uint4(idx8[0], idx8[1], idx8[2], idx8[3]), fb,
-                                                        KIND ? fa[0] : z4, KIND ? fa[1] : z4, KIND ? fa[2] : z4, KIND ? fa[3] : z4, c);
-                m_eb += m3.x; m_ef += m3.y; m_ms += m3.z;
+                                                        KIND ? fa[0] : z4, KIND ? fa[1] : z4, KIND ? fa[2] : z4, KIND ? fa[3] : z4, 1);
+                float4 ga[4] = {z4, z4, z4, z4};
+                uint4 gb = make_uint4(0u, 0u, 0u, 0u);
+                if (KIND == 0) gb = __ldg(fq - 2 * G::L * K * LH + k * LH);
+                else {
+#pragma unroll
+                    for (int w = 0; w < 4; ++w) ga[w] = __ldg(fp - 2 * G::L * W * LH + (4 * k + w) * LH);
+                }
+                const int3 m0 = res_measure_piece<KIND>(xr[k], make_uint4(0u, 0u, 0u, 0u), gb, ga[0], ga[1], ga[2], ga[3], 0);
+                m_eb += m3.x; m_ef += m3.y + m0.y; m_ms += m3.z + m0.z;
             }
         }
     }
@@ -522,6 +541,7 @@ __global__ void __launch_bounds__(THREADS, 1) k_sweep_res(const View v, const Re
     int* s_done = s_order + G::NBCAP;           // per block: tasks completed so far (one per phase)
     int* s_ctl = s_done + G::NBCAP;             // [0],[1] boundary tasks done in the open even / odd phase, [2] next task number, [3] boundary blocks
     long long* s_acc = reinterpret_cast<long long*>(s_ctl + 4);   // [rep][3] measurement accumulators
+    long long* s_wacc = s_acc + 3 * rp.cap_reps;                   // [warp][4]: replica held (-1: none), Eb, Ef, Msum of that replica
     // byte offset of row e of array (colour, class, piece)
     auto A = [&](int col, int s, int k, int e) { return (uint32_t)(((col * 2 + s) * K + k) * ARR + e * 16); };
 
@@ -576,8 +596,14 @@ __global__ void __launch_bounds__(THREADS, 1) k_sweep_res(const View v, const Re
         reinterpret_cast<uint2*>(s_tab + (size_t)r * kResTabBytes)[idx] = ent;
     }
     for (int i = tid; i < nb; i += THREADS) s_done[i] = 0;
+    if (tid < THREADS / 32) { s_wacc[4 * tid] = -1; s_wacc[4 * tid + 1] = 0; s_wacc[4 * tid + 2] = 0; s_wacc[4 * tid + 3] = 0; }
     if (tid == 0) { s_ctl[0] = 0; s_ctl[1] = 0; s_ctl[2] = 0; s_ctl[3] = 0; }
     __syncthreads();
+    // Gaussian Ef = 2 * (sum of g_i over up spins) - (sum of g_i over all sites): the second term, a constant of each plane
+    // (ResParams::gsum), goes into the accumulator now, scaled like the first one is measured (SP * sum over up spins)
+    if (KIND == 1 && rp.measure && tid < count)
+        atomicAdd(reinterpret_cast<unsigned long long*>(s_acc + 3 * s_plane[tid].rep + 1),
+                  (unsigned long long)(-(long long)(kResSP / 2) * rp.gsum[(long long)s_rep[s_plane[tid].rep].d * L + s_plane[tid].z]));
     // block order: blocks with a plane whose z-neighbour lives in another CTA first (any order among them)
     {
         bool bnd = false;
@@ -639,7 +665,7 @@ __global__ void __launch_bounds__(THREADS, 1) k_sweep_res(const View v, const Re
         #ifdef RFIM_DBG_NOMEAS
         const bool meas = false;
 #else
-        const bool meas = rp.measure && p >= rp.phases - 2;   // the last two phases also measure their colour
+        const bool meas = rp.measure && p == rp.phases - 1;   // the last phase (colour 1) also measures, both colours
 #endif
         const int c = p & 1, oc = 1 - c;
         const uint32_t sweep = rp.sweep0 + (uint32_t)(p >> 1);
@@ -649,7 +675,7 @@ __global__ void __launch_bounds__(THREADS, 1) k_sweep_res(const View v, const Re
         const int e_raw = eb * 32 + lane;
         const bool valid = !RAGGED || e_raw < E;
         const int e = valid ? e_raw : E - 1;
-        const int pl = e / LH, i = e % LH;
+        const int pl = (int)((unsigned)e / (unsigned)LH), i = (int)((unsigned)e % (unsigned)LH);
         const ResPlane pi = s_plane[pl];
         const ResRep* rr = s_rep + pi.rep;
         const int z = pi.z;
@@ -660,7 +686,8 @@ __global__ void __launch_bounds__(THREADS, 1) k_sweep_res(const View v, const Re
         // remote neighbour planes: their owners have published phase p-1
         if (p > 0) {
             const int b_zp = remote_p ? eb : e_zp >> 5, b_zm = remote_m ? eb : e_zm >> 5;
-            const bool ok = lds_volatile(s_done + eb) >= p && lds_volatile(s_done + b_zp) >= p && lds_volatile(s_done + b_zm) >= p;
+            const int d0 = lds_volatile(s_done + eb), d1 = lds_volatile(s_done + b_zp), d2 = lds_volatile(s_done + b_zm);
+            const bool ok = min(d0, min(d1, d2)) >= p;
             if (btask || !__all_sync(0xFFFFFFFFu, ok))
                 res_wait_slow(s_done, eb, b_zp, b_zm, p, remote_p ? rp.prog + pi.zp_owner : nullptr,
                               remote_m ? rp.prog + pi.zm_owner : nullptr, (rp.epoch << 8) | (uint32_t)p, rp.diag);
@@ -704,20 +731,24 @@ __global__ void __launch_bounds__(THREADS, 1) k_sweep_res(const View v, const Re
         }
 
         if (meas) {
-            // per-replica sums in shared memory: one warp usually holds one replica (a seam can split it)
+            // per-replica sums: a warp keeps the sums of the replica it is working on in its own shared-memory slot (plain
+            // read-modify-write by lane 0) and hands them to the CTA's accumulators only when the replica changes and after
+            // its last task: the 64-bit shared-memory atomics (compare-and-swap loops) would otherwise all collide at the
+            // end of the measuring phase.  A warp that straddles a replica seam adds lane by lane.
             const int rep = valid ? (int)pi.rep : -1;
             const int rep0 = __shfl_sync(0xFFFFFFFFu, rep, 0);
-            if (__all_sync(0xFFFFFFFFu, rep == rep0)) {
+            if (__all_sync(0xFFFFFFFFu, rep == rep0 || rep < 0)) {
                 m_eb = warp_sum(m_eb); m_ef = warp_sum(m_ef); m_ms = warp_sum(m_ms);
                 if (lane == 0 && rep0 >= 0) {
-                    atomicAdd(reinterpret_cast<unsigned long long*>(s_acc + 3 * rep0 + 0), (unsigned long long)m_eb);
-                    atomicAdd(reinterpret_cast<unsigned long long*>(s_acc + 3 * rep0 + 1), (unsigned long long)m_ef);
-                    atomicAdd(reinterpret_cast<unsigned long long*>(s_acc + 3 * rep0 + 2), (unsigned long long)m_ms);
+                    long long* wa = s_wacc + 4 * (tid >> 5);
+                    if (wa[0] != (long long)rep0) {
+                        res_flush_sums(s_acc, (int)wa[0], wa[1], wa[2], wa[3]);
+                        wa[0] = rep0; wa[1] = 0; wa[2] = 0; wa[3] = 0;
+                    }
+                    wa[1] += m_eb; wa[2] += m_ef; wa[3] += m_ms;
                 }
-            } else if (rep >= 0) {
-                atomicAdd(reinterpret_cast<unsigned long long*>(s_acc + 3 * rep + 0), (unsigned long long)m_eb);
-                atomicAdd(reinterpret_cast<unsigned long long*>(s_acc + 3 * rep + 1), (unsigned long long)m_ef);
-                atomicAdd(reinterpret_cast<unsigned long long*>(s_acc + 3 * rep + 2), (unsigned long long)m_ms);
+            } else {
+                res_flush_sums(s_acc, rep, m_eb, m_ef, m_ms);
             }
         }
         __syncwarp();
@@ -738,6 +769,10 @@ __global__ void __launch_bounds__(THREADS, 1) k_sweep_res(const View v, const Re
             atomicAdd(&s_done[eb], 1);
         }
     }
+    if (lane == 0) {                                  // hand this warp's measurement sums over
+        long long* wa = s_wacc + 4 * (tid >> 5);
+        res_flush_sums(s_acc, (int)wa[0], wa[1], wa[2], wa[3]);
+    }
     RES_STAMP(3);
     __syncthreads();
     RES_STAMP(4);
@@ -754,7 +789,11 @@ __global__ void __launch_bounds__(THREADS, 1) k_sweep_res(const View v, const Re
         }
         if (rp.measure)
             for (int r = tid; r < nrep * 3; r += THREADS)
-                atomicAdd(reinterpret_cast<unsigned long long*>(v.acc + (long long)(s_rep[r / 3].d * v.R + s_rep[r / 3].slot) * 3 + r % 3), (unsigned long long)s_acc[r]);
+            {
+                // Gaussian Ef: the accumulator holds SP * (sum of g_i over up spins) - (SP / 2) * (sum of g_i over the planes held)
+                const long long val = (KIND == 1 && r % 3 == 1) ? s_acc[r] / (long long)(kResSP / 2) : s_acc[r];
+                atomicAdd(reinterpret_cast<unsigned long long*>(v.acc + (long long)(s_rep[r / 3].d * v.R + s_rep[r / 3].slot) * 3 + r % 3), (unsigned long long)val);
+            }
     }
     RES_STAMP(5);
 #ifndef RFIM_DBG_NOEXCH
