@@ -182,6 +182,11 @@ int rfim_pt_thermal_observables(rfim_pt* h, int64_t skip, double* absM, double* 
 int rfim_pt_get_exchange_counts(rfim_pt* h, int d, uint64_t* attempted, uint64_t* accepted);
 /* device acceptance table entry as the 33-bit threshold of DESIGN.md S3 (bimodal only) */
 int rfim_pt_get_bimodal_threshold(rfim_pt* h, int d, int rank, int k, int b, uint64_t* thr);
+/* The planning step of rfim_pt_adapt_temperatures alone (host only, no handle): ladder T[n] (ascending) with the trial's
+ * exchange rates rate[n-1] of its adjacent pairs, capacity R, a insertions -> the new ladder in out_T (room for R values),
+ * its length in *out_n.  n < R: PAPER.md:147's rule, the min(a, R-n, n-1) lowest-rate intervals (ties: lower rank) get
+ * their midpoint temperature.  n == R: DESIGN.md S8's insert-and-prune.  RFIM_EINVAL on a bad argument. */
+int rfim_pt_plan_adaptation(const double* T, const double* rate, int n, int R, int a, double* out_T, int* out_n);
 /* diag[0] kernels launched so far, [1] Gaussian attempts decided by the exact binary64 path,
  * [2] decisions within 1e-5 of a binary64 threshold (device and host exp could disagree there;
  * expected 0), [3] exchange decisions taken with a random number */

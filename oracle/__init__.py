@@ -40,6 +40,7 @@ def lib():
             "oracle_sweep": (ctypes.c_int, [ctypes.c_void_p, ctypes.c_int64, ctypes.c_int]),
             "oracle_adapt_temperatures": (ctypes.c_int, [ctypes.c_void_p, ctypes.c_int64]),
             "oracle_set_adapt_params": (ctypes.c_int, [ctypes.c_void_p, ctypes.c_int, ctypes.c_int]),
+            "oracle_plan_adaptation": (ctypes.c_int, [_dp, _dp, ctypes.c_int, ctypes.c_int, ctypes.c_int, _dp, ctypes.POINTER(ctypes.c_int)]),
             "oracle_observables": (ctypes.c_int, [ctypes.c_void_p, _dp, _dp, _dp]),
             "oracle_get_spins": (ctypes.c_int, [ctypes.c_void_p, ctypes.c_int, _i8p]),
             "oracle_get_spins_slot": (ctypes.c_int, [ctypes.c_void_p, ctypes.c_int, _i8p]),
@@ -76,6 +77,20 @@ def philox4x32_10(key, ctr):
     out = (ctypes.c_uint32 * 4)()
     lib().oracle_philox4x32_10(key[0], key[1], ctr[0], ctr[1], ctr[2], ctr[3], out)
     return [int(v) for v in out]
+
+
+def plan_adaptation(T, rate, R, a):
+    """The planning step of the adaptation alone (S8): ladder T with interval exchange rates
+    `rate`, capacity R, a insertions -> the new ladder."""
+    T = np.ascontiguousarray(T, dtype=np.float64)
+    rate = np.ascontiguousarray(rate, dtype=np.float64)
+    assert len(rate) == len(T) - 1
+    out = np.zeros(R, dtype=np.float64)
+    n = ctypes.c_int()
+    rc = lib().oracle_plan_adaptation(_ptr(T, _dp), _ptr(rate, _dp), len(T), R, a, _ptr(out, _dp), ctypes.byref(n))
+    if rc:
+        raise OracleError(f"oracle_plan_adaptation failed ({rc})")
+    return out[:n.value].copy()
 
 
 def threshold_from_x(x):

@@ -82,6 +82,57 @@ uint64_t threshold_from_x(double x) {
 
 struct Measurement { int64_t Eb, Ef, Msum; };
 
+// The planning step of the adaptation (PAPER.md:147-153 + DESIGN.md reading S8), as a pure function of the ladder and
+// the trial's exchange rates: which intervals get their midpoint temperature (split[t], t = 0..n-2) and, in the fixed-count
+// mode (n == R), which ranks are given up (removed[u]).  Oracle::adapt applies it; the tests call it directly with
+// hand-built rate vectors.
+static void plan_ladder(const std::vector<double>& T, const std::vector<double>& rate, int n, int R, int insertions,
+                        std::vector<char>& split, std::vector<char>& removed) {
+    (void)T;
+    split.assign(n > 1 ? n - 1 : 0, 0);
+    removed.assign(n, 0);
+    // the a lowest-rate intervals, ties broken by lower t (the paper's min-heap pops)
+    std::vector<int> order(n - 1);
+    for (int t = 0; t < n - 1; ++t) order[t] = t;
+    std::stable_sort(order.begin(), order.end(), [&](int a, int b) { return rate[a] < rate[b]; });
+    if (n < R) {
+        // paper rule: insert midpoints, replica count grows
+        const int a = std::min(std::min(insertions, R - n), n - 1);
+        for (int q = 0; q < a; ++q) split[order[q]] = 1;
+        return;
+    }
+    // fixed-R rule (reading G10): insert-and-prune, rank preserving
+    const int a = std::min(insertions, n - 1);
+    if (a < 1) return;
+    std::vector<char> inS(n - 1, 0);
+    std::vector<int> S;
+    for (int q = 0; q < a; ++q) { inS[order[q]] = 1; S.push_back(order[q]); }
+    // rho = the largest rate among the intervals to be split.  Removing rank u merges intervals
+    // u-1 and u; its rate is predicted (conservatively) as r1*r2*min(r1,r2); u is eligible only
+    // if that prediction stays above rho, so a move never creates an interval worse than those it fixes.
+    const double rho = rate[S.back()];
+    auto score = [&](int u) {
+        const double r1 = rate[u - 1], r2 = rate[u];
+        return (r1 * r2) * std::min(r1, r2);
+    };
+    std::vector<int> cand;
+    for (int u = 1; u <= n - 2; ++u)
+        if (!inS[u - 1] && !inS[u] && score(u) > rho) cand.push_back(u);
+    // highest score first, ties broken by larger u
+    std::stable_sort(cand.begin(), cand.end(), [&](int p, int q) {
+        if (score(p) != score(q)) return score(p) > score(q);
+        return p > q;
+    });
+    int n_removed = 0;
+    for (int u : cand) {
+        if (n_removed == a) break;
+        if (removed[u - 1] || removed[u + 1]) continue;   // never two adjacent
+        removed[u] = 1;
+        n_removed += 1;
+    }
+    for (int q = 0; q < n_removed; ++q) split[S[q]] = 1;  // shrink the insertions if candidates ran out
+}
+
 struct Oracle {
     int L = 0, R = 0, n = 0, kind = 0;       // R = capacity (slots), n = active temperatures
     int64_t N = 0;
@@ -270,17 +321,12 @@ struct Oracle {
             if (att[t] == 0) { err = "no exchange attempts in trial"; return -2; }
             rate[t] = (double)acc[t] / (double)att[t];
         }
-        // the a lowest-rate intervals, ties broken by lower t (the paper's min-heap pops)
-        std::vector<int> order(n - 1);
-        for (int t = 0; t < n - 1; ++t) order[t] = t;
-        std::stable_sort(order.begin(), order.end(), [&](int a, int b) { return rate[a] < rate[b]; });
+        std::vector<char> split, removed;
+        plan_ladder(T, rate, n, R, insertions, split, removed);
         std::vector<double> newT;
         std::vector<int32_t> new_t2r;
         if (n < R) {
             // paper rule: insert midpoints, replica count grows
-            const int a = std::min(std::min(insertions, R - n), n - 1);
-            std::vector<char> split(n - 1, 0);
-            for (int q = 0; q < a; ++q) split[order[q]] = 1;
             int next_slot = n;                               // slots n..R-1 are the pre-allocated pool
             for (int t = 0; t < n; ++t) {
                 newT.push_back(T[t]);
@@ -294,36 +340,6 @@ struct Oracle {
             }
         } else {
             // fixed-R rule (reading G10): insert-and-prune, rank preserving
-            const int a = std::min(insertions, n - 1);
-            std::vector<char> inS(n - 1, 0);
-            std::vector<int> S;
-            for (int q = 0; q < a; ++q) { inS[order[q]] = 1; S.push_back(order[q]); }
-            // rho = the largest rate among the intervals to be split.  Removing rank u merges intervals
-            // u-1 and u; its rate is predicted (conservatively) as r1*r2*min(r1,r2); u is eligible only
-            // if that prediction stays above rho, so a move never creates an interval worse than those it fixes.
-            const double rho = rate[S.back()];
-            auto score = [&](int u) {
-                const double r1 = rate[u - 1], r2 = rate[u];
-                return (r1 * r2) * std::min(r1, r2);
-            };
-            std::vector<int> cand;
-            for (int u = 1; u <= n - 2; ++u)
-                if (!inS[u - 1] && !inS[u] && score(u) > rho) cand.push_back(u);
-            // highest score first, ties broken by larger u
-            std::stable_sort(cand.begin(), cand.end(), [&](int p, int q) {
-                if (score(p) != score(q)) return score(p) > score(q);
-                return p > q;
-            });
-            std::vector<char> removed(n, 0);
-            int n_removed = 0;
-            for (int u : cand) {
-                if (n_removed == a) break;
-                if (removed[u - 1] || removed[u + 1]) continue;   // never two adjacent
-                removed[u] = 1;
-                n_removed += 1;
-            }
-            std::vector<char> split(n - 1, 0);
-            for (int q = 0; q < n_removed; ++q) split[S[q]] = 1;  // shrink the insertions if candidates ran out
             for (int t = 0; t < n; ++t) {
                 if (!removed[t]) newT.push_back(T[t]);
                 if (t < n - 1 && split[t]) newT.push_back((T[t] + T[t + 1]) / 2.0);
@@ -430,6 +446,22 @@ int oracle_set_temperatures(void* p, const double* T, int n) {
 int oracle_sweep(void* p, int64_t n_sweeps, int exchange_every) { return ((Oracle*)p)->do_sweeps(n_sweeps, exchange_every); }
 
 int oracle_adapt_temperatures(void* p, int64_t trial_sweeps) { return ((Oracle*)p)->adapt(trial_sweeps); }
+
+// The planning step alone (no state): new ladder for ladder T[n] with interval rates rate[n-1], capacity R, a insertions.
+// out_T has room for R values; returns the new count in *out_n.  Inserted temperatures are midpoints (reading G5).
+int oracle_plan_adaptation(const double* T, const double* rate, int n, int R, int a, double* out_T, int* out_n) {
+    if (!T || !rate || !out_T || !out_n || n < 2 || n > R) return -1;
+    std::vector<double> Tv(T, T + n), rv(rate, rate + n - 1);
+    std::vector<char> split, removed;
+    plan_ladder(Tv, rv, n, R, a, split, removed);
+    int m = 0;
+    for (int t = 0; t < n; ++t) {
+        if (!removed[t]) out_T[m++] = Tv[t];
+        if (t < n - 1 && split[t]) out_T[m++] = (Tv[t] + Tv[t + 1]) / 2.0;
+    }
+    *out_n = m;
+    return 0;
+}
 
 int oracle_set_adapt_params(void* p, int exchange_every, int insertions) {
     Oracle* o = (Oracle*)p;

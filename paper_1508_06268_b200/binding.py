@@ -76,6 +76,7 @@ SIGNATURES = {
     "rfim_pt_get_exchange_counts": (ctypes.c_int, [_vp, ctypes.c_int, _u64p, _u64p]),
     "rfim_pt_get_bimodal_threshold": (ctypes.c_int, [_vp, ctypes.c_int, ctypes.c_int, ctypes.c_int, ctypes.c_int, _u64p]),
     "rfim_pt_get_diagnostics": (ctypes.c_int, [_vp, _u64p]),
+    "rfim_pt_plan_adaptation": (ctypes.c_int, [_dp, _dp, ctypes.c_int, ctypes.c_int, ctypes.c_int, _dp, ctypes.POINTER(ctypes.c_int)]),
     "rfim_pt_bench_philox": (ctypes.c_int, [_vp, ctypes.c_int, _dp, _dp]),
     "rfim_pt_bench_stream": (ctypes.c_int, [_vp, ctypes.c_size_t, _dp, _dp]),
 }
@@ -359,6 +360,18 @@ class RfimPT:
         d = (ctypes.c_uint64 * 4)()
         self._ck(load().rfim_pt_get_diagnostics(self._h, d))
         return {"launches": int(d[0]), "exact_path": int(d[1]), "ulp_ambiguous": int(d[2]), "exchange_draws": int(d[3])}
+
+
+def plan_adaptation(T, rate, R, a):
+    """rfim_pt_plan_adaptation: the host-side planning step of the temperature adaptation, no handle, no GPU."""
+    T = np.ascontiguousarray(T, dtype=np.float64)
+    rate = np.ascontiguousarray(rate, dtype=np.float64)
+    out = np.zeros(R, dtype=np.float64)
+    n = ctypes.c_int()
+    rc = load().rfim_pt_plan_adaptation(_p(T, _dp), _p(rate, _dp), len(T), R, a, _p(out, _dp), ctypes.byref(n))
+    if rc:
+        raise RfimPtError(rc, "rfim_pt_plan_adaptation")
+    return out[:n.value].copy()
 
 
 def bench_philox(calls_per_thread=2000, stream=None):

@@ -1267,6 +1267,16 @@ int rfim_pt_get_bimodal_threshold(rfim_pt* h, int d, int rank, int k, int b, uin
     return RFIM_OK;
 }
 
+int rfim_pt_plan_adaptation(const double* T, const double* rate, int n, int R, int a, double* out_T, int* out_n) {
+    if (!T || !rate || !out_T || !out_n || n < 2 || n > R || a < 0) return RFIM_EINVAL;
+    const std::vector<double> Tv(T, T + n), rv(rate, rate + n - 1);
+    const AdaptPlan plan = plan_adaptation(Tv, rv, n, R, a);
+    if ((int)plan.T.size() > R) return RFIM_EINVAL;
+    for (size_t i = 0; i < plan.T.size(); ++i) out_T[i] = plan.T[i];
+    *out_n = (int)plan.T.size();
+    return RFIM_OK;
+}
+
 int rfim_pt_get_diagnostics(rfim_pt* h, uint64_t diag[4]) {
     if (!h || !diag) return RFIM_EINVAL;
     unsigned long long d4[4];

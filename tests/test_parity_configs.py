@@ -103,7 +103,7 @@ def test_cfg4_first_100_sweeps_and_later_segment():
     g.sweep(1900, w.exchange_every)
     _snapshot_into_oracle(g, o)
     g.sweep(20, w.exchange_every); o.sweep(20, w.exchange_every)
-    for r in range(0, w.R, 7):
+    for r in range(w.R):
         assert np.array_equal(g.get_spins_slot(r), o.get_spins_slot(r)), r
     assert np.array_equal(g.get_permutation(), o.get_permutation())
     d = g.diagnostics()
@@ -112,6 +112,23 @@ def test_cfg4_first_100_sweeps_and_later_segment():
     E, M, rate = g.observables()
     assert sorted(g.get_permutation()) == list(range(w.R))
     assert np.all(np.abs(M) <= 1.0) and np.all(E / w.N > -3.0 - 2.0 * 5.0) and np.all(np.diff(E) > -0.05 * w.N)
+
+
+def test_cfg4_size_bimodal_field_100_sweeps():
+    """The paper's own field (bimodal +-1) at config 4's size and partition (148 CTAs x 55-56 planes, runs
+    crossing replica seams): the 32-bit table look-up specialisation (no zero threshold) of the resident kernel."""
+    from paper_1508_06268_b200 import binding
+    w = _cfg("cfg4")
+    g, o = make_pair(w.L, w.R, w.J, 1.0, binding.BIMODAL, 7, w.temperatures())
+    for _ in range(2):
+        g.sweep(50, w.exchange_every); o.sweep(50, w.exchange_every)
+        assert_same_state(g, o, what="cfg4-size bimodal")
+    assert_same_series(g, o)
+    # and with a ladder cold enough to produce zero thresholds (the 64-bit look-up specialisation)
+    T = np.concatenate([[0.05, 0.08], w.temperatures()[2:]])
+    g.set_temperatures(T); o.set_temperatures(T)
+    g.sweep(20, w.exchange_every); o.sweep(20, w.exchange_every)
+    assert_same_state(g, o, what="cfg4-size bimodal, zero thresholds")
 
 
 def test_cfg5_batched_disorder_members():
