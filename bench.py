@@ -42,6 +42,7 @@ def parse():
                          "of 24 B per replica per exchange step)")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-e2e", action="store_true")
+    ap.add_argument("--no-secondary", action="store_true", help="skip the secondary workloads (config 5 int8 / bit-packed, config 3, sustained config 4)")
     return ap.parse_args()
 
 
@@ -56,7 +57,7 @@ class ClockSampler:
     def start(self):
         try:
             self.proc = subprocess.Popen(["nvidia-smi", "-i", str(self.index), "--query-gpu=" + self.Q,
-                                          "--format=csv,noheader,nounits", "-lms", "100"],
+                                          "--format=csv,noheader,nounits", "-lms", "25"],
                                          stdout=subprocess.PIPE, stderr=subprocess.DEVNULL, text=True)
             self.thread = threading.Thread(target=self._read, daemon=True)
             self.thread.start()
@@ -233,20 +234,34 @@ def main():
     bytes_per_attempt = 2.0 if args.packing == 8 else 0.25
     hbm_bound = hbm_peak / bytes_per_attempt                                  # attempts/ns if HBM were the limit
     bound = min(philox_bound, hbm_bound)
-    roofline = {"bound": "alu", "achieved": sweep_rate, "peak": bound, "unit": UNIT, "frac": sweep_rate / bound,
-                # DRAM bytes of one launch of the dominant kernel from the committed `ncu --set full` capture of this
-                # command at config 4 (profiles/r1_res_sweep_full.md: 35.2 MB read + 2.2 MB written; the write-back of the
-                # run is still in L2 when the kernel ends); algorithmic = every int8 spin read once and written once per launch
-                "traffic": 37.45e6 if (wl.name == "cfg4" and args.packing == 8 and world == 1) else None,
+    # The issue-rate bound DESIGN.md section 6 derives for a Philox4x32-10 stream on one SM sub-partition: one call = 18.25
+    # IMAD.WIDE (warp-uniform products hoisted) + 21 three-input XORs, each holding the integer issue port for 2 cycles
+    # -> 4 attempts per (18.25 + 21) * 2 cycles per lane-slot ... expressed per SM: 32 lanes * 4 sub-partitions * 4 attempts
+    clocks_mhz = clocks.get("sm_mhz") or float(peaks.get("sm_max_mhz", 1965.0))
+    n_sm = torch.cuda.get_device_properties(local_rank).multi_processor_count
+    philox_theory = 32.0 * 4 * 4 / ((18.25 + 21.0) * 2.0) * n_sm * clocks_mhz * 1e-3          # attempts/ns
+    traffic, traffic_source = None, None
+    try:
+        cap = json.load(open(os.path.join(ROOT, "profiles", "r2_res_sweep_full.json")))
+        if wl.name == cap.get("workload") and args.packing == cap.get("packing_bits", 8) and world == 1:
+            traffic = float(cap["dram_bytes_read"]) + float(cap["dram_bytes_write"])
+            traffic_source = f"profiles/r2_res_sweep_full.json (ncu --set full capture at commit {cap.get('commit')}; not measured in this run)"
+    except Exception:
+        pass
+    roofline = {"bound": "alu" if philox_bound <= hbm_bound else "hbm", "achieved": sweep_rate, "peak": bound, "unit": UNIT,
+                "frac": sweep_rate / bound,
+                "traffic": traffic, "traffic_source": traffic_source,
                 "traffic_unit": "bytes per launch (ncu dram__bytes_read.sum + dram__bytes_write.sum)",
                 "algorithmic_bytes_per_launch": 2.0 * wl.N * wl.R * wl.D / (8 if args.packing == 1 else 1),
-                "kernel": "sweep (both colours), timed alone with CUDA events over the same steps",
-                "philox_bound_measured": philox_bound, "hbm_bound": hbm_bound,
+                "kernel": "k_sweep_res, sweeps only (exchange_every = 0), timed alone with CUDA events over the same steps",
+                "philox_bound_measured": philox_bound, "philox_bound_issue_model": philox_theory,
+                "frac_vs_issue_model": sweep_rate / min(philox_theory, hbm_bound), "hbm_bound": hbm_bound,
                 "hbm_peak_gbs": hbm_peak, "hbm_peak_source": "MEASURED_PEAKS.json" if peaks else "fallback 6650 GB/s",
                 "stream_rmw_gbs_this_run": stream_gbs,
                 "algorithmic_bytes_per_attempt": bytes_per_attempt,
                 "achieved_algorithmic_gbs": sweep_rate * bytes_per_attempt,
-                "whole_step_frac": (value / world) / bound}
+                "whole_step_frac": (value / world) / bound,
+                "whole_step_frac_vs_issue_model": (value / world) / min(philox_theory, hbm_bound)}
 
     line = {"metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps, "warmup": max(args.warmup, 3),
             "ms_per_step": total_ms / args.steps, "higher_is_better": True, "scaling": "strong" if replicas else "weak", "vs_baseline": None,
@@ -258,6 +273,59 @@ def main():
                        "parallelism": "1 GPU" if world == 1 else (f"replicas of one realisation over {world} GPUs, all-gather of energy terms per exchange step"
                                                                      if replicas else f"{world} independent realisations, one per GPU")},
             "clocks": clocks, "gpu_launches": int(l1 - l0), "wall_s_timed_region": t_wall, "roofline": roofline}
+
+    # secondary workloads ("also reported for config 5 int8 and bit-packed"), each with its own device timing
+    if world == 1 and not args.no_secondary:
+        def timed_other(h, kk, n_steps, do_flush=True):
+            for _ in range(3):
+                h.sweep(kk, kk)
+            ev = [(torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)) for _ in range(n_steps)]
+            for a, b in ev:
+                if do_flush:
+                    flush.zero_()
+                a.record(); h.sweep(kk, kk); b.record()
+            torch.cuda.synchronize()
+            return float(sum(a.elapsed_time(b) for a, b in ev)) / n_steps
+
+        def entry(w2, ms_step, extra=None):
+            att = float(w2.N) * w2.R * w2.D * w2.exchange_every
+            e = {"workload": f"{w2.name}: L={w2.L} R={w2.R} D={w2.D} {'Gaussian' if w2.field_kind else 'bimodal'} h={w2.h} exchange_every={w2.exchange_every}",
+                 "value": att / (ms_step * 1e6), "unit": UNIT, "ms_per_step": ms_step, "frac": att / (ms_step * 1e6) / bound,
+                 "step": f"{w2.exchange_every} sweeps + energy reduction + 1 exchange step, L2 flushed between steps"}
+            e.update(extra or {})
+            return e
+
+        secondary = {}
+        n_sec = max(5, min(args.steps, 20))
+        if wl.name == "cfg4" and args.packing == 8:
+            # the production protocol: ONE call of rfim_pt_sweep(10^4, 10), no flush, CUDA events around it, clocks sampled
+            s2 = ClockSampler(local_rank); s2.start()
+            a, b = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+            a.record(); g.sweep(wl.sweeps, k); b.record(); torch.cuda.synchronize()
+            c2 = s2.stop()
+            ms_run = a.elapsed_time(b)
+            att = float(wl.N) * wl.R * wl.sweeps
+            secondary["cfg4_sustained"] = {"workload": f"cfg4: one rfim_pt_sweep({wl.sweeps}, {k}) call, no L2 flush", "value": att / (ms_run * 1e6),
+                                           "unit": UNIT, "ms_total": ms_run, "ms_per_step": ms_run / (wl.sweeps / k),
+                                           "frac": att / (ms_run * 1e6) / bound, "clocks": c2}
+        w5 = workloads.CONFIGS["cfg5"]
+        h5 = binding.RfimPT(w5.L, w5.R, w5.J, w5.h, w5.field_kind, seeds=list(w5.seeds))
+        h5.set_temperatures(w5.temperatures())
+        secondary["cfg5_u8"] = entry(w5, timed_other(h5, w5.exchange_every, n_sec), {"dtype": "u8"})
+        h5.set_packing(1)
+        secondary["cfg5_u1"] = entry(w5, timed_other(h5, w5.exchange_every, n_sec), {"dtype": "u1", "note": "spins bit-packed in HBM"})
+        h5.close()
+        w3 = workloads.CONFIGS["cfg3"]
+        h3 = binding.RfimPT(w3.L, w3.R, w3.J, w3.h, w3.field_kind, seed=w3.seeds[0])
+        h3.set_temperatures(w3.temperatures())
+        secondary["cfg3"] = entry(w3, timed_other(h3, w3.exchange_every, n_sec), {"dtype": "u8"})
+        h3.close()
+        w2 = workloads.CONFIGS["cfg2"]
+        h2 = binding.RfimPT(w2.L, w2.R, w2.J, w2.h, w2.field_kind, seed=w2.seeds[0])
+        h2.set_temperatures(w2.temperatures())
+        secondary["cfg2"] = entry(w2, timed_other(h2, w2.exchange_every, n_sec), {"dtype": "u8"})
+        h2.close()
+        line["secondary"] = secondary
 
     # end to end through the C ABI with HOST buffers, every step: H2D of every lattice (the step's input state) from pinned
     # memory, the step, D2H of every lattice and of the observables (the step's result).  Timed twice: with the bit-packed

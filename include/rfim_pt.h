@@ -132,10 +132,12 @@ const char* rfim_pt_last_error(rfim_pt* h);
  * L is 32 or 64 and the kernel variant is 0 or 4; a later sweep fails with RFIM_EINVAL if the active planes do
  * not fit in shared memory.  Getters/setters keep their int8 +-1 interface in both modes. */
 int rfim_pt_set_packing(rfim_pt* h, int bits);
-/* which sweep implementation runs: 0 = automatic (default), 1 site, 2 word, 3 flow, 4 resident. */
+/* which sweep implementation runs: 0 = automatic (default), 1 site, 2 word, 3 flow, 4 resident, 5 small-lattice
+ * (one CTA per replica, whole lattice in shared memory). */
 int rfim_pt_set_kernel_variant(rfim_pt* h, int variant);
 /* tuning knobs (tests use them to force many-CTA partitions on small problems): key 0 = replicas per
- * work item of the flow kernel (1..64), key 1 = CTA limit of the resident kernel (0 = one per SM). */
+ * work item of the flow kernel (1..64), key 1 = CTA limit of the resident kernel (0 = one per SM), key 2 = partition
+ * of the resident kernel (0 automatic, 1 equal runs of planes, 2 whole replicas per CTA where they fit). */
 int rfim_pt_set_tuning(rfim_pt* h, int key, int value);
 /* exchange period used by adapt's trial (default 10) and insertions per trial
  * (default 4, Fig. 6; the paper recommends 1-5). */

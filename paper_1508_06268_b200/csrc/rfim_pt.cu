@@ -18,6 +18,7 @@
 #include "philox.cuh"
 #include "sweep_flow.cuh"
 #include "sweep_res.cuh"
+#include "sweep_small.cuh"
 #include "view.h"
 
 using namespace rfim;
@@ -71,6 +72,7 @@ struct rfim_pt {
     uint32_t res_epoch = 0;
     bool terms_fresh = false;         // View::last holds the energy terms of the CURRENT lattices (last call ended on an exchange step)
     int res_grid_limit = 0;           // 0 = one CTA per SM
+    int res_partition = 0;            // resident kernel: 0 automatic, 1 equal runs of planes, 2 whole replicas per CTA
     int sm_count = 0, smem_optin = 0;
     std::string err;
 };
@@ -316,7 +318,8 @@ int ensure_stage(rfim_pt* h, size_t bytes) {
 }
 
 // ---- launches ------------------------------------------------------------------------------
-// kernel variants: 0 automatic, 1 site kernel, 2 word kernel, 3 flow kernel, 4 resident kernel (3, 4: L = 32 or 64)
+// kernel variants: 0 automatic, 1 site kernel, 2 word kernel, 3 flow kernel, 4 resident kernel (3, 4: L = 32 or 64),
+// 5 small-lattice kernel (one CTA per replica, whole lattice in shared memory: L % 8 == 0, L^3 bytes resident)
 bool flow_supported(const rfim_pt* h) { return h->L == 32 || h->L == 64; }
 
 // the resident kernel's partition of the D*n*L planes over the grid, and whether the largest run fits in shared memory
@@ -326,7 +329,7 @@ int iterated(const rfim_pt* h) {
     return std::max(0, std::min(h->n, h->slot0 + h->Rs) - h->slot0);
 }
 
-struct ResPlan { int grid, total, q, rem, cap_planes, cap_reps, nd, groups; size_t smem; bool ok; };
+struct ResPlan { int grid, total, q, rem, cap_planes, cap_reps, nd, groups; size_t smem; bool ok; bool aligned; };
 // plan for `nd` members per launch
 ResPlan res_plan_nd(const rfim_pt* h, int nd) {
     ResPlan p{};
@@ -335,9 +338,30 @@ ResPlan res_plan_nd(const rfim_pt* h, int nd) {
     if (!flow_supported(h) || h->n < 1 || iterated(h) < 1 || h->sm_count < 1) return p;
     p.grid = std::min(h->sm_count, kResMaxGrid);
     if (h->res_grid_limit > 0) p.grid = std::min(p.grid, h->res_grid_limit);
-    const long long total = (long long)nd * iterated(h) * h->L;
+    const long long nrep = (long long)nd * iterated(h);
+    const long long total = nrep * h->L;
     if (total > (long long)p.grid * 32767) return p;
     p.total = (int)total;
+    // Small problems (fewer than 2.5 replicas' worth of planes per CTA on average -- measured crossover at L = 32, see
+    // profiles/r2_partition_scan.md): whole replicas per CTA instead of equal runs of planes.
+    // A CTA then has no z-neighbour in another CTA at all -- no halo through L2, no progress words, no waiting on a
+    // neighbour every phase -- and holds L planes' worth of tasks per phase instead of a handful; the price is that only
+    // ceil(nrep / k) SMs work.  (this is also the regime each GPU of a replica split ends up in.)
+    const int mode = h->res_partition;                      // 0 automatic, 1 equal runs, 2 replica-aligned
+    const bool fits_whole = h->L <= res_max_planes(h->L);
+    if (fits_whole && (mode == 2 || (mode == 0 && 2 * total < 5LL * p.grid * h->L))) {
+        const int k = (int)((nrep + p.grid - 1) / p.grid);  // replicas per CTA
+        if ((long long)k * h->L <= res_max_planes(h->L)) {
+            p.aligned = true;
+            p.q = k * h->L; p.rem = 0;
+            p.grid = (int)((nrep + k - 1) / k);
+            p.cap_planes = p.q;
+            p.cap_reps = k;
+            p.smem = res_smem_bytes(h->L, p.cap_reps);
+            p.ok = p.smem <= (size_t)h->smem_optin;
+            return p;
+        }
+    }
     p.q = p.total / p.grid; p.rem = p.total % p.grid;
     p.cap_planes = p.q + (p.rem ? 1 : 0);
     if (p.cap_planes > res_max_planes(h->L)) return p;
@@ -360,11 +384,17 @@ ResPlan res_plan(const rfim_pt* h) {
     return p;
 }
 
+bool small_supported(const rfim_pt* h) {
+    return h->v.W > 0 && h->packing == 8 && small_smem_bytes(h->N) <= (size_t)h->smem_optin && (long long)h->D * h->R <= 65535;
+}
+
 int chosen_variant(const rfim_pt* h) {
-    if (h->packing == 1 || h->shard) return 4;  // only the resident kernel reads the bit layout / visits a slot window
+    if (h->packing == 1) return 4;              // only the resident kernel reads the bit layout
+    if (h->shard) return flow_supported(h) ? 4 : (small_supported(h) ? 5 : 4);   // kernels that visit a slot window
     if (h->variant != 0) return h->variant;
     if (res_plan(h).ok) return 4;
     if (flow_supported(h)) return 3;
+    if (small_supported(h)) return 5;
     return h->v.W > 0 ? 2 : 1;
 }
 
@@ -465,7 +495,7 @@ int launch_res(rfim_pt* h, int sweeps, bool measure, bool* exchanged) {
         rp.phases = 2 * sweeps;
         rp.measure = measure ? 1 : 0;
         rp.exchange = *exchanged ? 1 : 0;
-        rp.nact = pl.q > 0 ? pl.grid : pl.rem;
+        rp.nact = pl.q > 0 ? pl.grid : pl.rem;       // CTAs that own planes (a replica-aligned plan sizes the grid to them)
         rp.xstep = (uint32_t)h->xstep;
         rp.xrow = h->series_steps;
         rp.ticket = h->res_prog + kResMaxGrid;       // the word after the progress words (zeroed at create, left at zero)
@@ -490,6 +520,36 @@ int launch_res(rfim_pt* h, int sweeps, bool measure, bool* exchanged) {
         }
         if (rc) return rc;
     }
+    return RFIM_OK;
+}
+
+// `sweeps` (<= 127) sweeps of every active replica in ONE launch of the small-lattice kernel, with the measurement and (single
+// handle, small batch) the exchange step inside
+int launch_small(rfim_pt* h, int sweeps, bool measure, bool* exchanged) {
+    *exchanged = false;
+    const int nrep = h->D * iterated(h);
+    if (nrep == 0) return RFIM_OK;                      // this shard stores no active slot
+    SmallParams sp{};
+    sp.phases = 2 * sweeps;
+    sp.measure = measure ? 1 : 0;
+    *exchanged = measure && h->D <= kResFusedExchangeMaxD && !h->shard;
+    sp.exchange = *exchanged ? 1 : 0;
+    sp.xstep = (uint32_t)h->xstep;
+    sp.xrow = h->series_steps;
+    sp.ticket = h->res_prog + kResMaxGrid;
+    sp.sweep0 = (uint32_t)h->sweep_g;
+    const int words = (int)(h->Nh / 4);
+    const int threads = std::min(kSmallMaxThreads, std::max(32, (words + 31) / 32 * 32));
+    const size_t smem = small_smem_bytes(h->N);
+    if (h->kind == RFIM_FIELD_BIMODAL) {
+        CU(cudaFuncSetAttribute(k_sweep_small<0>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
+        k_sweep_small<0><<<nrep, threads, smem, h->stream>>>(h->v, sp);
+    } else {
+        CU(cudaFuncSetAttribute(k_sweep_small<1>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
+        k_sweep_small<1><<<nrep, threads, smem, h->stream>>>(h->v, sp);
+    }
+    h->launches += 1;
+    CU(cudaGetLastError());
     return RFIM_OK;
 }
 
@@ -541,7 +601,7 @@ int do_sweeps(rfim_pt* h, int64_t n_sweeps, int k) {
         if (rc) return rc;
     }
     const int variant = chosen_variant(h);
-    const bool flow = variant == 3 || variant == 4;
+    const bool flow = variant == 3 || variant == 4 || variant == 5;
     int64_t left = n_sweeps;
     while (left > 0) {
         int64_t chunk = 1;
@@ -552,13 +612,15 @@ int do_sweeps(rfim_pt* h, int64_t n_sweeps, int k) {
         // the resident kernel measures in the same launch when its chunk ends on an exchange step
         const bool step_after = k > 0 && ((h->sweep_g + (uint64_t)chunk) % (uint64_t)k) == 0;
         bool exchanged = false;
-        int rc = variant == 4 ? launch_res(h, (int)chunk, step_after, &exchanged) : (flow ? launch_flow(h, (int)chunk) : launch_sweep(h));
+        int rc = variant == 4 ? launch_res(h, (int)chunk, step_after, &exchanged)
+               : variant == 5 ? launch_small(h, (int)chunk, step_after, &exchanged)
+               : (flow ? launch_flow(h, (int)chunk) : launch_sweep(h));
         if (rc) return rc;
         h->sweep_g += (uint64_t)chunk;
         left -= chunk;
         h->terms_fresh = step_after;                 // the lattices changed; an exchange step right now measures them
         if (step_after) {
-            if (variant != 4 && (rc = launch_reduce(h))) return rc;
+            if (variant != 4 && variant != 5 && (rc = launch_reduce(h))) return rc;
             if ((rc = gather_terms(h))) return rc;
             if (!exchanged && (rc = launch_exchange(h))) return rc;
             h->series_steps += 1;
@@ -849,7 +911,8 @@ int rfim_pt_set_packing(rfim_pt* h, int bits) {
 
 int rfim_pt_set_kernel_variant(rfim_pt* h, int variant) {
     if (!h) return RFIM_EINVAL;
-    if (variant < 0 || variant > 4) return fail(h, RFIM_EINVAL, "unknown kernel variant");
+    if (variant < 0 || variant > 5) return fail(h, RFIM_EINVAL, "unknown kernel variant");
+    if (variant == 5 && !small_supported(h)) return fail(h, RFIM_EINVAL, "small-lattice kernel needs L % 8 == 0 and L^3 bytes of shared memory");
     if (h->packing == 1 && variant != 0 && variant != 4) return fail(h, RFIM_EINVAL, "bit-packed storage is read by the resident kernel only");
     if (variant == 4 && !flow_supported(h)) return fail(h, RFIM_EINVAL, "resident kernel needs L = 32 or 64");
     if (variant == 2 && h->v.W == 0) return fail(h, RFIM_EINVAL, "word kernel needs L % 8 == 0");
@@ -862,6 +925,7 @@ int rfim_pt_set_tuning(rfim_pt* h, int key, int value) {
     if (!h) return RFIM_EINVAL;
     if (key == 0 && value >= 1 && value <= 64) { h->flow_rr = value; return RFIM_OK; }
     if (key == 1 && value >= 0 && value <= kResMaxGrid) { h->res_grid_limit = value; return RFIM_OK; }
+    if (key == 2 && value >= 0 && value <= 2) { h->res_partition = value; return RFIM_OK; }
     return fail(h, RFIM_EINVAL, "unknown tuning key or value out of range");
 }
 

@@ -529,8 +529,8 @@ __global__ void __launch_bounds__(THREADS, 1) k_sweep_res(const View v, const Re
     // (fewer exact-rule fall-backs), so the longer runs do not also carry the dearer planes
     const int nshort = (int)gridDim.x - rp.rem;                      // CTAs with rp.q planes
     const int start = b * rp.q + max(0, b - nshort);
-    const int count = rp.q + (b >= nshort ? 1 : 0);
-    if (count == 0) return;
+    const int count = min(rp.q + (b >= nshort ? 1 : 0), rp.total_planes - start);   // (a replica-aligned plan: the last CTA takes what is left)
+    if (count <= 0) return;
     const int E = count * LH;                   // rows in use (per colour and class)
     const int nb = (E + 31) / 32;               // 32-row blocks
 

@@ -15,15 +15,16 @@ pytestmark = pytest.mark.gpu
 BIMODAL, GAUSSIAN = 0, 1
 
 
-@pytest.mark.parametrize("L,R,grid", [(32, 5, 0), (32, 5, 7), (64, 3, 0), (64, 3, 5)])
+@pytest.mark.parametrize("L,R,grid,partition", [(32, 5, 0, 1), (32, 5, 7, 1), (64, 3, 0, 1), (64, 3, 5, 1), (32, 5, 0, 2), (32, 5, 3, 0)])
 @pytest.mark.parametrize("kind,h", [(BIMODAL, 2.0), (GAUSSIAN, 1.5)])
-def test_packed_storage_bit_exact(L, R, grid, kind, h):
+def test_packed_storage_bit_exact(L, R, grid, partition, kind, h):
     """pack at the start, sweep with exchanges in several launch shapes, compare everything with the oracle."""
     T = geometric_ladder(0.9, 5.5, R)
     g, o = make_pair(L, R, 1.0, h, kind, 23, T)
     g.set_packing(1)
     if grid:
         g.set_tuning(1, grid)
+    g.set_tuning(2, partition)               # 1: equal runs of planes (seams, halos through L2); 2 / 0: whole replicas per CTA
     for r in range(R):                       # the conversion kept the initial state
         assert np.array_equal(g.get_spins_slot(r), o.get_spins_slot(r))
     for n, k in ((3, 0), (10, 5), (7, 2)):

@@ -77,7 +77,8 @@ def _run_sharded(L, R, n, kind, h, seed, T, world, program, packing=8):
     return shards
 
 
-@pytest.mark.parametrize("L,R,n,world", [(32, 6, 6, 2), (32, 8, 7, 4), (64, 4, 4, 2), (32, 5, 5, 3), (32, 8, 4, 4)])
+@pytest.mark.parametrize("L,R,n,world", [(32, 6, 6, 2), (32, 8, 7, 4), (64, 4, 4, 2), (32, 5, 5, 3), (32, 8, 4, 4),
+                                         (16, 6, 6, 2), (8, 8, 7, 4)])     # small lattices: the one-CTA-per-replica kernel visits the slot window
 @pytest.mark.parametrize("kind,h", [(BIMODAL, 2.0), (GAUSSIAN, 1.5)])
 def test_sharded_run_equals_oracle(L, R, n, world, kind, h):
     import oracle

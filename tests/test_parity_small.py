@@ -28,7 +28,9 @@ def test_initial_state_field_and_tables(L, kind):
 
 
 @pytest.mark.parametrize("L,R,variant", [(2, 3, 1), (4, 4, 1), (6, 5, 1), (8, 6, 1), (8, 6, 2), (10, 3, 1), (12, 4, 1),
-                                         (16, 9, 2), (16, 9, 1), (24, 5, 2), (32, 3, 2), (40, 2, 2)])
+                                         (16, 9, 2), (16, 9, 1), (24, 5, 2), (32, 3, 2), (40, 2, 2),
+                                         # variant 5: one CTA per replica, whole lattice in shared memory, one launch per exchange period
+                                         (8, 6, 5), (16, 9, 5), (24, 5, 5), (32, 3, 5), (40, 2, 5)])
 @pytest.mark.parametrize("kind,h", [(BIMODAL, 1.0), (BIMODAL, 2.0), (GAUSSIAN, 1.5)])
 def test_sweeps_with_exchange_bit_exact(L, R, variant, kind, h):
     T = np.geomspace(0.8, 5.0, R)
@@ -239,15 +241,18 @@ def test_flow_kernel_batch_and_reference_kernels_agree():
 
 
 # ---- the shared-memory-resident kernel (variant 4; L = 32 or 64) ------------------------------------------
-@pytest.mark.parametrize("L,R,grid", [(32, 5, 0), (32, 5, 7), (32, 3, 148), (64, 3, 0), (64, 3, 5), (64, 2, 4)])
+@pytest.mark.parametrize("L,R,grid,partition", [(32, 5, 0, 1), (32, 5, 7, 1), (32, 3, 148, 1), (64, 3, 0, 1), (64, 3, 5, 1), (64, 2, 4, 1),
+                                                # whole replicas per CTA (the automatic choice for small problems): one, two, ragged last CTA
+                                                (32, 5, 0, 2), (32, 5, 3, 2), (32, 7, 2, 2), (32, 5, 0, 0)])
 @pytest.mark.parametrize("kind,h", [(BIMODAL, 2.0), (GAUSSIAN, 1.5)])
-def test_resident_kernel_bit_exact(L, R, grid, kind, h):
-    # grid limits force runs of many planes per CTA, runs that cross replica seams, odd plane counts (ragged
-    # last 32-row block at L = 32) and the one-plane-per-CTA extreme
+def test_resident_kernel_bit_exact(L, R, grid, partition, kind, h):
+    # equal runs (partition 1): grid limits force runs of many planes per CTA, runs that cross replica seams, odd plane
+    # counts (ragged last 32-row block at L = 32) and the one-plane-per-CTA extreme.  Partition 2: whole replicas per CTA.
     T = np.geomspace(0.8, 5.0, R)
     g, o = make_pair(L, R, 1.0, h, kind, 31 * L + R, T)
     g.set_kernel_variant(4)
     g.set_tuning(1, grid)
+    g.set_tuning(2, partition)
     for chunk, k in [(1, 0), (4, 2), (3, 3), (7, 5)]:
         g.sweep(chunk, k); o.sweep(chunk, k)
         assert_same_state(g, o, what=f"resident L={L} grid={grid} after chunk {chunk},{k}")
@@ -262,6 +267,7 @@ def test_resident_kernel_extreme_temperatures_and_long_launch(kind):
     g, o = make_pair(32, 5, 1.0, 1.3, kind, 5, T)
     g.set_kernel_variant(4)
     g.set_tuning(1, 11)
+    g.set_tuning(2, 1)
     g.sweep(6, 2); o.sweep(6, 2)
     assert_same_state(g, o, what="resident extreme T")
     g.sweep(130, 0); o.sweep(130, 0)
@@ -272,7 +278,7 @@ def test_resident_kernel_batch_n_less_than_R_and_flow_kernel_agree():
     from paper_1508_06268_b200 import binding
     seeds = [11, 12, 13]
     T = np.geomspace(1.0, 6.0, 5)                                      # n = 5 < R = 6
-    a = binding.RfimPT(32, 6, 1.0, 1.5, GAUSSIAN, seeds=seeds); a.set_kernel_variant(4); a.set_tuning(1, 9)
+    a = binding.RfimPT(32, 6, 1.0, 1.5, GAUSSIAN, seeds=seeds); a.set_kernel_variant(4); a.set_tuning(1, 9); a.set_tuning(2, 1)
     b = binding.RfimPT(32, 6, 1.0, 1.5, GAUSSIAN, seeds=seeds); b.set_kernel_variant(3)
     a.set_temperatures(T); b.set_temperatures(T)
     a.sweep(12, 4); b.sweep(12, 4)
