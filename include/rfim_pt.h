@@ -67,15 +67,34 @@ int rfim_pt_create_batch(rfim_pt** out, int L, int R, double J, double h, int fi
  *   stream           the handle's CUDA stream (cudaStream_t): the collective must be ordered after the work already
  *                    enqueued on it and before work enqueued later (e.g. ncclAllGather on that stream, in place)
  * returning 0 on success.  The pointer stays owned by the library.  Restrictions: D = 1; slot0 a multiple of nslots;
- * only the resident kernel visits a slot window (L = 32 or 64); an adaptation step that INSERTS replicas would copy a
- * lattice to another rank and returns RFIM_EINVAL (the fixed-count, rank-preserving mode works: no lattice moves);
- * rfim_pt_get/set_spins_slot accept the stored slots only and rfim_pt_get/set_spins_all move the nslots stored
- * lattices. */
+ * the kernels that visit a slot window are the resident one (L = 32 or 64) and the small-lattice one (L % 8 == 0);
+ * rfim_pt_get/set_spins_slot accept the stored slots only and rfim_pt_get/set_spins_all move the nslots stored lattices.
+ *
+ * rfim_pt_create_shard_rr deals the slots round-robin instead: rank g of G stores slots g, g + G, g + 2G, ...
+ * (ceil(R/G) of them, padded like the windows).  This is PAPER.md:153's placement -- "new replica i goes to GPU i mod k" --
+ * for every slot, so the replicas an adaptation inserts (pool slots n, n+1, ...) spread over the ranks instead of filling
+ * the last window.  The gather function then receives a rank-major copy of the term array (same arguments, local_offset =
+ * rank * local_bytes); everything else is as for windows.
+ *
+ * An adaptation step that INSERTS replicas (n < R) copies the colder neighbour's lattice into the new
+ * replica's pool slot, which may live on another rank: the library then calls the broadcast function, once per inserted
+ * replica and on every rank in the same order,
+ *   buffer_device    device pointer, `bytes` = L^3 / 8 bytes: one lattice, bit-packed in natural site order
+ *   root_rank        the rank whose buffer holds the lattice; on return every rank's buffer must hold it
+ *   stream           the handle's CUDA stream (e.g. ncclBroadcast on that stream, in place)
+ * returning 0 on success.  Without one, an inserting step on a shard returns RFIM_ESTATE (the fixed-count mode moves no
+ * lattice and needs none). */
 typedef int (*rfim_pt_gather_fn)(void* user, void* terms_device, size_t local_offset, size_t local_bytes,
                                  size_t total_bytes, void* stream);
+typedef int (*rfim_pt_bcast_fn)(void* user, void* buffer_device, size_t bytes, int root_rank, void* stream);
 int rfim_pt_create_shard(rfim_pt** out, int L, int R, double J, double h, int field_kind, uint64_t seed,
                          int slot0, int nslots);
+int rfim_pt_create_shard_rr(rfim_pt** out, int L, int R, double J, double h, int field_kind, uint64_t seed,
+                            int rank, int world);
 int rfim_pt_set_gather(rfim_pt* h, rfim_pt_gather_fn fn, void* user);
+int rfim_pt_set_broadcast(rfim_pt* h, rfim_pt_bcast_fn fn, void* user);
+/* this rank, the number of ranks, first stored slot, slot stride (1: window, G: round-robin), stored slots (any may be NULL) */
+int rfim_pt_get_shard_layout(rfim_pt* h, int* rank, int* world, int* first_slot, int* stride, int* nslots);
 /* slot window and the energy-term array the gather function completes (any output pointer may be NULL) */
 int rfim_pt_get_shard(rfim_pt* h, int* slot0, int* nslots, void** terms_device, size_t* terms_bytes);
 
@@ -142,6 +161,10 @@ int rfim_pt_set_tuning(rfim_pt* h, int key, int value);
 /* exchange period used by adapt's trial (default 10) and insertions per trial
  * (default 4, Fig. 6; the paper recommends 1-5). */
 int rfim_pt_set_adapt_params(rfim_pt* h, int exchange_every, int insertions);
+/* exchange rates of the adjacent pairs measured by the trial run of the LAST rfim_pt_adapt_temperatures call, i.e. the
+ * rates its update was decided on (Figure 9 plots their min / avg / max per trial): rate[0 .. *n_pairs),
+ * n_pairs = (replicas before that update) - 1.  RFIM_ESTATE before the first adaptation. */
+int rfim_pt_get_trial_rates(rfim_pt* h, int d, double* rate, int* n_pairs);
 
 /* ---- extensions used by tests and the benchmark (state must be observable to be compared) -- */
 

@@ -28,6 +28,7 @@ _GATHER_FN = ctypes.CFUNCTYPE(ctypes.c_int, ctypes.c_void_p, ctypes.c_void_p, ct
                               ctypes.c_void_p)
 _ALLOC_FN = ctypes.CFUNCTYPE(ctypes.c_void_p, ctypes.c_size_t)
 _FREE_FN = ctypes.CFUNCTYPE(None, ctypes.c_void_p)
+_BCAST_FN = ctypes.CFUNCTYPE(ctypes.c_int, ctypes.c_void_p, ctypes.c_void_p, ctypes.c_size_t, ctypes.c_int, ctypes.c_void_p)
 
 # every symbol include/rfim_pt.h declares: name -> (restype, argtypes)
 SIGNATURES = {
@@ -37,7 +38,12 @@ SIGNATURES = {
                                             ctypes.c_double, ctypes.c_int, ctypes.c_int, _u64p]),
     "rfim_pt_create_shard": (ctypes.c_int, [ctypes.POINTER(_vp), ctypes.c_int, ctypes.c_int, ctypes.c_double, ctypes.c_double,
                                             ctypes.c_int, ctypes.c_uint64, ctypes.c_int, ctypes.c_int]),
+    "rfim_pt_create_shard_rr": (ctypes.c_int, [ctypes.POINTER(_vp), ctypes.c_int, ctypes.c_int, ctypes.c_double, ctypes.c_double,
+                                               ctypes.c_int, ctypes.c_uint64, ctypes.c_int, ctypes.c_int]),
     "rfim_pt_set_gather": (ctypes.c_int, [_vp, _GATHER_FN, _vp]),
+    "rfim_pt_set_broadcast": (ctypes.c_int, [_vp, _BCAST_FN, _vp]),
+    "rfim_pt_get_shard_layout": (ctypes.c_int, [_vp, _ip, _ip, _ip, _ip, _ip]),
+    "rfim_pt_get_trial_rates": (ctypes.c_int, [_vp, ctypes.c_int, _dp, _ip]),
     "rfim_pt_get_shard": (ctypes.c_int, [_vp, _ip, _ip, ctypes.POINTER(_vp), ctypes.POINTER(ctypes.c_size_t)]),
     "rfim_pt_destroy": (ctypes.c_int, [_vp]),
     "rfim_pt_set_temperatures": (ctypes.c_int, [_vp, _dp, ctypes.c_int]),
@@ -138,7 +144,7 @@ def _p(a, t):
 class RfimPT:
     """Handle on D realisations x R replica slots of an L^3 lattice (see include/rfim_pt.h)."""
 
-    def __init__(self, L, R, J, h, field_kind, seed=None, seeds=None, torch_allocator=True, torch_stream=True, shard=None):
+    def __init__(self, L, R, J, h, field_kind, seed=None, seeds=None, torch_allocator=True, torch_stream=True, shard=None, shard_rr=None):
         lib = load()
         if torch_allocator:
             import torch
@@ -149,7 +155,13 @@ class RfimPT:
         self._h = _vp()
         self.shard = shard
         self._gather_ref = None
-        if shard is not None:             # (slot0, nslots): this handle stores that window of the R slots
+        self._bcast_ref = None
+        if shard_rr is not None:          # (rank, world): this handle stores slots rank, rank + world, ...
+            rc = lib.rfim_pt_create_shard_rr(ctypes.byref(self._h), L, R, J, h, field_kind, int(seed), int(shard_rr[0]), int(shard_rr[1]))
+            self.D = 1
+            shard = (int(shard_rr[0]), -(-R // int(shard_rr[1])))
+            self.shard = shard
+        elif shard is not None:           # (slot0, nslots): this handle stores that window of the R slots
             rc = lib.rfim_pt_create_shard(ctypes.byref(self._h), L, R, J, h, field_kind, int(seed), int(shard[0]), int(shard[1]))
             self.D = 1
         elif seeds is None:
@@ -238,6 +250,38 @@ class RfimPT:
                 return 1
         self._gather_ref = _GATHER_FN(_thunk)       # keep the thunk alive as long as the handle
         self._ck(load().rfim_pt_set_gather(self._h, self._gather_ref, None))
+
+    def set_broadcast(self, fn):
+        """fn(buffer_device_ptr, nbytes, root_rank, stream_ptr) -> None: hands one bit-packed lattice from its owner to every
+        rank (include/rfim_pt.h; used when an adaptation step inserts a replica on a shard)."""
+        def _thunk(user, buf, nbytes, root, stream):
+            try:
+                fn(buf, nbytes, root, stream)
+                return 0
+            except Exception:
+                import traceback
+                traceback.print_exc()
+                return 1
+        self._bcast_ref = _BCAST_FN(_thunk)
+        self._ck(load().rfim_pt_set_broadcast(self._h, self._bcast_ref, None))
+
+    def get_shard_layout(self):
+        v = [ctypes.c_int() for _ in range(5)]
+        self._ck(load().rfim_pt_get_shard_layout(self._h, *[ctypes.byref(x) for x in v]))
+        return dict(zip(("rank", "world", "first_slot", "stride", "nslots"), (x.value for x in v)))
+
+    def stored_slot_ids(self):
+        """Global slot indices of the lattices this handle stores, in storage order."""
+        lay = self.get_shard_layout()
+        return [lay["first_slot"] + j * lay["stride"] for j in range(lay["nslots"]) if lay["first_slot"] + j * lay["stride"] < self.R]
+
+    def get_trial_rates(self, d=0):
+        """Exchange rates measured by the trial run of the last adapt_temperatures call (the rates its update used)."""
+        n = ctypes.c_int()
+        self._ck(load().rfim_pt_get_trial_rates(self._h, d, None, ctypes.byref(n)))
+        rate = np.zeros(n.value, dtype=np.float64)
+        self._ck(load().rfim_pt_get_trial_rates(self._h, d, _p(rate, _dp), ctypes.byref(n)))
+        return rate
 
     def get_shard(self):
         a, b, ptr, nb = ctypes.c_int(), ctypes.c_int(), _vp(), ctypes.c_size_t()

@@ -1,6 +1,6 @@
 // kernels_ref.cuh -- the straightforward device kernels: one thread per site (any even L) and one
 // thread per 4-site word (L % 8 == 0), one launch per colour.  They are the in-library reference
-// the tuned kernels (sweep_fast.cuh) are checked against, and they serve every lattice size the
+// the tuned kernels (sweep_res.cuh, sweep_small.cuh, sweep_flow.cuh) are checked against, and they serve every lattice size the
 // tuned kernels do not.  All decisions follow DESIGN.md S2-S6.
 #pragma once
 #include <cstdint>
@@ -154,7 +154,7 @@ __global__ void k_sweep_word(View v, int colour, uint32_t sweep) {
 
 // ---- initial spins (S2, domain 3): one thread per site in natural order ---------------
 __global__ void k_init_spins(View v) {
-    const int d = blockIdx.y / v.Rs, slot = v.slot0 + blockIdx.y % v.Rs;      // grid.y = D * (stored slots per member)
+    const int d = blockIdx.y / v.Rs, slot = v.stored_slot(blockIdx.y % v.Rs);   // grid.y = D * (stored slots per member)
     const uint32_t k0 = v.keys[2 * d], k1 = v.keys[2 * d + 1];
     const int L = v.L, Lh = v.Lh;
     uint8_t* base = v.spins + (long long)blockIdx.y * 2 * v.Nh;
@@ -286,9 +286,9 @@ __device__ __forceinline__ long long warp_sum(long long x) {
 __global__ void k_reduce_site(View v) {
     const int d = blockIdx.y / v.n, t = blockIdx.y % v.n;
     const int slot = v.t2r[d * v.R + t];
-    if (slot < v.slot0 || slot >= v.slot0 + v.Rs) return;                     // a replica shard reduces the slots it stores
+    if (!v.stores(slot)) return;                                              // a replica shard reduces the slots it stores
     const long long Nh = v.Nh;
-    const uint8_t* c0 = v.spins + (long long)(d * v.Rs + slot - v.slot0) * 2 * Nh;
+    const uint8_t* c0 = v.spins + (long long)(d * v.Rs + v.stored_index(slot)) * 2 * Nh;
     const uint8_t* c1 = c0 + Nh;
     const long long f0 = (long long)d * 2 * Nh, f1 = f0 + Nh;
     const int L = v.L, Lh = v.Lh;
@@ -379,12 +379,10 @@ __global__ void k_thermal_moments(View v, long long skip, long long steps, doubl
     const int d = blockIdx.x / v.n, t = blockIdx.x % v.n;
     __shared__ double part[5][256];
     double a[5] = {0, 0, 0, 0, 0};
-    const double invN = 1.0 / (double)v.N;
     for (long long q = skip + threadIdx.x; q < steps; q += blockDim.x) {
         const long long* s = v.series + ((q * v.D + d) * v.R + t) * 3;
         const double E = __dsub_rn(__dmul_rn(-v.J, (double)s[0]), __dmul_rn(v.hs, (double)s[1]));
         const double e = E / (double)v.N, m = (double)s[2] / (double)v.N;
-        (void)invN;
         a[0] += e; a[1] += e * e; a[2] += fabs(m); a[3] += m * m; a[4] += (m * m) * (m * m);
     }
     for (int j = 0; j < 5; ++j) part[j][threadIdx.x] = a[j];

@@ -49,11 +49,19 @@ struct rfim_pt {
     View v{};
     std::vector<void*> owned;         // every device allocation, released in destroy
     int8_t* stage = nullptr;          // device staging for spin import/export
-    int slot0 = 0, Rs = 0;            // stored slot window (replica shard: [slot0, slot0 + Rs) of R; else 0, R)
+    int slot0 = 0, Rs = 0;            // stored slots (replica shard: slot0 + j * sstride, j < Rs; else 0, R)
+    int sstride = 1;                  // 1: contiguous window; G: round-robin deal over G ranks
+    int rank = 0, world = 1;          // replica shard: this rank, number of ranks
     bool shard = false;
     rfim_pt_gather_fn gather = nullptr;   // shard: completes View::acc across ranks before an exchange step
     void* gather_user = nullptr;
+    rfim_pt_bcast_fn bcast = nullptr;     // shard: hands one lattice from its owner to every rank (inserting adaptation)
+    void* bcast_user = nullptr;
+    long long* terms_all = nullptr;   // round-robin shard: [world][Rs][3] rank-major copy of the energy terms for the all-gather
+    std::vector<double> trial_rates;  // [D][R]: exchange rates of the last adaptation trial (rfim_pt_get_trial_rates)
+    int trial_n = 0;
     size_t acc_rows = 0;              // rows of View::acc (>= R; padded to a whole number of shards)
+    double* moments_dev = nullptr;    // thermal moments scratch (rfim_pt_thermal_moments)
     uint8_t* unpacked = nullptr;      // packed mode: byte-layout scratch for the stand-alone reduction (allocated on first use)
     size_t stage_bytes = 0;
     uint64_t sweep_g = 0, xstep = 0;
@@ -174,9 +182,9 @@ int upload_field(rfim_pt* h, int d) {
             for (int z = 0; z < L; ++z) for (int y = 0; y < L; ++y) for (int x = 0; x < L; ++x)
                 fr[res_field_index(h, x, y, z)] = f[x + (long long)L * (y + (long long)L * z)] > 0 ? 0x80 : 0x00;
             CU(cudaMemcpyAsync(h->fieldb_res + (long long)d * h->N, fr.data(), h->N, cudaMemcpyHostToDevice, h->stream));
-            CU(cudaStreamSynchronize(h->stream));
+            CU(cudaStreamSynchronize(h->stream));         // fr goes out of scope
         }
-        CU(cudaStreamSynchronize(h->stream));
+        CU(cudaStreamSynchronize(h->stream));             // fb goes out of scope (a no-op after the one above)
         h->amax[d] = std::fabs(hs);
     } else {
         std::vector<float> fa(h->N);
@@ -326,7 +334,10 @@ bool flow_supported(const rfim_pt* h) { return h->L == 32 || h->L == 64; }
 // replicas one sweep of this handle visits: every active rank, or the active slots a shard stores (active slots are 0 .. n-1)
 int iterated(const rfim_pt* h) {
     if (!h->shard) return h->n;
-    return std::max(0, std::min(h->n, h->slot0 + h->Rs) - h->slot0);
+    // active slots are 0 .. n-1; the stored ones among them are the first ones of the window
+    const int below = h->n - h->slot0;                        // slots slot0 + j * sstride < n  <=>  j < below / sstride (rounded up)
+    if (below <= 0) return 0;
+    return std::min(h->Rs, (below + h->sstride - 1) / h->sstride);
 }
 
 struct ResPlan { int grid, total, q, rem, cap_planes, cap_reps, nd, groups; size_t smem; bool ok; bool aligned; };
@@ -553,14 +564,38 @@ int launch_small(rfim_pt* h, int sweeps, bool measure, bool* exchanged) {
     return RFIM_OK;
 }
 
+// round-robin shard: slot s = j * G + r is row j of rank r
+__global__ void k_terms_pack(const long long* __restrict__ acc, long long* __restrict__ all, int rank, int Rs, int G) {
+    const int i = blockIdx.x * blockDim.x + threadIdx.x;
+    if (i < Rs * 3) all[((long long)rank * Rs + i / 3) * 3 + i % 3] = acc[((long long)(i / 3) * G + rank) * 3 + i % 3];
+}
+__global__ void k_terms_unpack(long long* __restrict__ acc, const long long* __restrict__ all, int Rs, int G) {
+    const int i = blockIdx.x * blockDim.x + threadIdx.x;
+    if (i < G * Rs * 3) {
+        const int c = i % 3, j = (i / 3) % Rs, r = i / (3 * Rs);
+        acc[((long long)j * G + r) * 3 + c] = all[i];
+    }
+}
+
 // replica shard: every rank now holds the energy terms of the slots it stores; the caller-supplied collective fills in
 // the rows of the other ranks (an all-gather of 24 bytes per slot) so that every rank takes the same
 // exchange decisions.  Runs on the handle's stream.
 int gather_terms(rfim_pt* h) {
     if (!h->shard) return RFIM_OK;
     if (!h->gather) return fail(h, RFIM_ESTATE, "replica shard: no gather function set (rfim_pt_set_gather)");
-    const int rc = h->gather(h->gather_user, h->v.acc, (size_t)h->slot0 * 24, (size_t)h->Rs * 24, h->acc_rows * 24, h->stream);
+    if (h->sstride == 1) {
+        const int rc = h->gather(h->gather_user, h->v.acc, (size_t)h->slot0 * 24, (size_t)h->Rs * 24, h->acc_rows * 24, h->stream);
+        if (rc) return fail(h, RFIM_ECUDA, "replica shard: the gather function failed");
+        return RFIM_OK;
+    }
+    // round-robin deal: this rank's rows rank, rank + G, ... are gathered through a rank-major copy (contiguous per rank)
+    const int cells = h->world * h->Rs * 3;
+    k_terms_pack<<<(h->Rs * 3 + 127) / 128, 128, 0, h->stream>>>(h->v.acc, h->terms_all, h->rank, h->Rs, h->world);
+    const int rc = h->gather(h->gather_user, h->terms_all, (size_t)h->rank * h->Rs * 24, (size_t)h->Rs * 24, (size_t)h->world * h->Rs * 24, h->stream);
     if (rc) return fail(h, RFIM_ECUDA, "replica shard: the gather function failed");
+    k_terms_unpack<<<(cells + 127) / 128, 128, 0, h->stream>>>(h->v.acc, h->terms_all, h->Rs, h->world);
+    h->launches += 2;
+    CU(cudaGetLastError());
     return RFIM_OK;
 }
 
@@ -677,7 +712,7 @@ int check_member(rfim_pt* h, int d) {
     return RFIM_OK;
 }
 
-int create_impl(rfim_pt** out, int L, int R, double J, double hh, int kind, int D, const uint64_t* seeds, int slot0 = 0, int nslots = -1) {
+int create_impl(rfim_pt** out, int L, int R, double J, double hh, int kind, int D, const uint64_t* seeds, int slot0 = 0, int nslots = -1, int sstride = 1) {
     if (!out) return RFIM_EINVAL;
     *out = nullptr;
     if (L < 2 || (L & 1) || L > 1024 || R < 1 || R > 4096 || D < 1 || D > 4096 || !seeds) return RFIM_EINVAL;
@@ -686,11 +721,15 @@ int create_impl(rfim_pt** out, int L, int R, double J, double hh, int kind, int 
     int ndev = 0;
     if (cudaGetDeviceCount(&ndev) != cudaSuccess || ndev < 1) return RFIM_ECUDA;   // no CPU fallback
     const bool shard = nslots >= 0;
-    if (shard && (D != 1 || slot0 < 0 || nslots < 1 || slot0 >= R || slot0 % nslots != 0)) return RFIM_EINVAL;
+    if (shard && (D != 1 || slot0 < 0 || nslots < 1 || slot0 >= R || sstride < 1)) return RFIM_EINVAL;
+    if (shard && sstride == 1 && slot0 % nslots != 0) return RFIM_EINVAL;                       // contiguous windows, ordered by rank
+    if (shard && sstride > 1 && (slot0 >= sstride || nslots != (R + sstride - 1) / sstride)) return RFIM_EINVAL;   // round-robin deal
     rfim_pt* h = new rfim_pt();
     h->L = L; h->R = R; h->D = D; h->kind = kind; h->J = J; h->h = hh;
-    h->shard = shard; h->slot0 = shard ? slot0 : 0; h->Rs = shard ? nslots : R;
-    h->acc_rows = shard ? (size_t)((R + nslots - 1) / nslots) * nslots : (size_t)R;
+    h->shard = shard; h->slot0 = shard ? slot0 : 0; h->Rs = shard ? nslots : R; h->sstride = shard ? sstride : 1;
+    h->acc_rows = !shard ? (size_t)R : (sstride == 1 ? (size_t)((R + nslots - 1) / nslots) * nslots : (size_t)sstride * nslots);
+    h->rank = !shard ? 0 : (sstride == 1 ? slot0 / nslots : slot0);
+    h->world = !shard ? 1 : (sstride == 1 ? (int)(h->acc_rows / nslots) : sstride);
     h->N = (long long)L * L * L; h->Nh = h->N / 2;
     h->seeds.assign(seeds, seeds + D);
     h->field_nat.assign((size_t)D * h->N, 0);
@@ -701,7 +740,7 @@ int create_impl(rfim_pt** out, int L, int R, double J, double hh, int kind, int 
     v.W = (L % 8 == 0) ? L / 8 : 0;
     v.N = h->N; v.Nh = h->Nh;
     v.J = J; v.hs = (kind == RFIM_FIELD_BIMODAL) ? hh : hh / kFieldScale;
-    v.shard = shard ? 1 : 0; v.slot0 = h->slot0; v.Rs = h->Rs; v.n_it = 0;
+    v.shard = shard ? 1 : 0; v.slot0 = h->slot0; v.Rs = h->Rs; v.n_it = 0; v.sstride = h->sstride;
     const size_t DR = (size_t)D * R;
     int rc = RFIM_OK;
     auto A = [&](int r) { if (rc == RFIM_OK) rc = r; };
@@ -721,6 +760,7 @@ int create_impl(rfim_pt** out, int L, int R, double J, double hh, int kind, int 
     A(alloc_into(h, &v.r2t, DR));
     A(alloc_into(h, const_cast<uint32_t**>(&v.keys), (size_t)D * 2));
     A(alloc_into(h, &v.acc, (size_t)D * h->acc_rows * 3));
+    if (h->sstride > 1) A(alloc_into(h, &h->terms_all, h->acc_rows * 3));
     A(alloc_into(h, &v.last, DR * 3));
     A(alloc_into(h, &v.ework, DR));
     A(alloc_into(h, &v.att, DR));
@@ -836,6 +876,38 @@ int rfim_pt_create_batch(rfim_pt** out, int L, int R, double J, double hh, int f
 
 int rfim_pt_create_shard(rfim_pt** out, int L, int R, double J, double hh, int field_kind, uint64_t seed, int slot0, int nslots) {
     return create_impl(out, L, R, J, hh, field_kind, 1, &seed, slot0, nslots);
+}
+
+int rfim_pt_create_shard_rr(rfim_pt** out, int L, int R, double J, double hh, int field_kind, uint64_t seed, int rank, int world) {
+    if (world < 1 || rank < 0 || rank >= world || rank >= R) return RFIM_EINVAL;
+    if (world == 1) return create_impl(out, L, R, J, hh, field_kind, 1, &seed, 0, R, 1);
+    return create_impl(out, L, R, J, hh, field_kind, 1, &seed, rank, (R + world - 1) / world, world);
+}
+
+int rfim_pt_set_broadcast(rfim_pt* h, rfim_pt_bcast_fn fn, void* user) {
+    if (!h) return RFIM_EINVAL;
+    if (!h->shard) return fail(h, RFIM_EINVAL, "not a replica shard");
+    h->bcast = fn; h->bcast_user = user;
+    return RFIM_OK;
+}
+
+int rfim_pt_get_shard_layout(rfim_pt* h, int* rank, int* world, int* first_slot, int* stride, int* nslots) {
+    if (!h) return RFIM_EINVAL;
+    if (rank) *rank = h->rank;
+    if (world) *world = h->world;
+    if (first_slot) *first_slot = h->slot0;
+    if (stride) *stride = h->sstride;
+    if (nslots) *nslots = h->Rs;
+    return RFIM_OK;
+}
+
+int rfim_pt_get_trial_rates(rfim_pt* h, int d, double* rate, int* n_pairs) {
+    int rc = check_member(h, d);
+    if (rc) return rc;
+    if (h->trial_n < 2) return fail(h, RFIM_ESTATE, "no adaptation trial has run yet");
+    if (n_pairs) *n_pairs = h->trial_n - 1;
+    if (rate) std::memcpy(rate, h->trial_rates.data() + (size_t)d * h->R, (size_t)(h->trial_n - 1) * sizeof(double));
+    return RFIM_OK;
 }
 
 int rfim_pt_set_gather(rfim_pt* h, rfim_pt_gather_fn fn, void* user) {
@@ -976,11 +1048,14 @@ int rfim_pt_adapt_temperatures(rfim_pt* h, int64_t trial_sweeps) {
     CU(cudaMemcpyAsync(t2r.data(), h->v.t2r, DR * 4, cudaMemcpyDeviceToHost, h->stream));
     CU(cudaStreamSynchronize(h->stream));
     std::vector<AdaptPlan> plans(D);
+    h->trial_rates.assign(DR, 0.0);
+    h->trial_n = n;
     for (int d = 0; d < D; ++d) {
         std::vector<double> Td(h->T.begin() + (size_t)d * R, h->T.begin() + (size_t)d * R + n), rate(std::max(n - 1, 0));
         for (int t = 0; t < n - 1; ++t) {
             if (att[(size_t)d * R + t] == 0) return fail(h, RFIM_ESTATE, "a pair saw no exchange attempt in the trial");
             rate[t] = (double)acc[(size_t)d * R + t] / (double)att[(size_t)d * R + t];
+            h->trial_rates[(size_t)d * R + t] = rate[t];
         }
         plans[d] = plan_adaptation(Td, rate, n, R, h->adapt_a);
         if (plans[d].T.size() != plans[0].T.size()) return fail(h, RFIM_ESTATE, "members disagree on the new replica count");
@@ -997,12 +1072,24 @@ int rfim_pt_adapt_temperatures(rfim_pt* h, int64_t trial_sweeps) {
             } else if (p.keep_of[j] >= 0) {
                 slot = t2r[(size_t)d * R + p.keep_of[j]];
             } else {
-                if (h->shard) return fail(h, RFIM_EINVAL, "replica shard: adaptation that inserts replicas would copy lattices between ranks (use n = R)");
                 slot = next_slot++;
                 const int src = t2r[(size_t)d * R + p.copy_of[j]];
-                const size_t lat = (size_t)h->N / (h->packing == 1 ? 8 : 1);      // bytes per lattice
-                CU(cudaMemcpyAsync(h->v.spins + ((size_t)d * R + slot) * lat, h->v.spins + ((size_t)d * R + src) * lat,
-                                   lat, cudaMemcpyDeviceToDevice, h->stream));
+                if (h->shard) {
+                    // the new replica lives on the rank its pool slot belongs to (slot mod G for a round-robin
+                    // deal); its spins come from the rank that stores the colder neighbour: one broadcast of N/8 bytes
+                    if (!h->bcast) return fail(h, RFIM_ESTATE, "replica shard: inserting a replica needs the lattice broadcast (rfim_pt_set_broadcast)");
+                    if ((rc = ensure_stage(h, (size_t)h->N / 8))) return rc;
+                    uint8_t* buf = reinterpret_cast<uint8_t*>(h->stage);
+                    if (h->v.stores(src)) { k_export_bits<<<grid_for(h->N / 8, 1), 256, 0, h->stream>>>(h->v, h->v.stored_index(src), buf); h->launches += 1; }
+                    const int root = h->sstride == 1 ? src / h->Rs : src % h->world;
+                    if (h->bcast(h->bcast_user, buf, (size_t)h->N / 8, root, h->stream)) return fail(h, RFIM_ECUDA, "replica shard: the lattice broadcast failed");
+                    if (h->v.stores(slot)) { k_import_bits<<<grid_for(h->N / 8, 1), 256, 0, h->stream>>>(h->v, h->v.stored_index(slot), buf); h->launches += 1; }
+                    CU(cudaGetLastError());
+                } else {
+                    const size_t lat = (size_t)h->N / (h->packing == 1 ? 8 : 1);      // bytes per lattice
+                    CU(cudaMemcpyAsync(h->v.spins + ((size_t)d * R + slot) * lat, h->v.spins + ((size_t)d * R + src) * lat,
+                                       lat, cudaMemcpyDeviceToDevice, h->stream));
+                }
             }
             new_t2r[(size_t)d * R + j] = slot;
             h->T[(size_t)d * R + j] = p.T[j];
@@ -1053,9 +1140,9 @@ int rfim_pt_get_spins_slot(rfim_pt* h, int d, int slot, int8_t* out) {
     int rc = check_member(h, d);
     if (rc) return rc;
     if (slot < 0 || slot >= h->R || !out) return fail(h, RFIM_EINVAL, "bad slot or null buffer");
-    if (slot < h->slot0 || slot >= h->slot0 + h->Rs) return fail(h, RFIM_EINVAL, "replica shard: this rank does not store that slot");
+    if (!h->v.stores(slot)) return fail(h, RFIM_EINVAL, "replica shard: this rank does not store that slot");
     if ((rc = ensure_stage(h, (size_t)h->N))) return rc;
-    k_export_spins<<<grid_for(h->N, 1), 256, 0, h->stream>>>(h->v, d * h->Rs + slot - h->slot0, h->stage);
+    k_export_spins<<<grid_for(h->N, 1), 256, 0, h->stream>>>(h->v, d * h->Rs + h->v.stored_index(slot), h->stage);
     h->launches += 1;
     CU(cudaGetLastError());
     CU(cudaMemcpyAsync(out, h->stage, (size_t)h->N, cudaMemcpyDeviceToHost, h->stream));
@@ -1083,10 +1170,10 @@ int rfim_pt_set_spins_slot(rfim_pt* h, int d, int slot, const int8_t* in) {
     if (slot < 0 || slot >= h->R || !in) return fail(h, RFIM_EINVAL, "bad slot or null buffer");
     for (long long i = 0; i < h->N; ++i)
         if (in[i] != 1 && in[i] != -1) return fail(h, RFIM_EINVAL, "spins must be +1 or -1");
-    if (slot < h->slot0 || slot >= h->slot0 + h->Rs) return fail(h, RFIM_EINVAL, "replica shard: this rank does not store that slot");
+    if (!h->v.stores(slot)) return fail(h, RFIM_EINVAL, "replica shard: this rank does not store that slot");
     if ((rc = ensure_stage(h, (size_t)h->N))) return rc;
     CU(cudaMemcpyAsync(h->stage, in, (size_t)h->N, cudaMemcpyHostToDevice, h->stream));
-    k_import_spins<<<grid_for(h->N, 1), 256, 0, h->stream>>>(h->v, d * h->Rs + slot - h->slot0, h->stage);
+    k_import_spins<<<grid_for(h->N, 1), 256, 0, h->stream>>>(h->v, d * h->Rs + h->v.stored_index(slot), h->stage);
     h->launches += 1;
     CU(cudaGetLastError());
     CU(cudaStreamSynchronize(h->stream));
@@ -1258,17 +1345,16 @@ int thermal_moments_all(rfim_pt* h, int64_t skip, std::vector<double>& mom) {
     if (!h->have_T) return fail(h, RFIM_ESTATE, "temperatures not set");
     if (skip < 0 || skip >= h->series_steps) return fail(h, RFIM_ESTATE, "no measurement steps after `skip` (sweep with exchange_every > 0 first)");
     const size_t cnt = (size_t)h->D * h->n * 5;
-    double* dev = nullptr;
-    int rc = alloc_into(h, &dev, cnt);
-    if (rc) return rc;
-    k_thermal_moments<<<h->D * h->n, 256, 0, h->stream>>>(h->v, (long long)skip, h->series_steps, dev);
+    if (!h->moments_dev) {                              // [D][R][5], allocated on first use, released with the handle
+        int rc = alloc_into(h, &h->moments_dev, (size_t)h->D * h->R * 5);
+        if (rc) return rc;
+    }
+    k_thermal_moments<<<h->D * h->n, 256, 0, h->stream>>>(h->v, (long long)skip, h->series_steps, h->moments_dev);
     h->launches += 1;
     mom.assign(cnt, 0.0);
-    cudaError_t e1 = cudaGetLastError();
-    cudaError_t e2 = cudaMemcpyAsync(mom.data(), dev, cnt * 8, cudaMemcpyDeviceToHost, h->stream);
-    cudaError_t e3 = cudaStreamSynchronize(h->stream);
-    release(h, dev);
-    CU(e1); CU(e2); CU(e3);
+    CU(cudaGetLastError());
+    CU(cudaMemcpyAsync(mom.data(), h->moments_dev, cnt * 8, cudaMemcpyDeviceToHost, h->stream));
+    CU(cudaStreamSynchronize(h->stream));
     return RFIM_OK;
 }
 }  // namespace

@@ -327,8 +327,8 @@ __global__ void k_reduce_word(View v) {
     const int d = blockIdx.y / v.n, t = blockIdx.y % v.n;
     const int slot = v.t2r[d * v.R + t];
     const int NW = (int)(v.Nh >> 2);
-    if (slot < v.slot0 || slot >= v.slot0 + v.Rs) return;                     // a replica shard reduces the slots it stores
-    const uint32_t* c0 = reinterpret_cast<const uint32_t*>(v.spins + (long long)(d * v.Rs + slot - v.slot0) * 2 * v.Nh);
+    if (!v.stores(slot)) return;                                              // a replica shard reduces the slots it stores
+    const uint32_t* c0 = reinterpret_cast<const uint32_t*>(v.spins + (long long)(d * v.Rs + v.stored_index(slot)) * 2 * v.Nh);
     const uint32_t* c1 = c0 + NW;
     const long long f0 = (long long)d * 2 * v.Nh;
     const int L = v.L, W = v.W;

@@ -289,7 +289,7 @@ __device__ __noinline__ void res_wait_slow(const int* s_done, int eb, int b_zp, 
 struct ResPiece { uint32_t me[4], cw[4], ns[4]; };
 
 // rem: where the rows of a z-neighbour plane that lives in another CTA are found in global memory (boundary tasks only)
-struct ResRemote { const uint8_t* spins; uint32_t off_p, off_m; bool any, p, m; int packed; };
+struct ResRemote { const uint8_t* spins; size_t off_p, off_m; bool any, p, m; int packed; };   // 64-bit: the spin buffer can exceed 2^32 sites
 
 // xr: the row's words of the other colour (all K pieces, loaded once per row: the far x-neighbour of a piece's edge
 // byte is a word of the neighbouring piece, periodic in x)
@@ -304,8 +304,8 @@ __device__ __forceinline__ ResPiece res_load_piece(const uint8_t* smem, const ui
     uint4 zm = *reinterpret_cast<const uint4*>(smem + a_zm + k * ARR);
     const uint4 m = *reinterpret_cast<const uint4*>(smem + a_me + k * ARR);
     if (rem.any) {                                  // warp-uniform: only boundary tasks come here
-        if (rem.p) zp = res_piece_from_global(rem.spins, (size_t)(rem.off_p + 16u * k), rem.packed);
-        if (rem.m) zm = res_piece_from_global(rem.spins, (size_t)(rem.off_m + 16u * k), rem.packed);
+        if (rem.p) zp = res_piece_from_global(rem.spins, rem.off_p + 16u * k, rem.packed);
+        if (rem.m) zm = res_piece_from_global(rem.spins, rem.off_m + 16u * k, rem.packed);
     }
     const uint32_t edge = dir == 0 ? xr[(k + K - 1) % K].w : xr[(k + 1) % K].x;
     ResPiece pc;
@@ -392,7 +392,7 @@ struct ResLane {
 template <int KIND, int K, bool NEVER, bool UNI, bool BND, bool MEAS, bool RAGGED>
 __device__ __forceinline__ void res_row(const View& v, const ResParams& rp, uint8_t* smem, const ResLane& ln, const int s, const int c, const int DIR,
                                         const uint32_t sweep, const uint32_t dom, const ResRep* rr, const bool valid,
-                                        const bool remote_p, const bool remote_m, const uint32_t roff_p, const uint32_t roff_m,
+                                        const bool remote_p, const bool remote_m, const size_t roff_p, const size_t roff_m,
                                         long long& m_eb, long long& m_ef, long long& m_ms) {
     using G = ResGeom<K>;
     constexpr int LH = G::LH, ROWB = G::ROWB, W = G::W, ARR = G::ARR;
@@ -474,13 +474,13 @@ __device__ __forceinline__ void res_row(const View& v, const ResParams& rp, uint
         uint4 nw = make_uint4(pc.me[0], pc.me[1], pc.me[2], pc.me[3]);
         if (KIND == 1 && mn < ln.band)          // rare: some site needs the exact binary64 rule
             nw = res_gauss_piece_fix(v, make_uint4(idx8[0], idx8[1], idx8[2], idx8[3]), ln.tab_addr, ln.band, fp + 4 * k * LH, LH,
-                                     v.fieldg + (size_t)((ln.d2 + (uint32_t)c) * (uint32_t)v.Nh + grow + 16u * k), rr, q0 + 4u * k, sweep, dom);
+                                     v.fieldg + ((size_t)(ln.d2 + (uint32_t)c) * (size_t)v.Nh + grow + 16u * k), rr, q0 + 4u * k, sweep, dom);
 
         // ---- write back ---------------------------------------------------------------------------------
         if (!RAGGED || valid) {
             *reinterpret_cast<uint4*>(smem + a_me + k * ARR) = nw;
             if (BND && (remote_p || remote_m))
-                res_piece_to_global(v.spins, (size_t)((ln.ds2 + (uint32_t)c) * (uint32_t)v.Nh + grow + 16u * k), v.packed, nw);
+                res_piece_to_global(v.spins, (size_t)(ln.ds2 + (uint32_t)c) * (size_t)v.Nh + grow + 16u * k, v.packed, nw);
             if (MEAS) {
                 // the final phase (colour 1) measures both colours: its own updated words (with Eb: every bond has one
                 // colour-1 end) and the colour-0 words of the same row, xr[k], final since the phase before; their field
@@ -507,7 +507,7 @@ __device__ __forceinline__ void res_row(const View& v, const ResParams& rp, uint
 template <int KIND, int K, bool NEVER, bool UNI, bool BND, bool MEAS, bool RAGGED>
 __device__ __forceinline__ void res_task_rows(const View& v, const ResParams& rp, uint8_t* smem, const ResLane& ln, const int c,
                                               const uint32_t sweep, const uint32_t dom, const ResRep* rr, const bool valid,
-                                              const bool remote_p, const bool remote_m, const uint32_t roff_p, const uint32_t roff_m,
+                                              const bool remote_p, const bool remote_m, const size_t roff_p, const size_t roff_m,
                                               long long& m_eb, long long& m_ef, long long& m_ms) {
 #pragma unroll 1
     for (int s = 0; s < 2; ++s)
@@ -569,9 +569,9 @@ __global__ void __launch_bounds__(THREADS, 1) k_sweep_res(const View v, const Re
         const int dt = dt0 + r, d = rp.d0 + dt / v.n_it, q = dt % v.n_it;
         ResRep rr;
         rr.d = d;
-        if (v.shard) { rr.slot = v.slot0 + q; rr.tr = d * v.R + v.r2t[d * v.R + rr.slot]; }      // visit stored slots
+        if (v.shard) { rr.slot = v.stored_slot(q); rr.tr = d * v.R + v.r2t[d * v.R + rr.slot]; }   // visit stored slots
         else { rr.tr = d * v.R + q; rr.slot = v.t2r[rr.tr]; }                                  // visit ranks
-        rr.ds = d * v.Rs + rr.slot - v.slot0;
+        rr.ds = d * v.Rs + v.stored_index(rr.slot);
         rr.band = KIND == 0 ? 0.f : v.band[rr.tr];
         rr.never = KIND == 0 ? v.never[rr.tr] : 0u;
         rr.beta = v.beta[rr.tr];
@@ -584,7 +584,7 @@ __global__ void __launch_bounds__(THREADS, 1) k_sweep_res(const View v, const Re
     for (int i = tid; i < nrep * 32; i += THREADS) {
         const int r = i >> 5, idx = i & 31;
         const int dt = dt0 + r, d = rp.d0 + dt / v.n_it, q = dt % v.n_it;
-        const int tr = d * v.R + (v.shard ? v.r2t[d * v.R + v.slot0 + q] : q);
+        const int tr = d * v.R + (v.shard ? v.r2t[d * v.R + v.stored_slot(q)] : q);
         uint2 ent = make_uint2(0u, 0u);
         if (KIND == 0) {
             ent.x = v.etab[(long long)tr * 32 + idx];
@@ -650,7 +650,6 @@ __global__ void __launch_bounds__(THREADS, 1) k_sweep_res(const View v, const Re
     const int n_bblocks = s_ctl[3];
     const int total_tasks = nb * rp.phases;
     const uint32_t tab0 = (uint32_t)__cvta_generic_to_shared(s_tab);
-    const uint32_t nh32 = (uint32_t)v.Nh;
 
     // ---- the task flow ------------------------------------------------------------------------------
     constexpr bool RAGGED = (LH % 32) != 0;
@@ -722,8 +721,8 @@ __global__ void __launch_bounds__(THREADS, 1) k_sweep_res(const View v, const Re
         } else {
             // rows of a z-neighbour plane that lives in another CTA: read from global memory (class 0; class 1 = + ROWB)
             const int zq_p = (z + 1) & (L - 1), zq_m = (z - 1) & (L - 1);
-            const uint32_t roff_p = (ln.ds2 + (uint32_t)oc) * nh32 + (uint32_t)(zq_p * L + 2 * i) * ROWB;
-            const uint32_t roff_m = (ln.ds2 + (uint32_t)oc) * nh32 + (uint32_t)(zq_m * L + 2 * i) * ROWB;
+            const size_t roff_p = (size_t)(ln.ds2 + (uint32_t)oc) * (size_t)v.Nh + (uint32_t)(zq_p * L + 2 * i) * ROWB;
+            const size_t roff_m = (size_t)(ln.ds2 + (uint32_t)oc) * (size_t)v.Nh + (uint32_t)(zq_m * L + 2 * i) * ROWB;
             if (btask && !meas)
                 res_task_rows<KIND, K, NEVER, UNI, true, false, RAGGED>(v, rp, smem, ln, c, sweep, dom, rr, valid, remote_p, remote_m, roff_p, roff_m, m_eb, m_ef, m_ms);
             else

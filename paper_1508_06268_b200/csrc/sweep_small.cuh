@@ -58,9 +58,9 @@ __global__ void __launch_bounds__(kSmallMaxThreads, 1) k_sweep_small(const View 
     // which replica: by rank, or (replica shard) by stored slot -- as in sweep_res.cuh
     const int d = blockIdx.x / v.n_it, q0 = blockIdx.x % v.n_it;
     int slot, tr;
-    if (v.shard) { slot = v.slot0 + q0; tr = d * v.R + v.r2t[d * v.R + slot]; }
+    if (v.shard) { slot = v.stored_slot(q0); tr = d * v.R + v.r2t[d * v.R + slot]; }
     else { tr = d * v.R + q0; slot = v.t2r[tr]; }
-    const long long ds = (long long)d * v.Rs + slot - v.slot0;
+    const long long ds = (long long)d * v.Rs + v.stored_index(slot);
     const uint32_t k0 = v.keys[2 * d], k1 = v.keys[2 * d + 1];
     const long long fbase0 = (long long)d * 2 * v.Nh;
 

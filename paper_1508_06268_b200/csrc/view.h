@@ -38,10 +38,15 @@ struct View {
     unsigned long long* diag;      // [4], see rfim_pt_get_diagnostics
     double J, hs;                  // hs = h (bimodal) or h * 2^-20 (Gaussian)
     int packed;                    // != 0: `spins` holds one BIT per spin (bit j & 7 of byte j >> 3, same index j as the byte layout)
-    // Replica sharding: this handle STORES the slots [slot0, slot0 + Rs) of every member (all R of
-    // them when shard == 0) and a sweep visits n_it replicas: every rank t < n (shard == 0) or the active stored slots
-    // slot0 .. slot0 + n_it - 1 (shard != 0).  t2r, r2t, tables, acc, series stay global (indexed by rank / slot < R).
-    int shard, slot0, Rs, n_it;
+    // Replica sharding: this handle STORES Rs slots of every member, slot0 + j * sstride for
+    // j = 0 .. Rs-1 (all R of them when shard == 0: slot0 = 0, sstride = 1; a contiguous window: sstride = 1; a round-robin
+    // deal over G ranks: slot0 = rank, sstride = G), and a sweep visits n_it replicas: every rank t < n
+    // (shard == 0) or the first n_it stored slots, the active ones (shard != 0).  t2r, r2t, tables, acc, series stay global
+    // (indexed by rank / slot < R).
+    int shard, slot0, Rs, n_it, sstride;
+    __host__ __device__ int stored_slot(int j) const { return slot0 + j * sstride; }                     // j-th stored slot
+    __host__ __device__ bool stores(int slot) const { return slot >= slot0 && (slot - slot0) % sstride == 0 && (slot - slot0) / sstride < Rs; }
+    __host__ __device__ int stored_index(int slot) const { return (slot - slot0) / sstride; }
 };
 
 }  // namespace rfim

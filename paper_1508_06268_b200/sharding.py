@@ -51,6 +51,14 @@ def replica_window(R: int, world: int, rank: int):
     return rank * m, m
 
 
+def replica_round_robin(R: int, world: int, rank: int):
+    """Slots of rank `rank` when the R slots are dealt round-robin: rank, rank + world, ... ("replica i goes
+    to GPU i mod k").  Pass (rank, world) as `shard_rr` to binding.RfimPT; returns the slot list for bookkeeping."""
+    if rank >= R:
+        raise ValueError(f"rank {rank} of {world} would store none of the {R} slots: use fewer ranks")
+    return list(range(int(rank), int(R), int(world)))
+
+
 def all_gather_rows(terms: torch.Tensor, rank: int, world: int, group=None):
     """In-place all-gather of a [world * m, 3] int64 array whose rows [rank*m, (rank+1)*m) are valid on this rank.
     Works on any device / backend (NCCL on CUDA tensors, gloo on CPU tensors); identity for world == 1."""
@@ -80,3 +88,19 @@ def make_terms_gather(rank: int, world: int, group=None):
         assert local_offset == rank * local_bytes and total_bytes == world * local_bytes, "windows must be equal and ordered by rank"
         all_gather_rows(t, rank, world, group)
     return gather
+
+
+def make_lattice_broadcast(group=None):
+    """The function to hand to RfimPT.set_broadcast: wraps the library's lattice buffer (device memory the library owns,
+    L^3 / 8 bytes) in a tensor and broadcasts it from `root_rank` over torch.distributed on the current stream."""
+    def bcast(buf_ptr, nbytes, root_rank, stream_ptr):
+        if not (dist.is_available() and dist.is_initialized()) or dist.get_world_size(group) == 1:
+            return
+        t = torch.as_tensor(_BytePtr(buf_ptr, nbytes), device="cuda")
+        dist.broadcast(t, src=dist.get_global_rank(group, root_rank) if group is not None else root_rank, group=group)
+    return bcast
+
+
+class _BytePtr:
+    def __init__(self, ptr: int, nbytes: int):
+        self.__cuda_array_interface__ = {"shape": (int(nbytes),), "typestr": "|u1", "data": (int(ptr), False), "version": 3}

@@ -135,3 +135,55 @@ def test_replica_windows_and_terms_all_gather():
         p.join(timeout=60)
         assert p.exitcode == 0
     assert len(rows) == 4 and all(r.shape == (6, 3) for r in rows)
+
+
+# ---- round-robin deal ("replica i goes to GPU i mod k") + the lattice broadcast of an inserting adaptation ----
+def _rr_worker(rank, world, port, q):
+    """Each rank owns slots rank, rank + world, ...  It contributes its rows in the rank-major layout the library hands to the
+    gather function for a round-robin shard; after the all-gather, row (r, j) is slot j * world + r.  Then one lattice
+    travels from its owner to every rank the way rfim_pt_adapt_temperatures moves an inserted replica's spins."""
+    os.environ["MASTER_ADDR"] = "127.0.0.1"
+    os.environ["MASTER_PORT"] = str(port)
+    dist.init_process_group("gloo", rank=rank, world_size=world)
+    try:
+        R = 7
+        mine = sharding.replica_round_robin(R, world, rank)
+        m = -(-R // world)
+        terms_by_slot = np.arange(world * m * 3, dtype=np.int64).reshape(world * m, 3) * 7 + 1     # what each slot's terms are
+        rank_major = torch.zeros((world * m, 3), dtype=torch.int64)
+        for j, slot in enumerate(mine):
+            rank_major[rank * m + j] = torch.from_numpy(terms_by_slot[slot])
+        sharding.all_gather_rows(rank_major, rank, world)
+        by_slot = np.zeros_like(terms_by_slot)
+        for r in range(world):
+            for j in range(m):
+                by_slot[j * world + r] = rank_major[r * m + j].numpy()
+        ok_gather = np.array_equal(by_slot[:R], terms_by_slot[:R])
+        # the new replica of pool slot 5 copies slot 2: owner of 2 is rank 2 % world; every rank ends up with the lattice
+        src_slot, root = 2, 2 % world
+        lattice = torch.full((64,), 255 if rank == root else 0, dtype=torch.uint8)
+        dist.broadcast(lattice, src=root)
+        ok_bcast = bool((lattice == 255).all())
+        dist.barrier()
+        q.put((rank, mine, ok_gather, ok_bcast))
+    finally:
+        dist.destroy_process_group()
+
+
+def test_round_robin_deal_gather_layout_and_lattice_broadcast():
+    assert sharding.replica_round_robin(7, 2, 0) == [0, 2, 4, 6] and sharding.replica_round_robin(7, 2, 1) == [1, 3, 5]
+    assert sharding.replica_round_robin(128, 8, 3)[:3] == [3, 11, 19]      # slot i lives on rank i mod 8
+    world = 2
+    ctx = mp.get_context("spawn")
+    q = ctx.Queue()
+    port = _free_port()
+    procs = [ctx.Process(target=_rr_worker, args=(r, world, port, q)) for r in range(world)]
+    for p in procs:
+        p.start()
+    got = sorted(q.get(timeout=120) for _ in range(world))
+    for p in procs:
+        p.join(timeout=60)
+        assert p.exitcode == 0
+    slots = sorted(s for _, mine, _, _ in got for s in mine)
+    assert slots == list(range(7))                                          # every slot stored by exactly one rank
+    assert all(ok_g and ok_b for _, _, ok_g, ok_b in got)

@@ -45,10 +45,36 @@ class LoopbackGather:
         return gather
 
 
-def _run_sharded(L, R, n, kind, h, seed, T, world, program, packing=8):
+class LoopbackBroadcast:
+    """Broadcast of one lattice buffer among G handles of one process: the root publishes its buffer, everybody meets at
+    a host barrier, the others copy it (device-to-device on their own stream), a second barrier keeps the root from
+    overwriting the buffer while a peer still reads it."""
+
+    def __init__(self, world):
+        self.world = world
+        self.barrier = threading.Barrier(world)
+        self.src = None
+
+    def make(self, rank):
+        def bcast(buf_ptr, nbytes, root, stream_ptr):
+            from paper_1508_06268_b200.sharding import _BytePtr
+            t = torch.as_tensor(_BytePtr(buf_ptr, nbytes), device="cuda")
+            if rank == root:
+                torch.cuda.current_stream().synchronize()
+                self.src = t
+            self.barrier.wait()
+            if rank != root:
+                t.copy_(self.src)
+                torch.cuda.current_stream().synchronize()
+            self.barrier.wait()
+        return bcast
+
+
+def _run_sharded(L, R, n, kind, h, seed, T, world, program, packing=8, round_robin=False):
     """program(handle) runs on every shard in its own thread; returns the shard handles."""
     from paper_1508_06268_b200 import binding
     lg = LoopbackGather(world)
+    lb = LoopbackBroadcast(world)
     shards, errors = [None] * world, []
     streams = [torch.cuda.Stream() for _ in range(world)]
     _KEEP.append(streams)                                        # the handles keep using these streams after the threads end
@@ -56,8 +82,12 @@ def _run_sharded(L, R, n, kind, h, seed, T, world, program, packing=8):
     def worker(rank):
         try:
             with torch.cuda.stream(streams[rank]):
-                g = binding.RfimPT(L, R, 1.0, h, kind, seed=seed, shard=replica_window(R, world, rank))
+                if round_robin:
+                    g = binding.RfimPT(L, R, 1.0, h, kind, seed=seed, shard_rr=(rank, world))
+                else:
+                    g = binding.RfimPT(L, R, 1.0, h, kind, seed=seed, shard=replica_window(R, world, rank))
                 g.set_gather(lg.make(rank))
+                g.set_broadcast(lb.make(rank))
                 if packing != 8:
                     g.set_packing(packing)
                 g.set_temperatures(T)
@@ -67,6 +97,7 @@ def _run_sharded(L, R, n, kind, h, seed, T, world, program, packing=8):
         except Exception as e:                                   # a dead thread would leave the others at the barrier
             errors.append(e)
             lg.barrier.abort()
+            lb.barrier.abort()
 
     threads = [threading.Thread(target=worker, args=(r,)) for r in range(world)]
     for t in threads:
@@ -150,6 +181,65 @@ def test_sharded_bit_packed_and_fixed_count_adaptation():
             assert np.array_equal(g.get_spins_slot(slot), o.get_spins_slot(slot)), (rank, slot)
         assert np.array_equal(g.get_permutation(), o.get_permutation())
         g.close()
+
+
+@pytest.mark.parametrize("L,R,n0,world,round_robin", [(32, 12, 5, 2, False), (32, 12, 5, 3, True), (16, 10, 4, 2, True), (32, 9, 6, 4, True),
+                                                       (64, 6, 3, 2, True)])
+@pytest.mark.parametrize("kind,h", [(BIMODAL, 2.0), (GAUSSIAN, 1.5)])
+def test_sharded_growing_adaptation_equals_oracle(L, R, n0, world, round_robin, kind, h):
+    """the adaptation inserts replicas (pool slots n, n+1, ...; with the round-robin deal the new replica i
+    lives on rank i mod G) whose spins are copied from the colder neighbour -- across ranks through the lattice broadcast.
+    Three growing trials then a run: every stored slot, the ladder, the permutation and the series equal the oracle's."""
+    import oracle
+    T = geometric_ladder(0.9, 5.0, n0)
+    o = oracle.Oracle(L, R, 1.0, h, kind, 53)
+    o.set_temperatures(T)
+    o.set_adapt_params(3, 2)
+    for _ in range(3):
+        o.adapt_temperatures(30)
+    o.sweep(9, 3)
+
+    def program(g):
+        g.set_adapt_params(3, 2)
+        for _ in range(3):
+            g.adapt_temperatures(30)
+        g.sweep(9, 3)
+
+    shards = _run_sharded(L, R, n0, kind, h, 53, T, world, program, round_robin=round_robin)
+    n = o.n
+    assert n == min(R, n0 + 6)
+    seen = set()
+    for rank, g in enumerate(shards):
+        assert g.n == n and np.array_equal(g.get_temperatures(), o.get_temperatures())
+        for slot in g.stored_slot_ids():
+            if slot < n:
+                assert np.array_equal(g.get_spins_slot(slot), o.get_spins_slot(slot)), (rank, slot)
+                seen.add(slot)
+        assert np.array_equal(g.get_permutation(), o.get_permutation()), rank
+        assert g.get_counters() == o.get_counters()
+        for x, y in zip(g.get_timeseries(), o.get_timeseries()):
+            assert np.array_equal(x, y)
+        if round_robin:
+            assert g.stored_slot_ids() == list(range(rank, R, world))       # slot i lives on rank i mod G
+    assert seen == set(range(n))                                              # every active lattice is stored by exactly one rank
+    for g in shards:
+        g.close()
+
+
+def test_trial_rates_getter_matches_oracle_trial():
+    """rfim_pt_get_trial_rates returns the rates the last adaptation's update was decided on (Figure 9's per-trial numbers)."""
+    import oracle
+    from paper_1508_06268_b200 import binding
+    T = geometric_ladder(0.9, 5.0, 6)
+    g = binding.RfimPT(16, 10, 1.0, 1.0, BIMODAL, seed=3); g.set_temperatures(T); g.set_adapt_params(2, 2)
+    o = oracle.Oracle(16, 10, 1.0, 1.0, BIMODAL, 3); o.set_temperatures(T)
+    with pytest.raises(binding.RfimPtError):
+        g.get_trial_rates()
+    o.sweep(40, 2)                                # the trial adapt_temperatures(40) runs: statistics start from zero
+    att, acc = o.get_exchange_counts()
+    g.adapt_temperatures(40)
+    assert np.array_equal(g.get_trial_rates(), acc / att)
+    g.close(); o.close()
 
 
 def test_shard_errors():
