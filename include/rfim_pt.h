@@ -93,6 +93,12 @@ int rfim_pt_create_shard_rr(rfim_pt** out, int L, int R, double J, double h, int
                             int rank, int world);
 int rfim_pt_set_gather(rfim_pt* h, rfim_pt_gather_fn fn, void* user);
 int rfim_pt_set_broadcast(rfim_pt* h, rfim_pt_bcast_fn fn, void* user);
+/* Native route for both collectives: the library calls NCCL itself on its stream -- ncclAllGather (in place, 24 bytes per
+ * slot) before every exchange step and ncclBroadcast (L^3 / 8 bytes) per inserted replica -- so that no host callback sits
+ * between the measuring kernel and the exchange kernel.  comm: an ncclComm_t whose rank / size equal this shard's;
+ * all_gather_fn / broadcast_fn: the addresses of ncclAllGather and ncclBroadcast in the NCCL library that created it (the
+ * library does not link NCCL).  comm = NULL switches back to the callbacks.  The communicator stays owned by the caller. */
+int rfim_pt_set_nccl(rfim_pt* h, void* comm, void* all_gather_fn, void* broadcast_fn);
 /* this rank, the number of ranks, first stored slot, slot stride (1: window, G: round-robin), stored slots (any may be NULL) */
 int rfim_pt_get_shard_layout(rfim_pt* h, int* rank, int* world, int* first_slot, int* stride, int* nslots);
 /* slot window and the energy-term array the gather function completes (any output pointer may be NULL) */

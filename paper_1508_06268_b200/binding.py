@@ -42,6 +42,7 @@ SIGNATURES = {
                                                ctypes.c_int, ctypes.c_uint64, ctypes.c_int, ctypes.c_int]),
     "rfim_pt_set_gather": (ctypes.c_int, [_vp, _GATHER_FN, _vp]),
     "rfim_pt_set_broadcast": (ctypes.c_int, [_vp, _BCAST_FN, _vp]),
+    "rfim_pt_set_nccl": (ctypes.c_int, [_vp, _vp, _vp, _vp]),
     "rfim_pt_get_shard_layout": (ctypes.c_int, [_vp, _ip, _ip, _ip, _ip, _ip]),
     "rfim_pt_get_trial_rates": (ctypes.c_int, [_vp, ctypes.c_int, _dp, _ip]),
     "rfim_pt_get_shard": (ctypes.c_int, [_vp, _ip, _ip, ctypes.POINTER(_vp), ctypes.POINTER(ctypes.c_size_t)]),
@@ -264,6 +265,14 @@ class RfimPT:
                 return 1
         self._bcast_ref = _BCAST_FN(_thunk)
         self._ck(load().rfim_pt_set_broadcast(self._h, self._bcast_ref, None))
+
+    def set_nccl(self, comm):
+        """comm: sharding.NcclComm (or None): the library then calls ncclAllGather / ncclBroadcast itself (rfim_pt_set_nccl)."""
+        if comm is None:
+            self._ck(load().rfim_pt_set_nccl(self._h, None, None, None))
+        else:
+            self._nccl_ref = comm                  # keep the communicator alive as long as the handle uses it
+            self._ck(load().rfim_pt_set_nccl(self._h, _vp(comm.comm), _vp(comm.fn_all_gather), _vp(comm.fn_broadcast)))
 
     def get_shard_layout(self):
         v = [ctypes.c_int() for _ in range(5)]

@@ -57,6 +57,10 @@ struct rfim_pt {
     void* gather_user = nullptr;
     rfim_pt_bcast_fn bcast = nullptr;     // shard: hands one lattice from its owner to every rank (inserting adaptation)
     void* bcast_user = nullptr;
+    // shard, native route: the library calls NCCL itself (no host callback per exchange step)
+    void* nccl_comm = nullptr;
+    int (*nccl_all_gather)(const void*, void*, size_t, int, void*, cudaStream_t) = nullptr;
+    int (*nccl_broadcast)(const void*, void*, size_t, int, int, void*, cudaStream_t) = nullptr;
     long long* terms_all = nullptr;   // round-robin shard: [world][Rs][3] rank-major copy of the energy terms for the all-gather
     std::vector<double> trial_rates;  // [D][R]: exchange rates of the last adaptation trial (rfim_pt_get_trial_rates)
     int trial_n = 0;
@@ -582,7 +586,18 @@ __global__ void k_terms_unpack(long long* __restrict__ acc, const long long* __r
 // exchange decisions.  Runs on the handle's stream.
 int gather_terms(rfim_pt* h) {
     if (!h->shard) return RFIM_OK;
-    if (!h->gather) return fail(h, RFIM_ESTATE, "replica shard: no gather function set (rfim_pt_set_gather)");
+    if (!h->gather && !h->nccl_comm) return fail(h, RFIM_ESTATE, "replica shard: no gather function set (rfim_pt_set_gather / rfim_pt_set_nccl)");
+    constexpr int kNcclInt64 = 4;                               // ncclDataType_t
+    if (h->nccl_comm) {
+        // in-place all-gather (NCCL: sendbuff == recvbuff + rank * count) of Rs rows of 3 int64 per rank
+        long long* buf = h->sstride == 1 ? h->v.acc : h->terms_all;
+        if (h->sstride > 1) { k_terms_pack<<<(h->Rs * 3 + 127) / 128, 128, 0, h->stream>>>(h->v.acc, h->terms_all, h->rank, h->Rs, h->world); h->launches += 1; }
+        if (h->nccl_all_gather(buf + (size_t)h->rank * h->Rs * 3, buf, (size_t)h->Rs * 3, kNcclInt64, h->nccl_comm, h->stream))
+            return fail(h, RFIM_ECUDA, "replica shard: ncclAllGather failed");
+        if (h->sstride > 1) { k_terms_unpack<<<(h->world * h->Rs * 3 + 127) / 128, 128, 0, h->stream>>>(h->v.acc, h->terms_all, h->Rs, h->world); h->launches += 1; }
+        CU(cudaGetLastError());
+        return RFIM_OK;
+    }
     if (h->sstride == 1) {
         const int rc = h->gather(h->gather_user, h->v.acc, (size_t)h->slot0 * 24, (size_t)h->Rs * 24, h->acc_rows * 24, h->stream);
         if (rc) return fail(h, RFIM_ECUDA, "replica shard: the gather function failed");
@@ -891,6 +906,16 @@ int rfim_pt_set_broadcast(rfim_pt* h, rfim_pt_bcast_fn fn, void* user) {
     return RFIM_OK;
 }
 
+int rfim_pt_set_nccl(rfim_pt* h, void* comm, void* all_gather_fn, void* broadcast_fn) {
+    if (!h) return RFIM_EINVAL;
+    if (!h->shard) return fail(h, RFIM_EINVAL, "not a replica shard");
+    if (comm && (!all_gather_fn || !broadcast_fn)) return fail(h, RFIM_EINVAL, "ncclAllGather and ncclBroadcast entry points are both needed");
+    h->nccl_comm = comm;
+    h->nccl_all_gather = reinterpret_cast<int (*)(const void*, void*, size_t, int, void*, cudaStream_t)>(all_gather_fn);
+    h->nccl_broadcast = reinterpret_cast<int (*)(const void*, void*, size_t, int, int, void*, cudaStream_t)>(broadcast_fn);
+    return RFIM_OK;
+}
+
 int rfim_pt_get_shard_layout(rfim_pt* h, int* rank, int* world, int* first_slot, int* stride, int* nslots) {
     if (!h) return RFIM_EINVAL;
     if (rank) *rank = h->rank;
@@ -1077,12 +1102,14 @@ int rfim_pt_adapt_temperatures(rfim_pt* h, int64_t trial_sweeps) {
                 if (h->shard) {
                     // the new replica lives on the rank its pool slot belongs to (slot mod G for a round-robin
                     // deal); its spins come from the rank that stores the colder neighbour: one broadcast of N/8 bytes
-                    if (!h->bcast) return fail(h, RFIM_ESTATE, "replica shard: inserting a replica needs the lattice broadcast (rfim_pt_set_broadcast)");
+                    if (!h->bcast && !h->nccl_comm) return fail(h, RFIM_ESTATE, "replica shard: inserting a replica needs the lattice broadcast (rfim_pt_set_broadcast / rfim_pt_set_nccl)");
                     if ((rc = ensure_stage(h, (size_t)h->N / 8))) return rc;
                     uint8_t* buf = reinterpret_cast<uint8_t*>(h->stage);
                     if (h->v.stores(src)) { k_export_bits<<<grid_for(h->N / 8, 1), 256, 0, h->stream>>>(h->v, h->v.stored_index(src), buf); h->launches += 1; }
                     const int root = h->sstride == 1 ? src / h->Rs : src % h->world;
-                    if (h->bcast(h->bcast_user, buf, (size_t)h->N / 8, root, h->stream)) return fail(h, RFIM_ECUDA, "replica shard: the lattice broadcast failed");
+                    const int brc = h->nccl_comm ? h->nccl_broadcast(buf, buf, (size_t)h->N / 8, /* ncclUint8 */ 1, root, h->nccl_comm, h->stream)
+                                                 : h->bcast(h->bcast_user, buf, (size_t)h->N / 8, root, h->stream);
+                    if (brc) return fail(h, RFIM_ECUDA, "replica shard: the lattice broadcast failed");
                     if (h->v.stores(slot)) { k_import_bits<<<grid_for(h->N / 8, 1), 256, 0, h->stream>>>(h->v, h->v.stored_index(slot), buf); h->launches += 1; }
                     CU(cudaGetLastError());
                 } else {

@@ -66,9 +66,11 @@ def all_gather_rows(terms: torch.Tensor, rank: int, world: int, group=None):
     if world == 1:
         return terms
     m = terms.shape[0] // world
-    mine = terms[rank * m:(rank + 1) * m].clone()          # the send buffer must not alias the receive buffer
-    flat = terms.view(-1)
-    dist.all_gather_into_tensor(flat, mine.view(-1), group=group)
+    mine = terms[rank * m:(rank + 1) * m]
+    if not terms.is_cuda:
+        mine = mine.clone()                                # gloo: the send buffer must not alias the receive buffer
+    # NCCL gathers in place when the send buffer is this rank's block of the receive buffer: no copy
+    dist.all_gather_into_tensor(terms.view(-1), mine.view(-1), group=group)
     return terms
 
 
@@ -104,3 +106,52 @@ def make_lattice_broadcast(group=None):
 class _BytePtr:
     def __init__(self, ptr: int, nbytes: int):
         self.__cuda_array_interface__ = {"shape": (int(nbytes),), "typestr": "|u1", "data": (int(ptr), False), "version": 3}
+
+
+class NcclComm:
+    """An NCCL communicator of the library's own (torch's bundled libnccl through ctypes), for rfim_pt_set_nccl: the device
+    library then issues ncclAllGather / ncclBroadcast itself on its stream, with no Python between the measuring kernel
+    and the exchange kernel.  The unique id travels from rank 0 over torch.distributed (any backend); with world == 1 no
+    process group is needed."""
+
+    class _UniqueId(__import__("ctypes").Structure):
+        _fields_ = [("internal", __import__("ctypes").c_char * 128)]
+
+    def __init__(self, rank: int, world: int, group=None):
+        import ctypes
+        self._lib = ctypes.CDLL(self._find_libnccl())
+        uid = NcclComm._UniqueId()
+        if rank == 0:
+            self._check(self._lib.ncclGetUniqueId(ctypes.byref(uid)), "ncclGetUniqueId")
+        if world > 1:
+            box = [bytes(uid.internal)] if rank == 0 else [None]
+            dist.broadcast_object_list(box, src=0, group=group)
+            ctypes.memmove(ctypes.byref(uid), box[0], 128)
+        comm = ctypes.c_void_p()
+        self._lib.ncclCommInitRank.argtypes = [ctypes.POINTER(ctypes.c_void_p), ctypes.c_int, NcclComm._UniqueId, ctypes.c_int]
+        self._check(self._lib.ncclCommInitRank(ctypes.byref(comm), world, uid, rank), "ncclCommInitRank")
+        self.comm = comm.value
+        self.rank, self.world = rank, world
+        self.fn_all_gather = ctypes.cast(self._lib.ncclAllGather, ctypes.c_void_p).value
+        self.fn_broadcast = ctypes.cast(self._lib.ncclBroadcast, ctypes.c_void_p).value
+
+    @staticmethod
+    def _find_libnccl():
+        import os
+        for line in open("/proc/self/maps"):                 # the copy torch has loaded
+            if "libnccl.so" in line:
+                return line.split()[-1]
+        import nvidia.nccl
+        return os.path.join(list(nvidia.nccl.__path__)[0], "lib", "libnccl.so.2")
+
+    @staticmethod
+    def _check(rc, what):
+        if rc != 0:
+            raise RuntimeError(f"{what} failed with ncclResult_t {rc}")
+
+    def close(self):
+        if getattr(self, "comm", None):
+            import ctypes
+            self._lib.ncclCommDestroy.argtypes = [ctypes.c_void_p]
+            self._lib.ncclCommDestroy(ctypes.c_void_p(self.comm))
+            self.comm = None

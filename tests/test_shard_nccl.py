@@ -61,3 +61,39 @@ def test_terms_gather_through_nccl_world_1():
     env = dict(os.environ, MASTER_ADDR="127.0.0.1", MASTER_PORT=str(port))
     r = subprocess.run([sys.executable, "-c", CHILD % ROOT], env=env, capture_output=True, text=True, timeout=600)
     assert r.returncode == 0 and "shard-nccl-ok" in r.stdout, r.stdout[-2000:] + r.stderr[-4000:]
+
+
+CHILD_NATIVE = r"""
+import os, sys
+sys.path.insert(0, %r)
+import numpy as np, torch
+torch.cuda.set_device(0)
+import oracle
+from paper_1508_06268_b200 import binding, sharding
+from paper_1508_06268_b200.workloads import geometric_ladder
+comm = sharding.NcclComm(0, 1)                    # the library's own communicator, world 1
+for rr in (False, True):
+    L, R, n0 = 32, 8, 5
+    T = geometric_ladder(0.9, 5.0, n0)
+    g = binding.RfimPT(L, R, 1.0, 1.5, binding.GAUSSIAN, seed=9, **({"shard_rr": (0, 1)} if rr else {"shard": sharding.replica_window(R, 1, 0)}))
+    g.set_nccl(comm)                              # no Python callback: ncclAllGather / ncclBroadcast are called from C
+    g.set_temperatures(T); g.set_adapt_params(3, 2)
+    o = oracle.Oracle(L, R, 1.0, 1.5, binding.GAUSSIAN, 9)
+    o.set_temperatures(T); o.set_adapt_params(3, 2)
+    g.adapt_temperatures(30); o.adapt_temperatures(30)     # inserts two replicas: ncclBroadcast of their lattices
+    g.sweep(12, 3); o.sweep(12, 3)                         # four exchange steps: ncclAllGather of the energy terms
+    assert g.n == o.n == 7
+    for r in range(g.n):
+        assert np.array_equal(g.get_spins_slot(r), o.get_spins_slot(r)), r
+    assert np.array_equal(g.get_permutation(), o.get_permutation())
+    for a, b in zip(g.get_timeseries(), o.get_timeseries()):
+        assert np.array_equal(a, b)
+    g.close()
+comm.close()
+print("shard-nccl-native-ok")
+"""
+
+
+def test_native_nccl_route_world_1():
+    r = subprocess.run([sys.executable, "-c", CHILD_NATIVE % ROOT], capture_output=True, text=True, timeout=600)
+    assert r.returncode == 0 and "shard-nccl-native-ok" in r.stdout, r.stdout[-2000:] + r.stderr[-4000:]
