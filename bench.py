@@ -346,6 +346,22 @@ def main():
             secondary["cfg4_sustained"] = {"workload": f"cfg4: one rfim_pt_sweep({wl.sweeps}, {k}) call, no L2 flush", "value": att / (ms_run * 1e6),
                                            "unit": UNIT, "ms_total": ms_run, "ms_per_step": ms_run / (wl.sweeps / k),
                                            "frac": att / (ms_run * 1e6) / bound, "clocks": c2}
+            # temporal blocking: sweeps fused per resident pass, exact dynamics (halo rows
+            # exchanged every phase), no measurement / exchange step; HBM bytes per attempt = 2 / sweeps_per_launch
+            tb = []
+            for spl in (1, 2, 5, 10, 20, 50, 100):
+                reps = max(3, 60 // spl)
+                g.sweep(spl, 0)
+                ev = [(torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)) for _ in range(reps)]
+                for a, b in ev:
+                    flush.zero_()
+                    a.record(); g.sweep(spl, 0); b.record()
+                torch.cuda.synchronize()
+                t = sorted(a.elapsed_time(b) for a, b in ev)[reps // 2]
+                tb.append({"sweeps_per_launch": spl, "value": float(wl.N) * wl.R * spl / (t * 1e6), "ms_per_launch": t,
+                           "hbm_bytes_per_attempt": 2.0 / spl})
+            secondary["temporal_blocking"] = {"workload": "cfg4, sweeps only, one launch = sweeps_per_launch sweeps of every replica, L2 flushed between launches",
+                                              "unit": UNIT, "points": tb}
         w5 = workloads.CONFIGS["cfg5"]
         h5 = binding.RfimPT(w5.L, w5.R, w5.J, w5.h, w5.field_kind, seeds=list(w5.seeds))
         h5.set_temperatures(w5.temperatures())

@@ -56,6 +56,15 @@ __device__ __forceinline__ unsigned long long res_now() { unsigned long long t; 
 #define RES_STAMP(i) do { } while (0)
 #endif
 
+// RFIM_RES_CHECK (debug builds; compute-sanitizer is not available on the GPU pool): every shared-memory row address, global
+// spin offset, field index and progress value the kernel forms is range-checked; a violation sets bit 1 of diag[0], which
+// every synchronising getter reports as an error (profiles/r2_sanitizer.md).
+#ifdef RFIM_RES_CHECK
+#define RES_CHECK(cond) do { if (!(cond)) atomicOr(rp.diag, 2ull); } while (0)
+#else
+#define RES_CHECK(cond) do { } while (0)
+#endif
+
 #ifndef RFIM_RES_THREADS
 #define RFIM_RES_THREADS 512
 #endif
@@ -421,6 +430,18 @@ __device__ __forceinline__ void res_row(const View& v, const ResParams& rp, uint
         }
     }
 
+    RES_CHECK(a_me + (K - 1) * ARR + 16 <= (uint32_t)G::SPINS_BYTES && a_x + (K - 1) * ARR + 16 <= (uint32_t)G::SPINS_BYTES &&
+              a_yp + (K - 1) * ARR + 16 <= (uint32_t)G::SPINS_BYTES && a_ym + (K - 1) * ARR + 16 <= (uint32_t)G::SPINS_BYTES &&
+              a_zp + (K - 1) * ARR + 16 <= (uint32_t)G::SPINS_BYTES && a_zm + (K - 1) * ARR + 16 <= (uint32_t)G::SPINS_BYTES);
+    RES_CHECK(((a_me | a_x | a_yp | a_ym | a_zp | a_zm) & 15u) == 0u);
+    RES_CHECK(KIND == 0 || (fp >= reinterpret_cast<const float4*>(rp.fielda_res) &&
+                            fp + (W - 1) * LH < reinterpret_cast<const float4*>(rp.fielda_res) + (size_t)v.D * v.N / 4));
+    RES_CHECK(KIND == 1 || (fq >= reinterpret_cast<const uint4*>(rp.fieldb_res) &&
+                            fq + (K - 1) * LH < reinterpret_cast<const uint4*>(rp.fieldb_res) + (size_t)v.D * v.N / 16));
+    RES_CHECK(!BND || ((!remote_p || rem.off_p + ROWB <= (size_t)v.D * v.Rs * v.N) && (!remote_m || rem.off_m + ROWB <= (size_t)v.D * v.Rs * v.N)));
+    RES_CHECK(!BND || (size_t)(ln.ds2 + (uint32_t)c) * (size_t)v.Nh + grow + ROWB <= (size_t)v.D * v.Rs * v.N);
+    RES_CHECK(ln.tab_addr >= (uint32_t)__cvta_generic_to_shared(smem + G::SPINS_BYTES) &&
+              ln.tab_addr + kResTabBytes <= (uint32_t)__cvta_generic_to_shared(smem + G::SPINS_BYTES) + (uint32_t)rp.cap_reps * kResTabBytes);
     uint4 xr[K];
 #pragma unroll
     for (int k = 0; k < K; ++k) xr[k] = *reinterpret_cast<const uint4*>(smem + a_x + k * ARR);
@@ -636,8 +657,11 @@ __global__ void __launch_bounds__(THREADS, 1) k_sweep_res(const View v, const Re
                     const int k = u % K, y = (u / K) % L, col = (u / (K * L)) & 1, p = u / (2 * K * L);
                     const ResPlane pi = s_plane[p];
                     const int ds = s_rep[pi.rep].ds, z = pi.z;
+                    RES_CHECK((size_t)(((long long)ds * 2 + col) * v.Nh + ((long long)z * L + y) * ROWB + 16 * k) + 16 <= (size_t)v.D * v.Rs * v.N &&
+                              ds >= 0 && ds < v.D * v.Rs && p < count);
                     raw[j] = res_piece_raw(v.spins, (size_t)(((long long)ds * 2 + col) * v.Nh + ((long long)z * L + y) * ROWB + 16 * k), v.packed);
                     dst[j] = A(col, (y + z) & 1, k, p * LH + (y >> 1));
+                    RES_CHECK(dst[j] + 16 <= (uint32_t)G::SPINS_BYTES);
                 }
             }
 #pragma unroll
@@ -671,6 +695,7 @@ __global__ void __launch_bounds__(THREADS, 1) k_sweep_res(const View v, const Re
         const uint32_t dom = c == 0 ? kDomColour0 : kDomColour1;
         const int eb = s_order[bidx];
         const bool btask = bidx < n_bblocks;
+        RES_CHECK(eb >= 0 && eb < nb && p >= 0 && p < rp.phases && lds_volatile(s_done + eb) <= p);
         const int e_raw = eb * 32 + lane;
         const bool valid = !RAGGED || e_raw < E;
         const int e = valid ? e_raw : E - 1;
@@ -678,6 +703,8 @@ __global__ void __launch_bounds__(THREADS, 1) k_sweep_res(const View v, const Re
         const ResPlane pi = s_plane[pl];
         const ResRep* rr = s_rep + pi.rep;
         const int z = pi.z;
+        RES_CHECK(pl >= 0 && pl < count && (int)pi.rep < nrep && z < L && (int)pi.zp_pl < count && (int)pi.zm_pl < count);
+        RES_CHECK((pi.zp_pl >= 0 || (int)pi.zp_owner < (int)gridDim.x) && (pi.zm_pl >= 0 || (int)pi.zm_owner < (int)gridDim.x));
         const bool remote_p = pi.zp_pl < 0, remote_m = pi.zm_pl < 0;
         const int e_zp = remote_p ? 0 : pi.zp_pl * LH + i, e_zm = remote_m ? 0 : pi.zm_pl * LH + i;
 
