@@ -44,6 +44,8 @@ def parse():
                     help="replica split: contiguous windows of ceil(R/N) slots (PAPER.md:125, Eq. 6) or round-robin, slot i on rank i mod N (PAPER.md:153)")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-e2e", action="store_true")
+    ap.add_argument("--stage-timing", action="store_true",
+                    help="debug builds with -DRFIM_RES_TIMING only: print the resident kernel's per-stage globaltimer stamps of one step")
     ap.add_argument("--no-secondary", action="store_true", help="skip the secondary workloads (config 5 int8 / bit-packed, config 3, sustained config 4)")
     return ap.parse_args()
 
@@ -287,6 +289,27 @@ def main():
                        "parallelism": "1 GPU" if world == 1 else (f"replicas of one realisation over {world} GPUs, all-gather of energy terms per exchange step"
                                                                      if replicas else f"{world} independent realisations, one per GPU")},
             "clocks": clocks, "gpu_launches": int(l1 - l0), "wall_s_timed_region": t_wall, "roofline": roofline}
+
+    if args.stage_timing and world == 1:
+        import ctypes
+        lib = binding.load()
+        if hasattr(lib, "rfim_pt_debug_timing"):
+            names = ["start", "setup_done", "run_loaded", "tasks_done_warp0", "after_barrier", "run_stored", "end"]
+            rows = {}
+            for kk, tag in ((0, "sweeps_only"), (k, "whole_step")):
+                acc = []
+                for _ in range(7):
+                    flush.zero_(); torch.cuda.synchronize()
+                    g.sweep(k, kk); torch.cuda.synchronize()
+                    buf = np.zeros((256, 8), dtype=np.uint64)
+                    lib.rfim_pt_debug_timing(buf.ctypes.data_as(ctypes.c_void_p))
+                    t = buf[:torch.cuda.get_device_properties(local_rank).multi_processor_count].astype(np.int64)
+                    acc.append((t - t[:, 0].min()) / 1e3)
+                rel = np.median(np.stack(acc[2:]), axis=0)
+                rows[tag] = {nm: {"median_over_ctas_us": float(np.median(rel[:, i])), "max_over_ctas_us": float(rel[:, i].max())} for i, nm in enumerate(names)}
+            line["stage_timing_us"] = rows
+        else:
+            line["stage_timing_us"] = "library not built with -DRFIM_RES_TIMING"
 
     # N > 1: the paper's own multi-GPU mode next to the default (independent realisations): ONE realisation, replicas dealt to the
     # ranks, one all-gather of 24 B per replica per exchange step -- strong scaling, measured in the same run

@@ -477,13 +477,7 @@ int launch_res_t(rfim_pt* h, const ResPlan& pl, const ResParams& rp) {
     auto kernel = k_sweep_res<KIND, K, NEVER, UNI, kResThreads>;
     CU(cudaFuncSetAttribute(kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)pl.smem));
     void* argv[] = {const_cast<void*>(static_cast<const void*>(&h->v)), const_cast<void*>(static_cast<const void*>(&rp))};
-#ifdef RFIM_DBG_PLAIN_LAUNCH
-    (void)argv;
-    kernel<<<dim3((unsigned)pl.grid), dim3(kResThreads), pl.smem, h->stream>>>(h->v, rp);
-    CU(cudaGetLastError());
-#else
     CU(cudaLaunchCooperativeKernel(reinterpret_cast<const void*>(kernel), dim3((unsigned)pl.grid), dim3(kResThreads), argv, pl.smem, h->stream));
-#endif
     h->launches += 1;
     return RFIM_OK;
 }

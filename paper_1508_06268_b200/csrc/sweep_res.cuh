@@ -48,6 +48,9 @@
 
 namespace rfim {
 
+// RFIM_RES_TIMING (debug builds): globaltimer stamps of the kernel's stages per CTA -- 0 start, 1 set-up done, 2 run loaded,
+// 3 task loop done (warp 0), 4 after the barrier, 5 run stored, 6 end -- read back with rfim_pt_debug_timing
+// (bench.py --stage-timing; profiles/r2_res_stage_timing.md)
 #ifdef RFIM_RES_TIMING
 __device__ unsigned long long g_res_timing[256][8];
 __device__ __forceinline__ unsigned long long res_now() { unsigned long long t; asm volatile("mov.u64 %0, %globaltimer;" : "=l"(t)); return t; }
@@ -685,11 +688,7 @@ __global__ void __launch_bounds__(THREADS, 1) k_sweep_res(const View v, const Re
         if (g >= total_tasks) break;
         while (g - base_cur >= nb) { base_cur += nb; ++p_cur; }
         const int p = p_cur, bidx = g - base_cur;
-        #ifdef RFIM_DBG_NOMEAS
-        const bool meas = false;
-#else
         const bool meas = rp.measure && p == rp.phases - 1;   // the last phase (colour 1) also measures, both colours
-#endif
         const int c = p & 1, oc = 1 - c;
         const uint32_t sweep = rp.sweep0 + (uint32_t)(p >> 1);
         const uint32_t dom = c == 0 ? kDomColour0 : kDomColour1;
@@ -822,7 +821,6 @@ __global__ void __launch_bounds__(THREADS, 1) k_sweep_res(const View v, const Re
             }
     }
     RES_STAMP(5);
-#ifndef RFIM_DBG_NOEXCH
     if (rp.exchange) {
         // the CTA that arrives last has every replica's sums in View::acc (integer atomics at L2): it runs the exchange step
         __threadfence();
@@ -838,7 +836,6 @@ __global__ void __launch_bounds__(THREADS, 1) k_sweep_res(const View v, const Re
             if (tid == 0) *rp.ticket = 0u;
         }
     }
-#endif
     RES_STAMP(6);
 }
 
