@@ -241,6 +241,18 @@ def main():
     philox_bound = ph_att / (ph_ms * 1e6)
     st_ms, st_bytes = binding.bench_stream(1 << 30, stream=torch.cuda.current_stream().cuda_stream)
     stream_gbs = st_bytes / (st_ms * 1e6)
+    # what one more warp instruction costs a sub-partition that is running the Philox stream
+    issue_probe = None
+    if world == 1:
+        cs = torch.cuda.current_stream().cuda_stream
+        ms0, wr = binding.bench_issue(0, 0, stream=cs)
+        mhz = 1965.0
+        cyc0 = ms0 * 1e-3 * mhz * 1e6 / wr
+        issue_probe = {"philox_only_cycles_per_warp_row": cyc0, "assumed_sm_mhz": mhz,
+                       "cycles_per_extra_warp_instruction": {}}
+        for name, kind in binding.PROBE_KINDS.items():
+            ms1, _ = binding.bench_issue(kind, 8, stream=cs)
+            issue_probe["cycles_per_extra_warp_instruction"][name] = (ms1 - ms0) * 1e-3 * mhz * 1e6 / wr / 2.0
     peaks = {}
     try:
         peaks = json.load(open(os.path.join(ROOT, "MEASURED_PEAKS.json")))
@@ -276,6 +288,7 @@ def main():
                 "stream_rmw_gbs_this_run": stream_gbs,
                 "algorithmic_bytes_per_attempt": bytes_per_attempt,
                 "achieved_algorithmic_gbs": sweep_rate * bytes_per_attempt,
+                "issue_cost_probe": issue_probe,
                 "whole_step_frac": (value / world) / bound,
                 "whole_step_frac_vs_issue_model": (value / world) / min(philox_theory, hbm_bound)}
 

@@ -228,6 +228,12 @@ int rfim_pt_get_diagnostics(rfim_pt* h, uint64_t diag[4]);
 /* Philox4x32-10 only: calls_per_thread calls per thread, outputs folded; *ms = device time of one
  * launch (CUDA events), *attempts = 4 * calls issued. */
 int rfim_pt_bench_philox(void* cuda_stream, int calls_per_thread, double* ms, double* attempts);
+/* Issue-cost probe: the same Philox stream on one CTA of 16 warps per SM, with extra_per_call (0 or 8) extra instructions of one
+ * kind per call spread between the rounds.  kind: 0 none (extra_per_call = 0), 1 LOP3, 2 PRMT, 3 I2FP (cvt.rn.f32.u32, ALU pipe),
+ * 4 I2F.RM (cvt.rm.f32.u32, XU pipe), 5 FFMA, 6 FADD, 7 MUFU.EX2, 8 LDS.64.  *ms = device time of one launch, *warp_rows =
+ * warp-rows (32 attempts) each SM sub-partition processed: (ms(kind) - ms(0)) * clock / warp_rows / 2 is the cost in cycles
+ * of one more warp instruction of that kind next to the Philox stream. */
+int rfim_pt_bench_issue(void* cuda_stream, int kind, int extra_per_call, double* ms, double* warp_rows);
 /* streaming int8 read-modify-write over bytes bytes of device memory (> L2 for an HBM figure). */
 int rfim_pt_bench_stream(void* cuda_stream, size_t bytes, double* ms, double* bytes_moved);
 

@@ -85,6 +85,7 @@ SIGNATURES = {
     "rfim_pt_get_diagnostics": (ctypes.c_int, [_vp, _u64p]),
     "rfim_pt_plan_adaptation": (ctypes.c_int, [_dp, _dp, ctypes.c_int, ctypes.c_int, ctypes.c_int, _dp, ctypes.POINTER(ctypes.c_int)]),
     "rfim_pt_bench_philox": (ctypes.c_int, [_vp, ctypes.c_int, _dp, _dp]),
+    "rfim_pt_bench_issue": (ctypes.c_int, [_vp, ctypes.c_int, ctypes.c_int, _dp, _dp]),
     "rfim_pt_bench_stream": (ctypes.c_int, [_vp, ctypes.c_size_t, _dp, _dp]),
 }
 
@@ -433,6 +434,18 @@ def bench_philox(calls_per_thread=2000, stream=None):
     if rc:
         raise RfimPtError(rc, "rfim_pt_bench_philox")
     return ms.value, att.value
+
+
+PROBE_KINDS = {"LOP3": 1, "PRMT": 2, "I2FP (ALU)": 3, "I2F.RM (XU)": 4, "FFMA": 5, "FADD": 6, "MUFU.EX2": 7, "LDS.64": 8}
+
+
+def bench_issue(kind, extra_per_call, stream=None):
+    """rfim_pt_bench_issue -> (ms of one launch, warp-rows per SM sub-partition)."""
+    ms, wr = ctypes.c_double(), ctypes.c_double()
+    rc = load().rfim_pt_bench_issue(_vp(stream or 0), kind, extra_per_call, ctypes.byref(ms), ctypes.byref(wr))
+    if rc:
+        raise RfimPtError(rc, "rfim_pt_bench_issue")
+    return ms.value, wr.value
 
 
 def bench_stream(nbytes, stream=None):

@@ -1492,6 +1492,59 @@ __global__ void __launch_bounds__(256) k_bench_philox(uint32_t* out, int calls, 
     out[blockIdx.x * blockDim.x + threadIdx.x] = acc;
 }
 
+// Issue-cost probe ("what an instruction costs next to Philox"): the same Philox stream with N extra
+// instructions of ONE kind per call, spread between the rounds, on operands that form their own dependency chains.  The
+// slope of the time per warp-row against N / 4 is what one more warp instruction of that kind costs the sub-partition
+// while it runs the Philox stream: the quantity the row update has to minimise.
+enum { kProbeNone = 0, kProbeLop3 = 1, kProbePrmt = 2, kProbeI2fp = 3, kProbeI2fRm = 4, kProbeFfma = 5, kProbeFadd = 6, kProbeMufu = 7, kProbeLds64 = 8, kProbeKinds = 9 };
+template <int OP>
+__device__ __forceinline__ void probe_op(uint32_t (&a)[4], float (&f)[4], int j, uint32_t saddr) {
+    uint32_t& x = a[j & 3]; const uint32_t y = a[(j + 1) & 3];
+    float& fx = f[j & 3]; const float fy = f[(j + 1) & 3];
+    if (OP == kProbeLop3) asm volatile("lop3.b32 %0, %0, %1, %2, 0x96;" : "+r"(x) : "r"(y), "r"(a[(j + 2) & 3]));
+    if (OP == kProbePrmt) asm volatile("prmt.b32 %0, %0, %1, %2;" : "+r"(x) : "r"(y), "r"(a[(j + 2) & 3]));
+    if (OP == kProbeI2fp) asm volatile("{ .reg .f32 t; cvt.rn.f32.u32 t, %1; mov.b32 %0, t; }" : "=r"(x) : "r"(y));
+    if (OP == kProbeI2fRm) asm volatile("{ .reg .f32 t; cvt.rm.f32.u32 t, %1; mov.b32 %0, t; }" : "=r"(x) : "r"(y));
+    if (OP == kProbeFfma) asm volatile("fma.rn.f32 %0, %0, %1, %2;" : "+f"(fx) : "f"(fy), "f"(f[(j + 2) & 3]));
+    if (OP == kProbeFadd) asm volatile("add.f32 %0, %0, %1;" : "+f"(fx) : "f"(fy));
+    if (OP == kProbeMufu) asm volatile("ex2.approx.ftz.f32 %0, %0;" : "+f"(fx));
+    if (OP == kProbeLds64) { uint32_t r0, r1; asm volatile("ld.shared.v2.u32 {%0,%1}, [%2];" : "=r"(r0), "=r"(r1) : "r"(saddr + (uint32_t)(j & 15) * 256u)); x ^= r0; a[(j + 3) & 3] = r1; }
+}
+template <int OP, int N>
+__global__ void __launch_bounds__(512, 1) k_bench_issue(uint32_t* out, int iters, BenchKeys rk, uint32_t sweep, uint32_t slot) {
+    extern __shared__ __align__(16) uint8_t probe_smem[];
+    for (int i = threadIdx.x; i < 4096; i += blockDim.x) reinterpret_cast<uint32_t*>(probe_smem)[i] = i * 2654435761u;
+    __syncthreads();
+    const uint32_t saddr = (uint32_t)__cvta_generic_to_shared(probe_smem) + (threadIdx.x & 31) * 8u;
+    uint32_t q = (blockIdx.x * blockDim.x + threadIdx.x) * 977u, acc = 0;
+    uint32_t a[4] = {q, q ^ 0x1234567u, q + 77u, q * 3u};
+    float f[4] = {1.0f + (q & 7), 2.0f, 0.5f, 1.5f};
+    constexpr int ILP = 4;
+    for (int it = 0; it < iters; ++it) {
+        uint32_t c0[ILP], c1[ILP], c2[ILP], c3[ILP];
+#pragma unroll
+        for (int j = 0; j < ILP; ++j) { c0[j] = q + j; c1[j] = sweep; c2[j] = slot; c3[j] = (uint32_t)it; }
+        int ja = 0;
+#pragma unroll
+        for (int r = 0; r < 10; ++r) {
+#pragma unroll
+            for (int j = 0; j < ILP; ++j) {
+                const uint32_t hi0 = __umulhi(kPhiloxM0, c0[j]), lo0 = kPhiloxM0 * c0[j];
+                const uint32_t hi1 = __umulhi(kPhiloxM1, c2[j]), lo1 = kPhiloxM1 * c2[j];
+                const uint32_t n0 = hi1 ^ c1[j] ^ rk.k[2 * r], n2 = hi0 ^ c3[j] ^ rk.k[2 * r + 1];
+                c1[j] = lo1; c3[j] = lo0; c0[j] = n0; c2[j] = n2;
+            }
+#pragma unroll
+            for (; ja < (r + 1) * N * ILP / 10; ++ja) probe_op<OP>(a, f, ja, saddr);
+        }
+        q += ILP;
+#pragma unroll
+        for (int j = 0; j < ILP; ++j) acc ^= c0[j] ^ c1[j] ^ c2[j] ^ c3[j];
+    }
+    acc ^= a[0] ^ a[1] ^ a[2] ^ a[3] ^ __float_as_uint(f[0] + f[1] + f[2] + f[3]);
+    out[blockIdx.x * blockDim.x + threadIdx.x] = acc;
+}
+
 __global__ void k_bench_stream(uint4* p, size_t n16) {
     const size_t stride = (size_t)gridDim.x * blockDim.x;
     for (size_t i = (size_t)blockIdx.x * blockDim.x + threadIdx.x; i < n16; i += stride) {
@@ -1543,6 +1596,41 @@ int rfim_pt_bench_philox(void* stream, int calls_per_thread, double* ms, double*
     int rc = time_launch(s, [&] { k_bench_philox<<<blocks, threads, 0, s>>>(out, calls, rk, 7u, 3u); }, ms);
     dev_free(out);
     *attempts = 4.0 * (double)blocks * threads * calls;
+    return rc;
+}
+
+int rfim_pt_bench_issue(void* stream, int kind, int extra_per_call, double* ms, double* warp_rows) {
+    if (kind < 0 || kind >= kProbeKinds || (extra_per_call != 0 && extra_per_call != 8) || !ms || !warp_rows) return RFIM_EINVAL;
+    if ((kind == kProbeNone) != (extra_per_call == 0)) return RFIM_EINVAL;
+    cudaStream_t s = reinterpret_cast<cudaStream_t>(stream);
+    int dev = 0, sms = 0;
+    if (cudaGetDevice(&dev) != cudaSuccess) return RFIM_ECUDA;
+    cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev);
+    const int blocks = sms, threads = 512, iters = 2000;             // one CTA of 16 warps per SM, like the sweep kernel
+    const size_t smem = 200 * 1024;
+    uint32_t* out = reinterpret_cast<uint32_t*>(dev_alloc((size_t)blocks * threads * 4));
+    if (!out) return RFIM_ENOMEM;
+    BenchKeys rk;
+    {
+        uint32_t k0 = 0x9E3779B9u, k1 = 0x1234567u;
+        for (int r = 0; r < 10; ++r) { rk.k[2 * r] = k0; rk.k[2 * r + 1] = k1; k0 += kPhiloxW0; k1 += kPhiloxW1; }
+    }
+    int rc = RFIM_EINVAL;
+#define RFIM_PROBE_CASE(K)                                                                                              \
+    case K: {                                                                                                            \
+        auto kern = k_bench_issue<K, (K == kProbeNone ? 0 : 8)>;                                                          \
+        if (cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem) != cudaSuccess) { rc = RFIM_ECUDA; break; } \
+        rc = time_launch(s, [&] { kern<<<blocks, threads, smem, s>>>(out, iters, rk, 7u, 3u); }, ms);                     \
+        break;                                                                                                            \
+    }
+    switch (kind) {
+        RFIM_PROBE_CASE(kProbeNone) RFIM_PROBE_CASE(kProbeLop3) RFIM_PROBE_CASE(kProbePrmt) RFIM_PROBE_CASE(kProbeI2fp) RFIM_PROBE_CASE(kProbeI2fRm)
+        RFIM_PROBE_CASE(kProbeFfma) RFIM_PROBE_CASE(kProbeFadd) RFIM_PROBE_CASE(kProbeMufu) RFIM_PROBE_CASE(kProbeLds64)
+        default: break;
+    }
+#undef RFIM_PROBE_CASE
+    dev_free(out);
+    *warp_rows = (double)iters * 4 /* calls */ * 4 /* attempts per call */ * (threads / 32 / 4);   // per SM sub-partition
     return rc;
 }
 
