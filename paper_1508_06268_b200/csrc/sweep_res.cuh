@@ -174,6 +174,26 @@ __device__ __forceinline__ uint32_t prmt(uint32_t a, uint32_t b, uint32_t sel) {
 
 __device__ __forceinline__ int lds_volatile(const int* p) { return *reinterpret_cast<const volatile int*>(p); }
 
+// per-block completion counters (shared memory, CTA scope): a task's rows are stored before its counter is bumped with
+// release semantics, and a reader that has seen the count with an acquire load may read those rows -- no separate fence
+// on the reading side (the acquire load compiles to a plain LDS; shared-memory accesses of a warp are issued in order)
+__device__ __forceinline__ int lds_acquire(const int* p) {
+    int v;
+#if defined(__CUDA_ARCH__)
+    asm volatile("ld.acquire.cta.shared.u32 %0, [%1];" : "=r"(v) : "r"((uint32_t)__cvta_generic_to_shared(p)) : "memory");
+#else
+    v = *p;
+#endif
+    return v;
+}
+__device__ __forceinline__ void sts_release_inc(int* p) {
+#if defined(__CUDA_ARCH__)
+    asm volatile("red.release.cta.shared.add.u32 [%0], 1;" :: "r"((uint32_t)__cvta_generic_to_shared(p)) : "memory");
+#else
+    ++*p;
+#endif
+}
+
 // ---- one 16-site piece between its global form (16 bytes of 0/1, or 16 bits when View::packed) and the shared-memory
 // form (16 bytes of 0/SP).  `off` is the piece's index in spins (a multiple of 16).
 __device__ __forceinline__ uint32_t res_nibble_to_word(uint32_t nib) { return ((nib & 0xFu) * 0x00204081u) & 0x01010101u; }
@@ -288,7 +308,7 @@ __device__ __noinline__ void res_wait_slow(const int* s_done, int eb, int b_zp, 
                                            const uint32_t* prog_m, uint32_t want, unsigned long long* diag) {
     int spins = 0;
     for (;;) {
-        bool ok = lds_volatile(s_done + eb) >= p && lds_volatile(s_done + b_zp) >= p && lds_volatile(s_done + b_zm) >= p;
+        bool ok = lds_acquire(s_done + eb) >= p && lds_acquire(s_done + b_zp) >= p && lds_acquire(s_done + b_zm) >= p;
         if (prog_p) ok = ok && (int32_t)(ld_acquire_gpu(prog_p) - want) >= 0;
         if (prog_m) ok = ok && (int32_t)(ld_acquire_gpu(prog_m) - want) >= 0;
         if (__all_sync(0xFFFFFFFFu, ok)) break;
@@ -337,42 +357,42 @@ __device__ __forceinline__ ResPiece res_load_piece(const uint8_t* smem, const ui
     return pc;
 }
 
-// Measurement of one piece, taken in the last phase of a launch from what the update holds in registers:
-// me = updated words of the piece, fb / f0..f3 = the piece's field (bimodal 0x80 flags / Gaussian g_i as floats, exact),
-// idx8 = table offsets before the update (bits 3..5 of a byte = SP * n1).  Returns {Eb, Ef, Msum} contributions of the
-// piece's 16 sites: Ef and Msum of this colour always, Eb (the six-neighbour form: every bond has one colour-1 end)
-// only when with_eb (the colour-1 words).  Both fit an int.
+// Measurement partials of one 16-site piece in the last phase of a launch (out of line: the measuring instantiation must not
+// add to the register pressure of the row update).  me = the colour-1 words just updated, idx8 = their table offsets before
+// the update (bits 3..5 of a byte = SP * n1), c0 = the colour-0 words of the same row and piece; f1 / f0 = the field of the
+// two (bimodal: one uint4 of 0x80 flags; Gaussian: four float4 `stride` apart, g_i exact).  Returns {64 sum s n1 over the
+// colour-1 sites, packed byte sums of the eight words (SP per up spin), field term, bimodal: number of h_i = +1 sites}:
+// field term = SP sum hb s (bimodal) or the sum of g_i over the up spins (Gaussian, |.| <= 32 * 2^23), both colours.
 template <int KIND>
-__device__ __noinline__ int3 res_measure_piece(uint4 mev, uint4 idx8v, uint4 fbv, float4 f0, float4 f1, float4 f2, float4 f3, int with_eb) {
-    const uint32_t me[4] = {mev.x, mev.y, mev.z, mev.w};
-    const uint32_t ns[4] = {idx8v.x & 0x38383838u, idx8v.y & 0x38383838u, idx8v.z & 0x38383838u, idx8v.w & 0x38383838u};
-    int sn = 0, s0 = 0, nn = 0;                   // 64 sum s n1, 8 sum s, 8 sum n1
-#pragma unroll
-    for (int w = 0; w < 4; ++w) {
-        sn += dot4(me[w], ns[w]); s0 += dot4(me[w], 0x01010101u); nn += dot4(ns[w], 0x01010101u);
-    }
-    int3 r;
-    r.x = with_eb ? sn / 16 - 12 * (s0 / 8) - 2 * (nn / 8) + 6 * 16 : 0;     // sum (2 s - 1)(2 n1 - 6) = 4 s.n1 - 12 s - 2 n1 + 6 per site
-    r.z = 2 * (s0 / 8) - 16;
+__device__ __noinline__ int4 res_measure_piece(uint4 mev, uint4 idx8v, uint4 c0v, const void* f1, const void* f0, int stride) {
+    const uint32_t me[4] = {mev.x, mev.y, mev.z, mev.w}, c0[4] = {c0v.x, c0v.y, c0v.z, c0v.w};
+    const uint32_t ix[4] = {idx8v.x, idx8v.y, idx8v.z, idx8v.w};
+    int sn = 0, ef = 0, hh = 0;
+    uint32_t ws = 0;
     if (KIND == 0) {
-        // sum (2 hb - 1)(2 s - 1) = 4 hb.s - 2 hb - 2 s + 1 per site
-        const uint32_t hb[4] = {fbv.x >> 7, fbv.y >> 7, fbv.z >> 7, fbv.w >> 7};   // 0/1 per byte
-        int hs0 = 0, hh = 0;
+        const uint4 b1 = __ldg(static_cast<const uint4*>(f1)), b0 = __ldg(static_cast<const uint4*>(f0));
+        const uint32_t h1[4] = {b1.x >> 7, b1.y >> 7, b1.z >> 7, b1.w >> 7}, h0[4] = {b0.x >> 7, b0.y >> 7, b0.z >> 7, b0.w >> 7};   // 0/1 per byte
 #pragma unroll
-        for (int w = 0; w < 4; ++w) { hs0 += dot4(hb[w], me[w]); hh += dot4(hb[w], 0x01010101u); }
-        r.y = 4 * (hs0 / 8) - 2 * hh - 2 * (s0 / 8) + 16;
+        for (int w = 0; w < 4; ++w) {
+            sn += dot4(me[w], ix[w] & 0x38383838u);
+            ws += me[w] + c0[w];
+            ef += dot4(h1[w], me[w]) + dot4(h0[w], c0[w]);
+            hh += dot4(h1[w] + h0[w], 0x01010101u);
+        }
     } else {
-        // SP * (sum of g_i over the up spins of the piece): |.| <= 16 * 2^23 * SP = 2^30.  Ef = 2 * (that / SP) - (sum of g_i over
-        // all sites), and the second term is a constant of the plane (ResParams::gsum), subtracted once when the sums are handed over
-        const float gf[16] = {f0.x, f0.y, f0.z, f0.w, f1.x, f1.y, f1.z, f1.w, f2.x, f2.y, f2.z, f2.w, f3.x, f3.y, f3.z, f3.w};
-        int ef = 0;
 #pragma unroll
-        for (int w = 0; w < 4; ++w)
+        for (int w = 0; w < 4; ++w) {
+            const float4 a1 = __ldg(static_cast<const float4*>(f1) + (long long)w * stride), a0 = __ldg(static_cast<const float4*>(f0) + (long long)w * stride);
+            const float g1[4] = {a1.x, a1.y, a1.z, a1.w}, g0[4] = {a0.x, a0.y, a0.z, a0.w};
+            sn += dot4(me[w], ix[w] & 0x38383838u);
+            ws += me[w] + c0[w];
+            const uint32_t s1 = me[w] >> 3, s0 = c0[w] >> 3;                               // 0/1 per byte
 #pragma unroll
-            for (int j = 0; j < 4; ++j) ef += __float2int_rn(gf[4 * w + j]) * (int)__byte_perm(me[w], 0u, 0x4440 + j);
-        r.y = ef;
+            for (int j = 0; j < 4; ++j)
+                ef += __float2int_rn(g1[j]) * (int)__byte_perm(s1, 0u, 0x4440 + j) + __float2int_rn(g0[j]) * (int)__byte_perm(s0, 0u, 0x4440 + j);
+        }
     }
-    return r;
+    return make_int4(sn, (int)ws, ef, hh);
 }
 
 __device__ __noinline__ void res_flush_sums(long long* s_acc, int rep, long long eb, long long ef, long long ms) {
@@ -448,6 +468,8 @@ __device__ __forceinline__ void res_row(const View& v, const ResParams& rp, uint
     uint4 xr[K];
 #pragma unroll
     for (int k = 0; k < K; ++k) xr[k] = *reinterpret_cast<const uint4*>(smem + a_x + k * ARR);
+    int r_sn = 0, r_ef = 0, r_hh = 0;                     // measurement partials of the row (MEAS only)
+    uint32_t r_ws = 0;
 #pragma unroll
     for (int k = 0; k < K; ++k) {             // one 16-site piece of the row at a time
         // field of the piece: issued first, consumed last
@@ -506,23 +528,25 @@ __device__ __forceinline__ void res_row(const View& v, const ResParams& rp, uint
             if (BND && (remote_p || remote_m))
                 res_piece_to_global(v.spins, (size_t)(ln.ds2 + (uint32_t)c) * (size_t)v.Nh + grow + 16u * k, v.packed, nw);
             if (MEAS) {
-                // the final phase (colour 1) measures both colours: its own updated words (with Eb: every bond has one
-                // colour-1 end) and the colour-0 words of the same row, xr[k], final since the phase before; their field
-                // sits one colour block (L planes x 2 classes) below this one
-                const float4 z4 = make_float4(0.f, 0.f, 0.f, 0.f);
-                const int3 m3 = res_measure_piece<KIND>(nw, make_uint4(idx8[0], idx8[1], idx8[2], idx8[3]), fb,
-                                                        KIND ? fa[0] : z4, KIND ? fa[1] : z4, KIND ? fa[2] : z4, KIND ? fa[3] : z4, 1);
-                float4 ga[4] = {z4, z4, z4, z4};
-                uint4 gb = make_uint4(0u, 0u, 0u, 0u);
-                if (KIND == 0) gb = __ldg(fq - 2 * G::L * K * LH + k * LH);
-                else {
-#pragma unroll
-                    for (int w = 0; w < 4; ++w) ga[w] = __ldg(fp - 2 * G::L * W * LH + (4 * k + w) * LH);
-                }
-                const int3 m0 = res_measure_piece<KIND>(xr[k], make_uint4(0u, 0u, 0u, 0u), gb, ga[0], ga[1], ga[2], ga[3], 0);
-                m_eb += m3.x; m_ef += m3.y + m0.y; m_ms += m3.z + m0.z;
+                // the final phase (colour 1) measures both colours: its own updated words and the colour-0 words of the same
+                // row, xr[k], final since the phase before; their field sits one colour block (L planes x 2 classes) below
+                const void* f1 = KIND == 0 ? static_cast<const void*>(fq + k * LH) : static_cast<const void*>(fp + 4 * k * LH);
+                const void* f0 = KIND == 0 ? static_cast<const void*>(fq - 2 * G::L * K * LH + k * LH)
+                                           : static_cast<const void*>(fp - 2 * G::L * W * LH + 4 * k * LH);
+                const int4 m4 = res_measure_piece<KIND>(nw, make_uint4(idx8[0], idx8[1], idx8[2], idx8[3]), xr[k], f1, f0, LH);
+                r_sn += m4.x; r_ws += (uint32_t)m4.y; r_ef += m4.z; r_hh += m4.w;
             }
         }
+    }
+    if (MEAS && (!RAGGED || valid)) {
+        // Eb = sum over the colour-1 sites of (2 s - 1)(2 n1 - 6) = 4 s n1 - 12 s - 2 n1 + 6 per site, and summed over a whole
+        // (periodic) lattice the n1 of the colour-1 sites count every up spin of colour 0 six times: - 2 sum n1 = - 12 S0.
+        // Every plane of a replica ends in the same accumulator, so the row hands in - 12 (its own colour-0 up spins) instead.
+        const int S = dot4(r_ws, 0x01010101u) / (int)kResSP;          // up spins of the row, both colours
+        m_eb += r_sn / 16 - 12 * S + 6 * ROWB;
+        m_ms += 2 * S - 2 * ROWB;
+        if (KIND == 0) m_ef += 4 * (r_ef / (int)kResSP) - 2 * r_hh - 2 * S + 2 * ROWB;   // sum (2 hb - 1)(2 s - 1), both colours
+        else m_ef += (long long)r_ef * (long long)kResSP;             // SP * (sum of g_i over the up spins), as the accumulators expect
     }
 }
 
@@ -711,12 +735,11 @@ __global__ void __launch_bounds__(THREADS, 1) k_sweep_res(const View v, const Re
         // remote neighbour planes: their owners have published phase p-1
         if (p > 0) {
             const int b_zp = remote_p ? eb : e_zp >> 5, b_zm = remote_m ? eb : e_zm >> 5;
-            const int d0 = lds_volatile(s_done + eb), d1 = lds_volatile(s_done + b_zp), d2 = lds_volatile(s_done + b_zm);
+            const int d0 = lds_acquire(s_done + eb), d1 = lds_acquire(s_done + b_zp), d2 = lds_acquire(s_done + b_zm);
             const bool ok = min(d0, min(d1, d2)) >= p;
             if (btask || !__all_sync(0xFFFFFFFFu, ok))
                 res_wait_slow(s_done, eb, b_zp, b_zm, p, remote_p ? rp.prog + pi.zp_owner : nullptr,
                               remote_m ? rp.prog + pi.zm_owner : nullptr, (rp.epoch << 8) | (uint32_t)p, rp.diag);
-            __threadfence_block();
         }
 
         // per-task lane constants; everything class-dependent is an immediate offset from these
@@ -788,10 +811,8 @@ __global__ void __launch_bounds__(THREADS, 1) k_sweep_res(const View v, const Re
                     __threadfence();
                     st_release_gpu(rp.prog + b, (rp.epoch << 8) | (uint32_t)(p + 1));
                 }
-            } else {
-                __threadfence_block();
             }
-            atomicAdd(&s_done[eb], 1);
+            sts_release_inc(&s_done[eb]);
         }
     }
     if (lane == 0) {                                  // hand this warp's measurement sums over
