@@ -255,6 +255,70 @@ __global__ void k_import_bits(View v, int first, const uint8_t* __restrict__ in)
     }
 }
 
+// ---- the same two conversions for L % 16 == 0 (L = 16, 32, 64: the sizes the host interface is timed on): one thread per 16
+// consecutive sites of a row of the natural order = two bytes of the bit format = eight sites of each colour (one aligned
+// 8-byte group of the byte layout, or one byte of the packed layout).  Even x belong to colour (y+z)&1, odd x to the other.
+__device__ __forceinline__ uint32_t bits_spread8(uint32_t v) {          // bit m of v -> bit 2m
+    v = (v | (v << 4)) & 0x0F0Fu; v = (v | (v << 2)) & 0x3333u; v = (v | (v << 1)) & 0x5555u;
+    return v;
+}
+__device__ __forceinline__ uint32_t bits_compact8(uint32_t v) {         // bit 2m of v -> bit m
+    v &= 0x5555u; v = (v | (v >> 1)) & 0x3333u; v = (v | (v >> 2)) & 0x0F0Fu; v = (v | (v >> 4)) & 0x00FFu;
+    return v;
+}
+__device__ __forceinline__ uint32_t bytes01_to_bits8(uint2 w) {        // eight bytes of 0/1 -> eight bits
+    return ((((w.x & 0x01010101u) * 0x01020408u) >> 24) & 0xFu) | (((((w.y & 0x01010101u) * 0x01020408u) >> 24) & 0xFu) << 4);
+}
+__device__ __forceinline__ uint2 bits8_to_bytes01(uint32_t b) {
+    return make_uint2(((b & 0xFu) * 0x00204081u) & 0x01010101u, (((b >> 4) & 0xFu) * 0x00204081u) & 0x01010101u);
+}
+__global__ void k_export_bits16(View v, int first, uint8_t* __restrict__ out) {
+    const int ds = first + blockIdx.y;
+    const int L = v.L, Lh = v.Lh, cpr = L >> 4;                          // 16-site chunks per row
+    const long long chunks = v.N >> 4;
+    unsigned short* o = reinterpret_cast<unsigned short*>(out + (long long)blockIdx.y * (v.N >> 3));
+    for (long long q = (long long)blockIdx.x * blockDim.x + threadIdx.x; q < chunks; q += (long long)gridDim.x * blockDim.x) {
+        const long long row = q / cpr;                                   // y + L z
+        const int xq = (int)(q - row * cpr), y = (int)(row % L), z = (int)(row / L);
+        const int ce = (y + z) & 1;                                      // colour of the even x of this row
+        const long long j0 = (long long)Lh * row + 8 * xq;               // same-colour index of the chunk's first site, both colours
+        uint32_t be, bo;
+        if (v.packed) {
+            const uint8_t* base = v.spins + (long long)ds * (v.N >> 3);
+            be = base[((long long)ce * v.Nh + j0) >> 3];
+            bo = base[((long long)(1 - ce) * v.Nh + j0) >> 3];
+        } else {
+            const uint8_t* base = v.spins + (long long)ds * 2 * v.Nh;
+            be = bytes01_to_bits8(*reinterpret_cast<const uint2*>(base + (long long)ce * v.Nh + j0));
+            bo = bytes01_to_bits8(*reinterpret_cast<const uint2*>(base + (long long)(1 - ce) * v.Nh + j0));
+        }
+        o[q] = (unsigned short)(bits_spread8(be) | (bits_spread8(bo) << 1));
+    }
+}
+__global__ void k_import_bits16(View v, int first, const uint8_t* __restrict__ in) {
+    const int ds = first + blockIdx.y;
+    const int L = v.L, Lh = v.Lh, cpr = L >> 4;
+    const long long chunks = v.N >> 4;
+    const unsigned short* src = reinterpret_cast<const unsigned short*>(in + (long long)blockIdx.y * (v.N >> 3));
+    for (long long q = (long long)blockIdx.x * blockDim.x + threadIdx.x; q < chunks; q += (long long)gridDim.x * blockDim.x) {
+        const long long row = q / cpr;
+        const int xq = (int)(q - row * cpr), y = (int)(row % L), z = (int)(row / L);
+        const int ce = (y + z) & 1;
+        const long long j0 = (long long)Lh * row + 8 * xq;
+        const uint32_t w = src[q];
+        const uint32_t be = bits_compact8(w), bo = bits_compact8(w >> 1);
+        if (v.packed) {
+            uint8_t* base = v.spins + (long long)ds * (v.N >> 3);
+            base[((long long)ce * v.Nh + j0) >> 3] = (uint8_t)be;
+            base[((long long)(1 - ce) * v.Nh + j0) >> 3] = (uint8_t)bo;
+        } else {
+            uint8_t* base = v.spins + (long long)ds * 2 * v.Nh;
+            *reinterpret_cast<uint2*>(base + (long long)ce * v.Nh + j0) = bits8_to_bytes01(be);
+            *reinterpret_cast<uint2*>(base + (long long)(1 - ce) * v.Nh + j0) = bits8_to_bytes01(bo);
+        }
+    }
+}
+
 // ---- whole-buffer conversion between the byte and the bit layout (same index j, eight spins per byte) ----------
 __global__ void k_pack_bits(const uint8_t* __restrict__ bytes, uint8_t* __restrict__ bits, long long nbits_bytes) {
     for (long long b = (long long)blockIdx.x * blockDim.x + threadIdx.x; b < nbits_bytes; b += (long long)gridDim.x * blockDim.x) {

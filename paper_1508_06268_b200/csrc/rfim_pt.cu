@@ -150,6 +150,16 @@ dim3 grid_for(long long work, int ny, int threads = 256) {
     return dim3((unsigned)bx, (unsigned)ny, 1);
 }
 
+// natural-order bit format <-> device layout: the 16-site kernels for L % 16 == 0, the generic per-bit ones otherwise
+void launch_export_bits(rfim_pt* h, int ny, int first, uint8_t* out) {
+    if (h->L % 16 == 0) k_export_bits16<<<grid_for(h->N / 16, ny), 256, 0, h->stream>>>(h->v, first, out);
+    else k_export_bits<<<grid_for(h->N / 8, ny), 256, 0, h->stream>>>(h->v, first, out);
+}
+void launch_import_bits(rfim_pt* h, int ny, int first, const uint8_t* in) {
+    if (h->L % 16 == 0) k_import_bits16<<<grid_for(h->N / 16, ny), 256, 0, h->stream>>>(h->v, first, in);
+    else k_import_bits<<<grid_for(h->N / 8, ny), 256, 0, h->stream>>>(h->v, first, in);
+}
+
 // ---- field ---------------------------------------------------------------------------------
 void generate_field_host(rfim_pt* h, int d) {
     const uint32_t k0 = (uint32_t)(h->seeds[d] & 0xFFFFFFFFull), k1 = (uint32_t)(h->seeds[d] >> 32);
@@ -1099,12 +1109,12 @@ int rfim_pt_adapt_temperatures(rfim_pt* h, int64_t trial_sweeps) {
                     if (!h->bcast && !h->nccl_comm) return fail(h, RFIM_ESTATE, "replica shard: inserting a replica needs the lattice broadcast (rfim_pt_set_broadcast / rfim_pt_set_nccl)");
                     if ((rc = ensure_stage(h, (size_t)h->N / 8))) return rc;
                     uint8_t* buf = reinterpret_cast<uint8_t*>(h->stage);
-                    if (h->v.stores(src)) { k_export_bits<<<grid_for(h->N / 8, 1), 256, 0, h->stream>>>(h->v, h->v.stored_index(src), buf); h->launches += 1; }
+                    if (h->v.stores(src)) { launch_export_bits(h, 1, h->v.stored_index(src), buf); h->launches += 1; }
                     const int root = h->sstride == 1 ? src / h->Rs : src % h->world;
                     const int brc = h->nccl_comm ? h->nccl_broadcast(buf, buf, (size_t)h->N / 8, /* ncclUint8 */ 1, root, h->nccl_comm, h->stream)
                                                  : h->bcast(h->bcast_user, buf, (size_t)h->N / 8, root, h->stream);
                     if (brc) return fail(h, RFIM_ECUDA, "replica shard: the lattice broadcast failed");
-                    if (h->v.stores(slot)) { k_import_bits<<<grid_for(h->N / 8, 1), 256, 0, h->stream>>>(h->v, h->v.stored_index(slot), buf); h->launches += 1; }
+                    if (h->v.stores(slot)) { launch_import_bits(h, 1, h->v.stored_index(slot), buf); h->launches += 1; }
                     CU(cudaGetLastError());
                 } else {
                     const size_t lat = (size_t)h->N / (h->packing == 1 ? 8 : 1);      // bytes per lattice
@@ -1233,7 +1243,7 @@ int rfim_pt_get_spins_all_bits(rfim_pt* h, uint8_t* out) {
     const size_t bytes = (size_t)DR * (size_t)(h->N / 8);
     int rc = ensure_stage(h, bytes);
     if (rc) return rc;
-    k_export_bits<<<grid_for(h->N / 8, DR), 256, 0, h->stream>>>(h->v, 0, reinterpret_cast<uint8_t*>(h->stage));
+    launch_export_bits(h, DR, 0, reinterpret_cast<uint8_t*>(h->stage));
     h->launches += 1;
     CU(cudaGetLastError());
     CU(cudaMemcpyAsync(out, h->stage, bytes, cudaMemcpyDeviceToHost, h->stream));
@@ -1249,7 +1259,7 @@ int rfim_pt_set_spins_all_bits(rfim_pt* h, const uint8_t* in) {
     int rc = ensure_stage(h, bytes);
     if (rc) return rc;
     CU(cudaMemcpyAsync(h->stage, in, bytes, cudaMemcpyHostToDevice, h->stream));
-    k_import_bits<<<grid_for(h->N / 8, DR), 256, 0, h->stream>>>(h->v, 0, reinterpret_cast<const uint8_t*>(h->stage));
+    launch_import_bits(h, DR, 0, reinterpret_cast<const uint8_t*>(h->stage));
     h->launches += 1;
     CU(cudaGetLastError());
     return RFIM_OK;

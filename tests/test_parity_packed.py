@@ -110,7 +110,7 @@ def test_packing_errors():
 def test_bit_packed_host_interface_roundtrip():
     """rfim_pt_get/set_spins_all_bits: natural-order bits on the host, both device storage modes, against the int8 getters."""
     from paper_1508_06268_b200 import binding
-    for L, packing in ((8, 8), (32, 8), (32, 1)):
+    for L, packing in ((8, 8), (12, 8), (16, 8), (32, 8), (32, 1), (64, 8), (64, 1)):
         g = binding.RfimPT(L, 3, 1.0, 1.0, BIMODAL, seeds=[5, 6])
         if packing == 1:
             g.set_packing(1)
