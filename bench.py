@@ -381,7 +381,7 @@ def main():
             c2 = s2.stop()
             ms_run = a.elapsed_time(b)
             att = float(wl.N) * wl.R * wl.sweeps
-            secondary["cfg4_sustained"] = {"workload": f"cfg4: one rfim_pt_sweep({wl.sweeps}, {k}) call, no L2 flush", "value": att / (ms_run * 1e6),
+            secondary["cfg4_sustained"] = {"workload": f"cfg4: one rfim_pt_sweep({wl.sweeps}, {k}) call (12 parallel-tempering moves per launch), no L2 flush", "value": att / (ms_run * 1e6),
                                            "unit": UNIT, "ms_total": ms_run, "ms_per_step": ms_run / (wl.sweeps / k),
                                            "frac": att / (ms_run * 1e6) / bound, "clocks": c2}
             # temporal blocking: sweeps fused per resident pass, exact dynamics (halo rows
@@ -411,6 +411,14 @@ def main():
         h3 = binding.RfimPT(w3.L, w3.R, w3.J, w3.h, w3.field_kind, seed=w3.seeds[0])
         h3.set_temperatures(w3.temperatures())
         secondary["cfg3"] = entry(w3, timed_other(h3, w3.exchange_every, n_sec), {"dtype": "u8"})
+        # config 3's production run as ONE call (the library holds as many exchange periods per launch as fit in 127 sweeps)
+        a, b = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        a.record(); h3.sweep(w3.sweeps, w3.exchange_every); b.record(); torch.cuda.synchronize()
+        att3 = float(w3.N) * w3.R * w3.sweeps
+        secondary["cfg3_sustained"] = {"workload": f"cfg3: one rfim_pt_sweep({w3.sweeps}, {w3.exchange_every}) call, no L2 flush",
+                                       "value": att3 / (a.elapsed_time(b) * 1e6), "unit": UNIT, "ms_total": a.elapsed_time(b),
+                                       "ms_per_step": a.elapsed_time(b) / (w3.sweeps / w3.exchange_every),
+                                       "frac": att3 / (a.elapsed_time(b) * 1e6) / bound}
         h3.close()
         w2 = workloads.CONFIGS["cfg2"]
         h2 = binding.RfimPT(w2.L, w2.R, w2.J, w2.h, w2.field_kind, seed=w2.seeds[0])

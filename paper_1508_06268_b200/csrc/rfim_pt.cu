@@ -85,6 +85,7 @@ struct rfim_pt {
     bool terms_fresh = false;         // View::last holds the energy terms of the CURRENT lattices (last call ended on an exchange step)
     int res_grid_limit = 0;           // 0 = one CTA per SM
     int res_partition = 0;            // resident kernel: 0 automatic, 1 equal runs of planes, 2 whole replicas per CTA
+    int res_multi = 1;                // resident kernel: != 0 allows several parallel-tempering moves per launch (single handle, fused exchange)
     int sm_count = 0, smem_optin = 0;
     std::string err;
 };
@@ -482,9 +483,9 @@ int launch_flow(rfim_pt* h, int sweeps) {
     return RFIM_OK;
 }
 
-template <int KIND, int K, bool NEVER, bool UNI>
+template <int KIND, int K, bool NEVER, bool UNI, bool MULTI = false>
 int launch_res_t(rfim_pt* h, const ResPlan& pl, const ResParams& rp) {
-    auto kernel = k_sweep_res<KIND, K, NEVER, UNI, kResThreads>;
+    auto kernel = k_sweep_res<KIND, K, NEVER, UNI, kResThreads, MULTI>;
     CU(cudaFuncSetAttribute(kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)pl.smem));
     void* argv[] = {const_cast<void*>(static_cast<const void*>(&h->v)), const_cast<void*>(static_cast<const void*>(&rp))};
     CU(cudaLaunchCooperativeKernel(reinterpret_cast<const void*>(kernel), dim3((unsigned)pl.grid), dim3(kResThreads), argv, pl.smem, h->stream));
@@ -494,14 +495,24 @@ int launch_res_t(rfim_pt* h, const ResPlan& pl, const ResParams& rp) {
 
 template <int KIND, int K, bool NEVER>
 int launch_res_u(rfim_pt* h, const ResPlan& pl, const ResParams& rp) {
+    if (rp.nseg > 1) return launch_res_t<KIND, K, NEVER, true, true>(h, pl, rp);     // several moves per launch: single handles only
     return pl.nd == 1 ? launch_res_t<KIND, K, NEVER, true>(h, pl, rp) : launch_res_t<KIND, K, NEVER, false>(h, pl, rp);
 }
 
 template <int KIND, int K, bool NEVER>
 int launch_res_k(rfim_pt* h, const ResPlan& pl, const ResParams& rp) { return launch_res_u<KIND, K, NEVER>(h, pl, rp); }
 
+// several parallel-tempering moves in one launch: single realisation, not sharded, exchange step fused
+bool res_multi_ok(const rfim_pt* h) {
+    if (!h->res_multi || h->shard || h->D != 1) return false;
+    const ResPlan pl = res_plan(h);
+    return pl.ok && pl.groups == 1 && pl.nd == 1;
+}
+
 // `sweeps` (<= 127) sweeps of every active replica of every member: one cooperative launch per group of members
-int launch_res(rfim_pt* h, int sweeps, bool measure, bool* exchanged) {
+// nseg > 1 (res_multi_moves() said so): the launch ends on an exchange step and holds nseg of them, the first after `first`
+// sweeps, then every `period`; all of them run inside the kernel
+int launch_res(rfim_pt* h, int sweeps, bool measure, bool* exchanged, int nseg = 1, int first = 0, int period = 0) {
     if (h->shard && iterated(h) == 0) { *exchanged = false; return RFIM_OK; }      // this shard stores no active slot
     const ResPlan pl0 = res_plan(h);
     if (!pl0.ok) return fail(h, RFIM_EINVAL, "resident kernel: the planes of one CTA do not fit in shared memory");
@@ -518,6 +529,8 @@ int launch_res(rfim_pt* h, int sweeps, bool measure, bool* exchanged) {
         rp.xstep = (uint32_t)h->xstep;
         rp.xrow = h->series_steps;
         rp.ticket = h->res_prog + kResMaxGrid;       // the word after the progress words (zeroed at create, left at zero)
+        rp.xflag = h->res_prog + kResMaxGrid + 1;
+        rp.nseg = nseg; rp.first2 = 2 * first; rp.period2 = 2 * period;
         rp.sweep0 = (uint32_t)h->sweep_g;
         rp.epoch = ++h->res_epoch;
         rp.prog = h->res_prog;
@@ -659,14 +672,24 @@ int do_sweeps(rfim_pt* h, int64_t n_sweeps, int k) {
     int64_t left = n_sweeps;
     while (left > 0) {
         int64_t chunk = 1;
+        int nseg = 1;
+        const int64_t first = k > 0 ? (int64_t)k - (int64_t)(h->sweep_g % (uint64_t)k) : 0;   // sweeps to the next exchange step
         if (flow) {
             chunk = std::min<int64_t>(left, 127);
-            if (k > 0) chunk = std::min<int64_t>(chunk, (int64_t)k - (int64_t)(h->sweep_g % (uint64_t)k));
+            if (k > 0) {
+                // the resident kernel can hold several moves: as many whole exchange periods as fit in 127 sweeps
+                if (variant == 4 && chunk >= first + k && res_multi_ok(h)) {
+                    nseg = 1 + (int)((chunk - first) / k);
+                    chunk = first + (int64_t)(nseg - 1) * k;
+                } else {
+                    chunk = std::min<int64_t>(chunk, first);
+                }
+            }
         }
         // the resident kernel measures in the same launch when its chunk ends on an exchange step
         const bool step_after = k > 0 && ((h->sweep_g + (uint64_t)chunk) % (uint64_t)k) == 0;
         bool exchanged = false;
-        int rc = variant == 4 ? launch_res(h, (int)chunk, step_after, &exchanged)
+        int rc = variant == 4 ? launch_res(h, (int)chunk, step_after, &exchanged, nseg, (int)first, k)
                : variant == 5 ? launch_small(h, (int)chunk, step_after, &exchanged)
                : (flow ? launch_flow(h, (int)chunk) : launch_sweep(h));
         if (rc) return rc;
@@ -677,8 +700,8 @@ int do_sweeps(rfim_pt* h, int64_t n_sweeps, int k) {
             if (variant != 4 && variant != 5 && (rc = launch_reduce(h))) return rc;
             if ((rc = gather_terms(h))) return rc;
             if (!exchanged && (rc = launch_exchange(h))) return rc;
-            h->series_steps += 1;
-            h->xstep += 1;
+            h->series_steps += nseg;
+            h->xstep += nseg;
         }
     }
     return RFIM_OK;
@@ -786,7 +809,7 @@ int create_impl(rfim_pt** out, int L, int R, double J, double hh, int kind, int 
     A(alloc_into(h, &v.accn, DR));
     A(alloc_into(h, &v.diag, 4));
     A(alloc_into(h, &h->flow_prog, DR * 32));
-    A(alloc_into(h, &h->res_prog, (size_t)kResMaxGrid + 1));
+    A(alloc_into(h, &h->res_prog, (size_t)kResMaxGrid + 2));
     if (flow_supported(h)) {
         if (kind == RFIM_FIELD_BIMODAL) A(alloc_into(h, &h->fieldb_res, (size_t)D * h->N));
         else { A(alloc_into(h, &h->fielda_res, (size_t)D * h->N)); A(alloc_into(h, &h->gsum_res, (size_t)D * L)); }
@@ -805,7 +828,7 @@ int create_impl(rfim_pt** out, int L, int R, double J, double hh, int kind, int 
         CU(cudaMemcpyAsync(const_cast<uint32_t*>(v.keys), keys.data(), keys.size() * 4, cudaMemcpyHostToDevice, h->stream));
         CU(cudaMemsetAsync(v.diag, 0, 32, h->stream));
         CU(cudaMemsetAsync(h->flow_prog, 0, DR * 32 * 4, h->stream));
-        CU(cudaMemsetAsync(h->res_prog, 0, ((size_t)kResMaxGrid + 1) * 4, h->stream));
+        CU(cudaMemsetAsync(h->res_prog, 0, ((size_t)kResMaxGrid + 2) * 4, h->stream));
         CU(cudaMemsetAsync(v.t2r, 0xFF, DR * 4, h->stream));
         CU(cudaMemsetAsync(v.r2t, 0xFF, DR * 4, h->stream));
         CU(cudaStreamSynchronize(h->stream));
@@ -1027,6 +1050,7 @@ int rfim_pt_set_tuning(rfim_pt* h, int key, int value) {
     if (key == 0 && value >= 1 && value <= 64) { h->flow_rr = value; return RFIM_OK; }
     if (key == 1 && value >= 0 && value <= kResMaxGrid) { h->res_grid_limit = value; return RFIM_OK; }
     if (key == 2 && value >= 0 && value <= 2) { h->res_partition = value; return RFIM_OK; }
+    if (key == 3 && value >= 0 && value <= 1) { h->res_multi = value; return RFIM_OK; }
     return fail(h, RFIM_EINVAL, "unknown tuning key or value out of range");
 }
 

@@ -110,6 +110,10 @@ struct ResParams {
     const uint8_t* fieldb_res;   // bimodal:  [D][2][L][2][K][L/2] uint4, 0x80 where h_i = +1
     const long long* gsum;       // Gaussian: [D][L] sum of g_i over plane z
     unsigned long long* diag;
+    // several parallel-tempering moves per launch (MULTI instantiation only): the launch ends on an exchange step and holds
+    // nseg of them, after phase first2 - 1, first2 + period2 - 1, ...; the run stays in shared memory across them
+    int nseg, first2, period2;
+    uint32_t* xflag;             // release word of the mid-launch exchange steps: (epoch << 8) | steps done
     uint32_t rk0[20];            // Philox round keys of member 0 (used from the constant bank when D == 1)
 };
 
@@ -564,7 +568,7 @@ __device__ __forceinline__ void res_task_rows(const View& v, const ResParams& rp
 }
 
 // K = 16-byte pieces per row per colour (L = 32 K); UNI: one member, round keys come from the constant bank
-template <int KIND, int K, bool NEVER, bool UNI, int THREADS>
+template <int KIND, int K, bool NEVER, bool UNI, int THREADS, bool MULTI = false>
 __global__ void __launch_bounds__(THREADS, 1) k_sweep_res(const View v, const ResParams rp) {
     using G = ResGeom<K>;
     constexpr int L = G::L, LH = G::LH, ROWB = G::ROWB, W = G::W, ARR = G::ARR;
@@ -705,14 +709,23 @@ __global__ void __launch_bounds__(THREADS, 1) k_sweep_res(const View v, const Re
     // ---- the task flow ------------------------------------------------------------------------------
     constexpr bool RAGGED = (LH % 32) != 0;
     int p_cur = 0, base_cur = 0;                      // phase of this warp's current task number (numbers only grow)
+    // MULTI: the launch holds rp.nseg exchange steps; the task flow runs segment by segment (all tasks of the phases up to an
+    // exchange step, then a grid-wide rendezvous in which the last CTA to arrive runs the step, then new tables), and a warp
+    // that drew a ticket beyond the open segment keeps it for the next one.
+    int seg = 0, seg_end = MULTI ? rp.first2 : rp.phases, g_keep = -1;
+    for (;;) {
+    const int seg_tasks = MULTI ? nb * seg_end : total_tasks;
     for (;;) {
         int g = 0;
-        if (lane == 0) g = atomicAdd(&s_ctl[2], 1);
-        g = __shfl_sync(0xFFFFFFFFu, g, 0);
-        if (g >= total_tasks) break;
+        if (MULTI && g_keep >= 0) { g = g_keep; g_keep = -1; }
+        else {
+            if (lane == 0) g = atomicAdd(&s_ctl[2], 1);
+            g = __shfl_sync(0xFFFFFFFFu, g, 0);
+        }
+        if (g >= seg_tasks) { if (MULTI) g_keep = g; break; }
         while (g - base_cur >= nb) { base_cur += nb; ++p_cur; }
         const int p = p_cur, bidx = g - base_cur;
-        const bool meas = rp.measure && p == rp.phases - 1;   // the last phase (colour 1) also measures, both colours
+        const bool meas = rp.measure && p == (MULTI ? seg_end : rp.phases) - 1;   // the last phase before an exchange step (colour 1) also measures, both colours
         const int c = p & 1, oc = 1 - c;
         const uint32_t sweep = rp.sweep0 + (uint32_t)(p >> 1);
         const uint32_t dom = c == 0 ? kDomColour0 : kDomColour1;
@@ -815,6 +828,72 @@ __global__ void __launch_bounds__(THREADS, 1) k_sweep_res(const View v, const Re
             sts_release_inc(&s_done[eb]);
         }
     }
+    if (!MULTI || seg == rp.nseg - 1) break;
+    // ---- an exchange step inside the launch (MULTI) ------------------------------------------------------------
+    {
+        if (lane == 0) {
+            long long* wa = s_wacc + 4 * (tid >> 5);
+            res_flush_sums(s_acc, (int)wa[0], wa[1], wa[2], wa[3]);
+            wa[0] = -1; wa[1] = 0; wa[2] = 0; wa[3] = 0;
+        }
+        __syncthreads();
+        for (int r = tid; r < nrep * 3; r += THREADS) {
+            const long long val = (KIND == 1 && r % 3 == 1) ? s_acc[r] / (long long)(kResSP / 2) : s_acc[r];
+            atomicAdd(reinterpret_cast<unsigned long long*>(v.acc + (long long)(s_rep[r / 3].d * v.R + s_rep[r / 3].slot) * 3 + r % 3), (unsigned long long)val);
+        }
+        __threadfence();
+        __syncthreads();
+        if (tid == 0) s_ctl[0] = (atomicAdd(rp.ticket, 1u) == (uint32_t)(rp.nact * (seg + 1) - 1)) ? 1 : 0;   // (no boundary task is open: the slot is free)
+        __syncthreads();
+        const uint32_t xwant = (rp.epoch << 8) | (uint32_t)(seg + 1);
+        if (s_ctl[0]) {                                // every CTA's sums are in View::acc: this one runs the step
+            __threadfence();
+            for (int d = 0; d < v.D; ++d) {
+                exchange_member(v, d, rp.xstep + (uint32_t)seg, rp.xrow + seg, 1);
+                __syncthreads();
+            }
+            __threadfence();
+            if (tid == 0) st_release_gpu(rp.xflag, xwant);
+        } else if (tid == 0) {
+            int polls = 0;
+            while (ld_acquire_gpu(rp.xflag) != xwant) {
+                backoff();
+                if (++polls > (1 << 22)) { atomicOr(rp.diag, 1ull); break; }
+            }
+        }
+        __syncthreads();
+        if (tid == 0) s_ctl[0] = 0;
+        // the resident lattices keep their slots; their ranks (temperatures) are the new ones
+        for (int r = tid; r < nrep; r += THREADS) {
+            const int d = s_rep[r].d, tr = d * v.R + __ldcg(v.r2t + d * v.R + s_rep[r].slot);
+            s_rep[r].tr = tr;
+            s_rep[r].band = KIND == 0 ? 0.f : v.band[tr];
+            s_rep[r].never = KIND == 0 ? v.never[tr] : 0u;
+            s_rep[r].beta = v.beta[tr];
+            s_acc[3 * r] = 0; s_acc[3 * r + 1] = 0; s_acc[3 * r + 2] = 0;
+        }
+        for (int i = tid; i < nrep * 32; i += THREADS) {
+            const int r = i >> 5, idx = i & 31;
+            const int d = s_rep[r].d, tr = d * v.R + __ldcg(v.r2t + d * v.R + s_rep[r].slot);
+            uint2 ent = make_uint2(0u, 0u);
+            if (KIND == 0) {
+                ent.x = v.etab[(long long)tr * 32 + idx];
+                ent.y = (v.never[tr] >> idx) & 1u;
+            } else if (idx < 16) {
+                const GaussEntry ge = v.gtab[(long long)tr * 16 + idx];
+                ent.x = __float_as_uint(ge.x); ent.y = __float_as_uint(ge.y);
+            }
+            reinterpret_cast<uint2*>(s_tab + (size_t)r * kResTabBytes)[idx] = ent;
+        }
+        __syncthreads();
+        if (KIND == 1 && tid < count)
+            atomicAdd(reinterpret_cast<unsigned long long*>(s_acc + 3 * s_plane[tid].rep + 1),
+                      (unsigned long long)(-(long long)(kResSP / 2) * rp.gsum[(long long)s_rep[s_plane[tid].rep].d * L + s_plane[tid].z]));
+        __syncthreads();
+        ++seg;
+        seg_end += rp.period2;
+    }
+    }
     if (lane == 0) {                                  // hand this warp's measurement sums over
         long long* wa = s_wacc + 4 * (tid >> 5);
         res_flush_sums(s_acc, (int)wa[0], wa[1], wa[2], wa[3]);
@@ -846,12 +925,12 @@ __global__ void __launch_bounds__(THREADS, 1) k_sweep_res(const View v, const Re
         // the CTA that arrives last has every replica's sums in View::acc (integer atomics at L2): it runs the exchange step
         __threadfence();
         __syncthreads();
-        if (tid == 0) s_ctl[0] = (atomicAdd(rp.ticket, 1u) == (uint32_t)(rp.nact - 1)) ? 1 : 0;
+        if (tid == 0) s_ctl[0] = (atomicAdd(rp.ticket, 1u) == (uint32_t)(rp.nact * (MULTI ? rp.nseg : 1) - 1)) ? 1 : 0;
         __syncthreads();
         if (s_ctl[0]) {
             __threadfence();
             for (int d = 0; d < v.D; ++d) {
-                exchange_member(v, d, rp.xstep, rp.xrow, 1);
+                exchange_member(v, d, rp.xstep + (MULTI ? (uint32_t)(rp.nseg - 1) : 0u), rp.xrow + (MULTI ? rp.nseg - 1 : 0), 1);
                 __syncthreads();
             }
             if (tid == 0) *rp.ticket = 0u;

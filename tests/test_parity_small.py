@@ -261,6 +261,34 @@ def test_resident_kernel_bit_exact(L, R, grid, partition, kind, h):
     assert d["ulp_ambiguous"] == 0
 
 
+@pytest.mark.parametrize("L,R,grid,partition", [(32, 5, 7, 1), (32, 3, 148, 1), (64, 3, 5, 1), (64, 2, 0, 1), (32, 5, 3, 2), (32, 7, 0, 0)])
+@pytest.mark.parametrize("kind,h", [(BIMODAL, 2.0), (GAUSSIAN, 1.5)])
+def test_resident_kernel_several_moves_per_launch(L, R, grid, partition, kind, h):
+    """One launch of the resident kernel holds every exchange period that fits in 127 sweeps (the run stays in shared memory,
+    the exchange steps run inside the kernel behind a grid-wide rendezvous): calls that start off a period boundary, end on
+    one or past one, and a call long enough to need two launches -- against the oracle and against one launch per move."""
+    T = np.geomspace(0.8, 5.0, R)
+    g, o = make_pair(L, R, 1.0, h, kind, 17 * L + R, T)
+    g1, _ = make_pair(L, R, 1.0, h, kind, 17 * L + R, T)
+    for x in (g, g1):
+        x.set_kernel_variant(4)
+        x.set_tuning(1, grid)
+        x.set_tuning(2, partition)
+    g1.set_tuning(3, 0)                                            # one launch per move
+    for chunk, k in [(2, 3), (13, 3), (20, 5), (9, 4), (133, 7)]:
+        l0 = g.diagnostics()["launches"]
+        g.sweep(chunk, k)
+        if (chunk, k) == (20, 5):
+            assert g.diagnostics()["launches"] - l0 == 1           # four exchange steps, one launch
+        g1.sweep(chunk, k); o.sweep(chunk, k)
+        assert_same_state(g, o, what=f"several moves per launch, L={L} grid={grid} after chunk {chunk},{k}")
+        assert_same_state(g1, o, what=f"one move per launch, L={L} grid={grid} after chunk {chunk},{k}")
+    assert_same_series(g, o)
+    assert_same_series(g1, o)
+    assert g.diagnostics()["ulp_ambiguous"] == 0
+    g.close(); g1.close(); o.close()
+
+
 @pytest.mark.parametrize("kind", [BIMODAL, GAUSSIAN])
 def test_resident_kernel_extreme_temperatures_and_long_launch(kind):
     T = np.array([1e-30, 0.05, 1.0, 1e3, 1e30])
