@@ -319,6 +319,63 @@ __global__ void k_import_bits16(View v, int first, const uint8_t* __restrict__ i
     }
 }
 
+// natural-order +-1 int8 <-> device layout, L % 16 == 0: one thread per 16 consecutive sites of a row (one 16-byte load or store)
+__device__ __forceinline__ uint32_t bytes01_to_pm1(uint32_t w) { return ((w ^ 0x01010101u) * 0xFFu) | 0x01010101u; }   // 1 -> 0x01, 0 -> 0xFF
+__device__ __forceinline__ uint32_t pm1_to_bytes01(uint32_t w) {                                                       // s > 0 -> 1, s <= 0 -> 0, per byte
+    return ((((w & 0x7F7F7F7Fu) + 0x7F7F7F7Fu) & ~w & 0x80808080u) >> 7);
+}
+__global__ void k_export_spins16(View v, int first, int8_t* __restrict__ out) {
+    const int ds = first + blockIdx.y;
+    const int L = v.L, Lh = v.Lh, cpr = L >> 4;
+    const long long chunks = v.N >> 4;
+    uint4* o = reinterpret_cast<uint4*>(out + (long long)blockIdx.y * v.N);
+    for (long long q = (long long)blockIdx.x * blockDim.x + threadIdx.x; q < chunks; q += (long long)gridDim.x * blockDim.x) {
+        const long long row = q / cpr;
+        const int xq = (int)(q - row * cpr), y = (int)(row % L), z = (int)(row / L);
+        const int ce = (y + z) & 1;
+        const long long j0 = (long long)Lh * row + 8 * xq;
+        uint2 e, od;
+        if (v.packed) {
+            const uint8_t* base = v.spins + (long long)ds * (v.N >> 3);
+            e = bits8_to_bytes01(base[((long long)ce * v.Nh + j0) >> 3]);
+            od = bits8_to_bytes01(base[((long long)(1 - ce) * v.Nh + j0) >> 3]);
+        } else {
+            const uint8_t* base = v.spins + (long long)ds * 2 * v.Nh;
+            e = *reinterpret_cast<const uint2*>(base + (long long)ce * v.Nh + j0);
+            od = *reinterpret_cast<const uint2*>(base + (long long)(1 - ce) * v.Nh + j0);
+        }
+        uint4 n;
+        n.x = bytes01_to_pm1(__byte_perm(e.x, od.x, 0x5140)); n.y = bytes01_to_pm1(__byte_perm(e.x, od.x, 0x7362));
+        n.z = bytes01_to_pm1(__byte_perm(e.y, od.y, 0x5140)); n.w = bytes01_to_pm1(__byte_perm(e.y, od.y, 0x7362));
+        o[q] = n;
+    }
+}
+__global__ void k_import_spins16(View v, int first, const int8_t* __restrict__ in) {
+    const int ds = first + blockIdx.y;
+    const int L = v.L, Lh = v.Lh, cpr = L >> 4;
+    const long long chunks = v.N >> 4;
+    const uint4* src = reinterpret_cast<const uint4*>(in + (long long)blockIdx.y * v.N);
+    for (long long q = (long long)blockIdx.x * blockDim.x + threadIdx.x; q < chunks; q += (long long)gridDim.x * blockDim.x) {
+        const long long row = q / cpr;
+        const int xq = (int)(q - row * cpr), y = (int)(row % L), z = (int)(row / L);
+        const int ce = (y + z) & 1;
+        const long long j0 = (long long)Lh * row + 8 * xq;
+        uint4 n = src[q];
+        n.x = pm1_to_bytes01(n.x); n.y = pm1_to_bytes01(n.y); n.z = pm1_to_bytes01(n.z); n.w = pm1_to_bytes01(n.w);
+        const uint2 e = make_uint2(__byte_perm(n.x, n.y, 0x6420), __byte_perm(n.z, n.w, 0x6420));
+        const uint2 od = make_uint2(__byte_perm(n.x, n.y, 0x7531), __byte_perm(n.z, n.w, 0x7531));
+        if (v.packed) {
+            uint8_t* base = v.spins + (long long)ds * (v.N >> 3);
+            base[((long long)ce * v.Nh + j0) >> 3] = (uint8_t)bytes01_to_bits8(e);
+            base[((long long)(1 - ce) * v.Nh + j0) >> 3] = (uint8_t)bytes01_to_bits8(od);
+        } else {
+            uint8_t* base = v.spins + (long long)ds * 2 * v.Nh;
+            *reinterpret_cast<uint2*>(base + (long long)ce * v.Nh + j0) = e;
+            *reinterpret_cast<uint2*>(base + (long long)(1 - ce) * v.Nh + j0) = od;
+        }
+    }
+}
+
 // ---- whole-buffer conversion between the byte and the bit layout (same index j, eight spins per byte) ----------
 __global__ void k_pack_bits(const uint8_t* __restrict__ bytes, uint8_t* __restrict__ bits, long long nbits_bytes) {
     for (long long b = (long long)blockIdx.x * blockDim.x + threadIdx.x; b < nbits_bytes; b += (long long)gridDim.x * blockDim.x) {

@@ -161,6 +161,15 @@ void launch_import_bits(rfim_pt* h, int ny, int first, const uint8_t* in) {
     else k_import_bits<<<grid_for(h->N / 8, ny), 256, 0, h->stream>>>(h->v, first, in);
 }
 
+void launch_export_spins(rfim_pt* h, int ny, int first, int8_t* out) {
+    if (h->L % 16 == 0) k_export_spins16<<<grid_for(h->N / 16, ny), 256, 0, h->stream>>>(h->v, first, out);
+    else k_export_spins<<<grid_for(h->N, ny), 256, 0, h->stream>>>(h->v, first, out);
+}
+void launch_import_spins(rfim_pt* h, int ny, int first, const int8_t* in) {
+    if (h->L % 16 == 0) k_import_spins16<<<grid_for(h->N / 16, ny), 256, 0, h->stream>>>(h->v, first, in);
+    else k_import_spins<<<grid_for(h->N, ny), 256, 0, h->stream>>>(h->v, first, in);
+}
+
 // ---- field ---------------------------------------------------------------------------------
 void generate_field_host(rfim_pt* h, int d) {
     const uint32_t k0 = (uint32_t)(h->seeds[d] & 0xFFFFFFFFull), k1 = (uint32_t)(h->seeds[d] >> 32);
@@ -1197,7 +1206,7 @@ int rfim_pt_get_spins_slot(rfim_pt* h, int d, int slot, int8_t* out) {
     if (slot < 0 || slot >= h->R || !out) return fail(h, RFIM_EINVAL, "bad slot or null buffer");
     if (!h->v.stores(slot)) return fail(h, RFIM_EINVAL, "replica shard: this rank does not store that slot");
     if ((rc = ensure_stage(h, (size_t)h->N))) return rc;
-    k_export_spins<<<grid_for(h->N, 1), 256, 0, h->stream>>>(h->v, d * h->Rs + h->v.stored_index(slot), h->stage);
+    launch_export_spins(h, 1, d * h->Rs + h->v.stored_index(slot), h->stage);
     h->launches += 1;
     CU(cudaGetLastError());
     CU(cudaMemcpyAsync(out, h->stage, (size_t)h->N, cudaMemcpyDeviceToHost, h->stream));
@@ -1228,7 +1237,7 @@ int rfim_pt_set_spins_slot(rfim_pt* h, int d, int slot, const int8_t* in) {
     if (!h->v.stores(slot)) return fail(h, RFIM_EINVAL, "replica shard: this rank does not store that slot");
     if ((rc = ensure_stage(h, (size_t)h->N))) return rc;
     CU(cudaMemcpyAsync(h->stage, in, (size_t)h->N, cudaMemcpyHostToDevice, h->stream));
-    k_import_spins<<<grid_for(h->N, 1), 256, 0, h->stream>>>(h->v, d * h->Rs + h->v.stored_index(slot), h->stage);
+    launch_import_spins(h, 1, d * h->Rs + h->v.stored_index(slot), h->stage);
     h->launches += 1;
     CU(cudaGetLastError());
     CU(cudaStreamSynchronize(h->stream));
@@ -1240,7 +1249,7 @@ int rfim_pt_get_spins_all(rfim_pt* h, int8_t* out) {
     const int DR = h->D * h->Rs;          // every stored lattice (a replica shard: its slot window)
     int rc = ensure_stage(h, (size_t)DR * h->N);
     if (rc) return rc;
-    k_export_spins<<<grid_for(h->N, DR), 256, 0, h->stream>>>(h->v, 0, h->stage);
+    launch_export_spins(h, DR, 0, h->stage);
     h->launches += 1;
     CU(cudaGetLastError());
     CU(cudaMemcpyAsync(out, h->stage, (size_t)DR * h->N, cudaMemcpyDeviceToHost, h->stream));
@@ -1255,7 +1264,7 @@ int rfim_pt_set_spins_all(rfim_pt* h, const int8_t* in) {
     int rc = ensure_stage(h, (size_t)DR * h->N);
     if (rc) return rc;
     CU(cudaMemcpyAsync(h->stage, in, (size_t)DR * h->N, cudaMemcpyHostToDevice, h->stream));
-    k_import_spins<<<grid_for(h->N, DR), 256, 0, h->stream>>>(h->v, 0, h->stage);
+    launch_import_spins(h, DR, 0, h->stage);
     h->launches += 1;
     CU(cudaGetLastError());
     return RFIM_OK;
