@@ -425,7 +425,7 @@ struct ResLane {
 // One row (L/2 same-colour sites) of one checkerboard class S: K pieces of 16 sites.  DIR (warp-uniform): the
 // second x-neighbour sits at xh-1 (0) or xh+1 (1).  BND: a z-neighbour plane lives in another CTA (rows read from and
 // published to global memory); MEAS: also measure; RAGGED: lanes past the last row redo it and do not store.
-template <int KIND, int K, bool NEVER, bool UNI, bool BND, bool MEAS, bool RAGGED>
+template <int KIND, int K, bool NEVER, bool UNI, bool BND, bool MEAS, bool RAGGED, bool FLATE = true>
 __device__ __forceinline__ void res_row(const View& v, const ResParams& rp, uint8_t* smem, const ResLane& ln, const int s, const int c, const int DIR,
                                         const uint32_t sweep, const uint32_t dom, const ResRep* rr, const bool valid,
                                         const bool remote_p, const bool remote_m, const size_t roff_p, const size_t roff_m,
@@ -476,15 +476,27 @@ __device__ __forceinline__ void res_row(const View& v, const ResParams& rp, uint
     uint32_t r_ws = 0;
 #pragma unroll
     for (int k = 0; k < K; ++k) {             // one 16-site piece of the row at a time
-        // field of the piece: issued first, consumed last
+        // field of the piece
         float4 fa[4];
         uint4 fb = make_uint4(0u, 0u, 0u, 0u);
-        if (KIND == 0) fb = __ldg(fq + k * LH);
-        else {
+        // Where the field loads stand in program order relative to the piece's shared-memory loads decides how ptxas lays the
+        // 128-register loop out: after them is 1.4 % faster in the single-move kernel at L = 64 and a little faster at L = 32,
+        // before them 4 % faster in the several-moves-per-launch instantiation at L = 64 (both measured).
+        if (!FLATE) {
+            if (KIND == 0) fb = __ldg(fq + k * LH);
+            else {
 #pragma unroll
-            for (int w = 0; w < 4; ++w) fa[w] = __ldg(fp + (4 * k + w) * LH);
+                for (int w = 0; w < 4; ++w) fa[w] = __ldg(fp + (4 * k + w) * LH);
+            }
         }
         ResPiece pc = res_load_piece<K>(smem, xr, a_yp, a_ym, a_zp, a_zm, a_me, k, DIR, rem);
+        if (FLATE) {
+            if (KIND == 0) fb = __ldg(fq + k * LH);
+            else {
+#pragma unroll
+                for (int w = 0; w < 4; ++w) fa[w] = __ldg(fp + (4 * k + w) * LH);
+            }
+        }
         const uint32_t fw[4] = {fb.x, fb.y, fb.z, fb.w};
         uint32_t idx8[4];
 #pragma unroll
@@ -556,14 +568,14 @@ __device__ __forceinline__ void res_row(const View& v, const ResParams& rp, uint
 
 // both rows (classes) of a task, one after the other through the same code (the loop body must stay inside the
 // instruction cache: two unrolled copies of it were measured 15 % slower)
-template <int KIND, int K, bool NEVER, bool UNI, bool BND, bool MEAS, bool RAGGED>
+template <int KIND, int K, bool NEVER, bool UNI, bool BND, bool MEAS, bool RAGGED, bool FLATE = true>
 __device__ __forceinline__ void res_task_rows(const View& v, const ResParams& rp, uint8_t* smem, const ResLane& ln, const int c,
                                               const uint32_t sweep, const uint32_t dom, const ResRep* rr, const bool valid,
                                               const bool remote_p, const bool remote_m, const size_t roff_p, const size_t roff_m,
                                               long long& m_eb, long long& m_ef, long long& m_ms) {
 #pragma unroll 1
     for (int s = 0; s < 2; ++s)
-        res_row<KIND, K, NEVER, UNI, BND, MEAS, RAGGED>(v, rp, smem, ln, s, c, (s + c) & 1, sweep, dom, rr, valid, remote_p, remote_m, roff_p, roff_m,
+        res_row<KIND, K, NEVER, UNI, BND, MEAS, RAGGED, FLATE>(v, rp, smem, ln, s, c, (s + c) & 1, sweep, dom, rr, valid, remote_p, remote_m, roff_p, roff_m,
                                                         m_eb, m_ef, m_ms);
 }
 
@@ -708,6 +720,7 @@ __global__ void __launch_bounds__(THREADS, 1) k_sweep_res(const View v, const Re
 
     // ---- the task flow ------------------------------------------------------------------------------
     constexpr bool RAGGED = (LH % 32) != 0;
+    constexpr bool kFieldLate = !(MULTI && K == 2);     // see res_row
     int p_cur = 0, base_cur = 0;                      // phase of this warp's current task number (numbers only grow)
     // MULTI: the launch holds rp.nseg exchange steps; the task flow runs segment by segment (all tasks of the phases up to an
     // exchange step, then a grid-wide rendezvous in which the last CTA to arrive runs the step, then new tables), and a warp
@@ -779,16 +792,16 @@ __global__ void __launch_bounds__(THREADS, 1) k_sweep_res(const View v, const Re
 
         long long m_eb = 0, m_ef = 0, m_ms = 0;
         if (!btask && !meas) {
-            res_task_rows<KIND, K, NEVER, UNI, false, false, RAGGED>(v, rp, smem, ln, c, sweep, dom, rr, valid, false, false, 0u, 0u, m_eb, m_ef, m_ms);
+            res_task_rows<KIND, K, NEVER, UNI, false, false, RAGGED, kFieldLate>(v, rp, smem, ln, c, sweep, dom, rr, valid, false, false, 0u, 0u, m_eb, m_ef, m_ms);
         } else {
             // rows of a z-neighbour plane that lives in another CTA: read from global memory (class 0; class 1 = + ROWB)
             const int zq_p = (z + 1) & (L - 1), zq_m = (z - 1) & (L - 1);
             const size_t roff_p = (size_t)(ln.ds2 + (uint32_t)oc) * (size_t)v.Nh + (uint32_t)(zq_p * L + 2 * i) * ROWB;
             const size_t roff_m = (size_t)(ln.ds2 + (uint32_t)oc) * (size_t)v.Nh + (uint32_t)(zq_m * L + 2 * i) * ROWB;
             if (btask && !meas)
-                res_task_rows<KIND, K, NEVER, UNI, true, false, RAGGED>(v, rp, smem, ln, c, sweep, dom, rr, valid, remote_p, remote_m, roff_p, roff_m, m_eb, m_ef, m_ms);
+                res_task_rows<KIND, K, NEVER, UNI, true, false, RAGGED, kFieldLate>(v, rp, smem, ln, c, sweep, dom, rr, valid, remote_p, remote_m, roff_p, roff_m, m_eb, m_ef, m_ms);
             else
-                res_task_rows<KIND, K, NEVER, UNI, true, true, RAGGED>(v, rp, smem, ln, c, sweep, dom, rr, valid, remote_p && btask, remote_m && btask, roff_p, roff_m, m_eb, m_ef, m_ms);
+                res_task_rows<KIND, K, NEVER, UNI, true, true, RAGGED, kFieldLate>(v, rp, smem, ln, c, sweep, dom, rr, valid, remote_p && btask, remote_m && btask, roff_p, roff_m, m_eb, m_ef, m_ms);
         }
 
         if (meas) {
