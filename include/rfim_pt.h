@@ -219,6 +219,12 @@ int rfim_pt_get_bimodal_threshold(rfim_pt* h, int d, int rank, int k, int b, uin
  * its length in *out_n.  n < R: PAPER.md:147's rule, the min(a, R-n, n-1) lowest-rate intervals (ties: lower rank) get
  * their midpoint temperature.  n == R: DESIGN.md S8's insert-and-prune.  RFIM_EINVAL on a bad argument. */
 int rfim_pt_plan_adaptation(const double* T, const double* rate, int n, int R, int a, double* out_T, int* out_n);
+/* The launch planning of rfim_pt_sweep alone (host only, no handle): with sweep_index sweeps done, n_sweeps >= 1 still asked for
+ * and exchange steps every exchange_every sweeps (0: none), the next launch of a persistent sweep kernel covers *launch_sweeps
+ * sweeps (<= 127) and holds *exchange_steps exchange steps: it stops at the first step it reaches, or, with several_moves != 0
+ * (resident kernel, single unsharded handle), runs on through every whole period that fits.  RFIM_EINVAL on a bad argument. */
+int rfim_pt_plan_launch(uint64_t sweep_index, int64_t n_sweeps, int exchange_every, int several_moves, int64_t* launch_sweeps,
+                        int* exchange_steps);
 /* diag[0] kernels launched so far, [1] Gaussian attempts decided by the exact binary64 path,
  * [2] decisions within 1e-5 of a binary64 threshold (device and host exp could disagree there;
  * expected 0), [3] exchange decisions taken with a random number */

@@ -84,6 +84,7 @@ SIGNATURES = {
     "rfim_pt_get_bimodal_threshold": (ctypes.c_int, [_vp, ctypes.c_int, ctypes.c_int, ctypes.c_int, ctypes.c_int, _u64p]),
     "rfim_pt_get_diagnostics": (ctypes.c_int, [_vp, _u64p]),
     "rfim_pt_plan_adaptation": (ctypes.c_int, [_dp, _dp, ctypes.c_int, ctypes.c_int, ctypes.c_int, _dp, ctypes.POINTER(ctypes.c_int)]),
+    "rfim_pt_plan_launch": (ctypes.c_int, [ctypes.c_uint64, ctypes.c_int64, ctypes.c_int, ctypes.c_int, ctypes.POINTER(ctypes.c_int64), ctypes.POINTER(ctypes.c_int)]),
     "rfim_pt_bench_philox": (ctypes.c_int, [_vp, ctypes.c_int, _dp, _dp]),
     "rfim_pt_bench_issue": (ctypes.c_int, [_vp, ctypes.c_int, ctypes.c_int, _dp, _dp]),
     "rfim_pt_bench_stream": (ctypes.c_int, [_vp, ctypes.c_size_t, _dp, _dp]),
@@ -426,6 +427,15 @@ def plan_adaptation(T, rate, R, a):
     if rc:
         raise RfimPtError(rc, "rfim_pt_plan_adaptation")
     return out[:n.value].copy()
+
+
+def plan_launch(sweep_index, n_sweeps, exchange_every, several_moves):
+    """rfim_pt_plan_launch: (sweeps, exchange steps) of the next launch of a persistent sweep kernel; no handle, no GPU."""
+    sw, st = ctypes.c_int64(), ctypes.c_int()
+    rc = load().rfim_pt_plan_launch(int(sweep_index), int(n_sweeps), int(exchange_every), int(bool(several_moves)), ctypes.byref(sw), ctypes.byref(st))
+    if rc:
+        raise RfimPtError(rc, "rfim_pt_plan_launch")
+    return int(sw.value), int(st.value)
 
 
 def bench_philox(calls_per_thread=2000, stream=None):

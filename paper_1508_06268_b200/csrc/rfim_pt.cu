@@ -492,10 +492,20 @@ int launch_flow(rfim_pt* h, int sweeps) {
     return RFIM_OK;
 }
 
+// the largest dynamic shared-memory size the kernel can be given on this device (opt-in maximum minus its static part)
+cudaError_t set_max_dynamic_smem(const void* kernel, int optin) {
+    cudaFuncAttributes fa{};
+    cudaError_t e = cudaFuncGetAttributes(&fa, kernel);
+    if (e != cudaSuccess) return e;
+    return cudaFuncSetAttribute(kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, optin - (int)fa.sharedSizeBytes);
+}
+
 template <int KIND, int K, bool NEVER, bool UNI, bool MULTI = false>
 int launch_res_t(rfim_pt* h, const ResPlan& pl, const ResParams& rp) {
     auto kernel = k_sweep_res<KIND, K, NEVER, UNI, kResThreads, MULTI>;
-    CU(cudaFuncSetAttribute(kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)pl.smem));
+    // always the device's opt-in maximum, never this plan's own size: handles driven from several host threads share the
+    // kernel's attribute, and a smaller value set by one between another's set and launch made that launch fail
+    CU(set_max_dynamic_smem(reinterpret_cast<const void*>(kernel), h->smem_optin));
     void* argv[] = {const_cast<void*>(static_cast<const void*>(&h->v)), const_cast<void*>(static_cast<const void*>(&rp))};
     CU(cudaLaunchCooperativeKernel(reinterpret_cast<const void*>(kernel), dim3((unsigned)pl.grid), dim3(kResThreads), argv, pl.smem, h->stream));
     h->launches += 1;
@@ -510,6 +520,24 @@ int launch_res_u(rfim_pt* h, const ResPlan& pl, const ResParams& rp) {
 
 template <int KIND, int K, bool NEVER>
 int launch_res_k(rfim_pt* h, const ResPlan& pl, const ResParams& rp) { return launch_res_u<KIND, K, NEVER>(h, pl, rp); }
+
+// How many sweeps the next launch of a persistent kernel covers and how many exchange steps it holds (pure: no handle).
+// sweep_index = sweeps done so far, left = sweeps still asked for, k = exchange period (0: none), multi = the kernel may hold
+// several steps (resident kernel, single handle).  A launch never exceeds 127 sweeps (the progress words carry 8 bits of phase),
+// ends on an exchange step whenever it reaches one, and with `multi` runs on through as many whole periods as fit.
+void plan_launch(uint64_t sweep_index, int64_t left, int k, bool multi, int64_t* chunk, int* nseg, int64_t* first) {
+    *nseg = 1;
+    *first = k > 0 ? (int64_t)k - (int64_t)(sweep_index % (uint64_t)k) : 0;
+    *chunk = std::min<int64_t>(left, 127);
+    if (k > 0) {
+        if (multi && *chunk >= *first + k) {
+            *nseg = 1 + (int)((*chunk - *first) / k);
+            *chunk = *first + (int64_t)(*nseg - 1) * k;
+        } else {
+            *chunk = std::min<int64_t>(*chunk, *first);
+        }
+    }
+}
 
 // several parallel-tempering moves in one launch: single realisation, not sharded, exchange step fused
 bool res_multi_ok(const rfim_pt* h) {
@@ -583,10 +611,10 @@ int launch_small(rfim_pt* h, int sweeps, bool measure, bool* exchanged) {
     const int threads = std::min(kSmallMaxThreads, std::max(32, (words + 31) / 32 * 32));
     const size_t smem = small_smem_bytes(h->N);
     if (h->kind == RFIM_FIELD_BIMODAL) {
-        CU(cudaFuncSetAttribute(k_sweep_small<0>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
+        CU(set_max_dynamic_smem(reinterpret_cast<const void*>(k_sweep_small<0>), h->smem_optin));   // (a constant: see launch_res_t)
         k_sweep_small<0><<<nrep, threads, smem, h->stream>>>(h->v, sp);
     } else {
-        CU(cudaFuncSetAttribute(k_sweep_small<1>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
+        CU(set_max_dynamic_smem(reinterpret_cast<const void*>(k_sweep_small<1>), h->smem_optin));
         k_sweep_small<1><<<nrep, threads, smem, h->stream>>>(h->v, sp);
     }
     h->launches += 1;
@@ -680,21 +708,10 @@ int do_sweeps(rfim_pt* h, int64_t n_sweeps, int k) {
     const bool flow = variant == 3 || variant == 4 || variant == 5;
     int64_t left = n_sweeps;
     while (left > 0) {
-        int64_t chunk = 1;
+        int64_t chunk = 1, first = 0;
         int nseg = 1;
-        const int64_t first = k > 0 ? (int64_t)k - (int64_t)(h->sweep_g % (uint64_t)k) : 0;   // sweeps to the next exchange step
-        if (flow) {
-            chunk = std::min<int64_t>(left, 127);
-            if (k > 0) {
-                // the resident kernel can hold several moves: as many whole exchange periods as fit in 127 sweeps
-                if (variant == 4 && chunk >= first + k && res_multi_ok(h)) {
-                    nseg = 1 + (int)((chunk - first) / k);
-                    chunk = first + (int64_t)(nseg - 1) * k;
-                } else {
-                    chunk = std::min<int64_t>(chunk, first);
-                }
-            }
-        }
+        // the resident kernel can hold several moves: as many whole exchange periods as fit in 127 sweeps
+        if (flow) plan_launch(h->sweep_g, left, k, variant == 4 && k > 0 && left >= 2 && res_multi_ok(h), &chunk, &nseg, &first);
         // the resident kernel measures in the same launch when its chunk ends on an exchange step
         const bool step_after = k > 0 && ((h->sweep_g + (uint64_t)chunk) % (uint64_t)k) == 0;
         bool exchanged = false;
@@ -1478,6 +1495,16 @@ int rfim_pt_get_bimodal_threshold(rfim_pt* h, int d, int rank, int k, int b, uin
     CU(cudaMemcpyAsync(&nv, h->v.never + (size_t)d * h->R + rank, 4, cudaMemcpyDeviceToHost, h->stream));
     CU(cudaStreamSynchronize(h->stream));
     *thr = ((nv >> idx) & 1u) ? 0ull : (uint64_t)e + 1ull;
+    return RFIM_OK;
+}
+
+int rfim_pt_plan_launch(uint64_t sweep_index, int64_t n_sweeps, int exchange_every, int several_moves, int64_t* launch_sweeps,
+                        int* exchange_steps) {
+    if (n_sweeps < 1 || exchange_every < 0 || !launch_sweeps || !exchange_steps) return RFIM_EINVAL;
+    int64_t first = 0;
+    int nseg = 1;
+    plan_launch(sweep_index, n_sweeps, exchange_every, several_moves != 0, launch_sweeps, &nseg, &first);
+    *exchange_steps = (exchange_every > 0 && (sweep_index + (uint64_t)*launch_sweeps) % (uint64_t)exchange_every == 0) ? nseg : 0;
     return RFIM_OK;
 }
 
