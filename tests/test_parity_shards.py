@@ -226,6 +226,45 @@ def test_sharded_growing_adaptation_equals_oracle(L, R, n0, world, round_robin, 
         g.close()
 
 
+def test_handles_on_several_host_threads_share_the_kernels():
+    """Handles of different sizes (different shared-memory plans of the same kernels) swept concurrently from several host threads,
+    many short calls each: every launch must succeed (the kernels' launch attributes are shared, process-wide state) and each
+    handle must reproduce what it computes alone."""
+    from paper_1508_06268_b200 import binding
+    specs = [(32, 3, GAUSSIAN, 1.5, 11), (64, 2, GAUSSIAN, 1.5, 12), (32, 7, BIMODAL, 2.0, 13), (16, 5, GAUSSIAN, 1.0, 14), (8, 6, BIMODAL, 1.0, 15)]
+    calls = 25
+
+    def run(spec, stream, out, errors):
+        L, R, kind, h, seed = spec
+        try:
+            with torch.cuda.stream(stream):
+                g = binding.RfimPT(L, R, 1.0, h, kind, seed=seed)
+                g.set_temperatures(geometric_ladder(0.9, 5.0, R))
+                for _ in range(calls):
+                    g.sweep(4, 2)
+                out.append((g.get_spins_all(), g.get_permutation()))
+                g.close()
+        except Exception as e:
+            errors.append(e)
+
+    alone = []
+    for spec in specs:
+        out, errors = [], []
+        run(spec, torch.cuda.Stream(), out, errors)
+        assert not errors, errors
+        alone.append(out[0])
+    streams = [torch.cuda.Stream() for _ in specs]
+    outs, errors = [[] for _ in specs], []
+    threads = [threading.Thread(target=run, args=(spec, streams[i], outs[i], errors)) for i, spec in enumerate(specs)]
+    for t in threads:
+        t.start()
+    for t in threads:
+        t.join(timeout=300)
+    assert not errors, errors
+    for (s0, p0), out in zip(alone, outs):
+        assert np.array_equal(out[0][0], s0) and np.array_equal(out[0][1], p0)
+
+
 def test_trial_rates_getter_matches_oracle_trial():
     """rfim_pt_get_trial_rates returns the rates the last adaptation's update was decided on (Figure 9's per-trial numbers)."""
     import oracle
