@@ -44,7 +44,7 @@ def parse():
                     help="replica split: contiguous windows of ceil(R/N) slots (PAPER.md:125, Eq. 6) or round-robin, slot i on rank i mod N (PAPER.md:153)")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-e2e", action="store_true")
-    ap.add_argument("--e2e-handles", type=int, default=3,
+    ap.add_argument("--e2e-handles", type=int, default=4,
                     help="end-to-end leg: handles (host threads, streams) whose steps overlap, copies against sweeps; 1 = one handle, serial")
     ap.add_argument("--stage-timing", action="store_true",
                     help="debug builds with -DRFIM_RES_TIMING only: print the resident kernel's per-stage globaltimer stamps of one step")
@@ -476,7 +476,9 @@ def main():
                 hs.append(hi)
             for hi in hs:
                 hosts.append(torch.empty((wl.D, hi.stored_slots, wl.N // 8), dtype=torch.uint8).pin_memory().numpy())
-            streams = [torch.cuda.Stream() for _ in hs]
+            # distinct stream priorities: when a sweep ends, the copy-out kernel of the handle that just finished is picked before
+            # the next handle's queued sweep, so the handles do not fall into lock-step (all copies, then all sweeps)
+            streams = [torch.cuda.Stream(priority=-(i % 4)) for i in range(len(hs))]
             per = max(6, n_e2e)                   # steps per handle: long enough that filling and draining the pipeline do not count
             errs = []
 
@@ -515,7 +517,7 @@ def main():
                     "h2d_bytes_per_step": int(hosts[0].nbytes), "d2h_bytes_per_step": int(hosts[0].nbytes + obs_bytes),
                     "steps": per * n_pipe, "handles": n_pipe,
                     "what": f"per step: rfim_pt_set_spins_all_bits(host) + rfim_pt_sweep(k,k) + rfim_pt_get_spins_all_bits(host) + rfim_pt_observables; "
-                            f"{n_pipe} handles (independent realisations) driven by {n_pipe} host threads on {n_pipe} streams, so one handle's copies "
+                            f"{n_pipe} handles (independent realisations) driven by {n_pipe} host threads on {n_pipe} streams of distinct priority, so one handle's copies "
                             f"overlap another's sweep; wall clock over all steps"}
 
         bits = torch.empty((wl.D, g.stored_slots, wl.N // 8), dtype=torch.uint8).pin_memory().numpy()
