@@ -27,6 +27,11 @@
 // CTA that finishes last then runs the exchange step itself (small batches), so a whole
 // parallel-tempering move is one launch.
 //
+// Several moves per launch (the MULTI instantiation; single realisation, not sharded).  A call that spans several exchange periods
+// keeps the run in shared memory across them: at the end of a period the CTAs hand their sums over, meet at an arrival counter,
+// the last one to arrive runs the exchange step and releases a flag word, and every CTA re-reads the ranks of its resident slots
+// (lattices never move: only the per-replica tables change) before the task flow goes on with the next period's phases.
+//
 // In shared memory a spin is a byte holding 0 or SP (= 8), four same-colour sites per 32-bit word
 // exactly as in global memory (where it is 0/1), so the six-neighbour count of four sites is a few
 // IADD3, and count*SP + spin*8*SP [+ field bit] is directly the byte offset of the site's entry in
