@@ -163,7 +163,7 @@ int rfim_pt_set_kernel_variant(rfim_pt* h, int variant);
 /* tuning knobs (tests use them to force many-CTA partitions on small problems): key 0 = replicas per
  * work item of the flow kernel (1..64), key 1 = CTA limit of the resident kernel (0 = one per SM), key 2 = partition
  * of the resident kernel (0 automatic, 1 equal runs of planes, 2 whole replicas per CTA where they fit), key 3 = several
- * parallel-tempering moves per launch of the resident kernel (1 allowed, the default; 0 one launch per move). */
+ * parallel-tempering moves per launch of the resident and small-lattice kernels (1 allowed, the default; 0 one launch per move). */
 int rfim_pt_set_tuning(rfim_pt* h, int key, int value);
 /* exchange period used by adapt's trial (default 10) and insertions per trial
  * (default 4, Fig. 6; the paper recommends 1-5). */

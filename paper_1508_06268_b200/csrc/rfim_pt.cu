@@ -85,7 +85,8 @@ struct rfim_pt {
     bool terms_fresh = false;         // View::last holds the energy terms of the CURRENT lattices (last call ended on an exchange step)
     int res_grid_limit = 0;           // 0 = one CTA per SM
     int res_partition = 0;            // resident kernel: 0 automatic, 1 equal runs of planes, 2 whole replicas per CTA
-    int res_multi = 1;                // resident kernel: != 0 allows several parallel-tempering moves per launch (single handle, fused exchange)
+    int res_multi = 1;                // != 0 allows several parallel-tempering moves per launch (resident and small-lattice kernels)
+    int small_per_sm = -1;            // small-lattice kernel: CTAs per SM (occupancy), -1 = not asked yet
     int sm_count = 0, smem_optin = 0;
     std::string err;
 };
@@ -594,7 +595,29 @@ int launch_res(rfim_pt* h, int sweeps, bool measure, bool* exchanged, int nseg =
 
 // `sweeps` (<= 127) sweeps of every active replica in ONE launch of the small-lattice kernel, with the measurement and (single
 // handle, small batch) the exchange step inside
-int launch_small(rfim_pt* h, int sweeps, bool measure, bool* exchanged) {
+int small_threads(const rfim_pt* h) {
+    const int words = (int)(h->Nh / 4);
+    return std::min(kSmallMaxThreads, std::max(32, (words + 31) / 32 * 32));
+}
+// several moves per launch of the small-lattice kernel: the CTAs meet inside the launch, so all of them must be resident at once
+// (a cooperative launch); unsharded handles whose exchange step is fused
+bool small_multi_ok(rfim_pt* h) {
+    if (!h->res_multi || h->shard || h->D > kResFusedExchangeMaxD || h->sm_count < 1) return false;
+    const int nrep = h->D * iterated(h);
+    if (h->small_per_sm < 0) {                          // CTAs of this handle's size one SM holds: a constant of the handle
+        int per_sm = 0;
+        const void* kern = h->kind == RFIM_FIELD_BIMODAL ? reinterpret_cast<const void*>(k_sweep_small<0, true>) : reinterpret_cast<const void*>(k_sweep_small<1, true>);
+        if (set_max_dynamic_smem(kern, h->smem_optin) != cudaSuccess) return false;
+        const cudaError_t e = h->kind == RFIM_FIELD_BIMODAL
+            ? cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, k_sweep_small<0, true>, small_threads(h), small_smem_bytes(h->N))
+            : cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, k_sweep_small<1, true>, small_threads(h), small_smem_bytes(h->N));
+        if (e != cudaSuccess) return false;
+        h->small_per_sm = per_sm;
+    }
+    return nrep >= 1 && (long long)h->small_per_sm * h->sm_count >= nrep;
+}
+
+int launch_small(rfim_pt* h, int sweeps, bool measure, bool* exchanged, int nseg = 1, int first = 0, int period = 0) {
     *exchanged = false;
     const int nrep = h->D * iterated(h);
     if (nrep == 0) return RFIM_OK;                      // this shard stores no active slot
@@ -607,14 +630,21 @@ int launch_small(rfim_pt* h, int sweeps, bool measure, bool* exchanged) {
     sp.xrow = h->series_steps;
     sp.ticket = h->res_prog + kResMaxGrid;
     sp.sweep0 = (uint32_t)h->sweep_g;
-    const int words = (int)(h->Nh / 4);
-    const int threads = std::min(kSmallMaxThreads, std::max(32, (words + 31) / 32 * 32));
+    sp.nseg = nseg; sp.first2 = 2 * first; sp.period2 = 2 * period;
+    sp.xflag = h->res_prog + kResMaxGrid + 1;
+    sp.epoch = ++h->res_epoch;
+    sp.diag = h->v.diag;
+    const int threads = small_threads(h);
     const size_t smem = small_smem_bytes(h->N);
-    if (h->kind == RFIM_FIELD_BIMODAL) {
-        CU(set_max_dynamic_smem(reinterpret_cast<const void*>(k_sweep_small<0>), h->smem_optin));   // (a constant: see launch_res_t)
+    const void* kern = nseg > 1 ? (h->kind == RFIM_FIELD_BIMODAL ? reinterpret_cast<const void*>(k_sweep_small<0, true>) : reinterpret_cast<const void*>(k_sweep_small<1, true>))
+                                : (h->kind == RFIM_FIELD_BIMODAL ? reinterpret_cast<const void*>(k_sweep_small<0>) : reinterpret_cast<const void*>(k_sweep_small<1>));
+    CU(set_max_dynamic_smem(kern, h->smem_optin));                     // (a constant: see launch_res_t)
+    if (nseg > 1) {                                                    // the CTAs wait on one another: co-residency must be guaranteed
+        void* argv[] = {const_cast<void*>(static_cast<const void*>(&h->v)), static_cast<void*>(&sp)};
+        CU(cudaLaunchCooperativeKernel(kern, dim3((unsigned)nrep), dim3((unsigned)threads), argv, smem, h->stream));
+    } else if (h->kind == RFIM_FIELD_BIMODAL) {
         k_sweep_small<0><<<nrep, threads, smem, h->stream>>>(h->v, sp);
     } else {
-        CU(set_max_dynamic_smem(reinterpret_cast<const void*>(k_sweep_small<1>), h->smem_optin));
         k_sweep_small<1><<<nrep, threads, smem, h->stream>>>(h->v, sp);
     }
     h->launches += 1;
@@ -711,12 +741,16 @@ int do_sweeps(rfim_pt* h, int64_t n_sweeps, int k) {
         int64_t chunk = 1, first = 0;
         int nseg = 1;
         // the resident kernel can hold several moves: as many whole exchange periods as fit in 127 sweeps
-        if (flow) plan_launch(h->sweep_g, left, k, variant == 4 && k > 0 && left >= 2 && res_multi_ok(h), &chunk, &nseg, &first);
+        if (flow) {
+            // (the two *_multi_ok checks cost host time: ask only when the call does reach past the next exchange step)
+            const bool spans = k > 0 && std::min<int64_t>(left, 127) >= (int64_t)k - (int64_t)(h->sweep_g % (uint64_t)k) + k;
+            plan_launch(h->sweep_g, left, k, spans && ((variant == 4 && res_multi_ok(h)) || (variant == 5 && small_multi_ok(h))), &chunk, &nseg, &first);
+        }
         // the resident kernel measures in the same launch when its chunk ends on an exchange step
         const bool step_after = k > 0 && ((h->sweep_g + (uint64_t)chunk) % (uint64_t)k) == 0;
         bool exchanged = false;
         int rc = variant == 4 ? launch_res(h, (int)chunk, step_after, &exchanged, nseg, (int)first, k)
-               : variant == 5 ? launch_small(h, (int)chunk, step_after, &exchanged)
+               : variant == 5 ? launch_small(h, (int)chunk, step_after, &exchanged, nseg, (int)first, k)
                : (flow ? launch_flow(h, (int)chunk) : launch_sweep(h));
         if (rc) return rc;
         h->sweep_g += (uint64_t)chunk;

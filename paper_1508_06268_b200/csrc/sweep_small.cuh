@@ -27,6 +27,12 @@ struct SmallParams {
     long long xrow;
     uint32_t* ticket;            // arrival counter (left at zero)
     uint32_t sweep0;             // global sweep index of phase 0
+    // several parallel-tempering moves per launch (cooperative launches only): the launch ends on an exchange step and holds nseg
+    // of them, after phase first2 - 1, first2 + period2 - 1, ...; the lattices stay in shared memory across them
+    int nseg, first2, period2;
+    uint32_t* xflag;             // release word of the mid-launch exchange steps: (epoch << 8) | steps done
+    uint32_t epoch;
+    unsigned long long* diag;
 };
 
 __host__ __device__ inline size_t small_smem_bytes(long long N) { return (size_t)N + 32 * 8 + 3 * 32 * sizeof(long long); }
@@ -45,7 +51,7 @@ __device__ __forceinline__ uint32_t small_neighbours(const uint32_t* o, int w, i
     return cw + sh + o[W * (yp + L * z) + w] + o[W * (ym + L * z) + w] + o[W * (y + L * zp) + w] + o[W * (y + L * zm) + w];
 }
 
-template <int KIND>
+template <int KIND, bool MULTI = false>
 __global__ void __launch_bounds__(kSmallMaxThreads, 1) k_sweep_small(const View v, const SmallParams sp) {
     extern __shared__ __align__(16) uint8_t sm_raw[];
     const int tid = threadIdx.x, T = blockDim.x;
@@ -71,13 +77,17 @@ __global__ void __launch_bounds__(kSmallMaxThreads, 1) k_sweep_small(const View 
     }
     if (KIND == 0) { if (tid < 32) s_tab[tid] = v.etab[(long long)tr * 32 + tid]; }
     else if (tid < 32) s_tab[tid] = reinterpret_cast<const uint32_t*>(v.gtab + (long long)tr * 16)[tid];
-    const uint32_t never = KIND == 0 ? v.never[tr] : 0u;
-    const float band = KIND == 0 ? 0.f : v.band[tr];
-    const double beta = v.beta[tr];
+    uint32_t never = KIND == 0 ? v.never[tr] : 0u;
+    float band = KIND == 0 ? 0.f : v.band[tr];
+    double beta = v.beta[tr];
     __syncthreads();
 
+    const int nseg = MULTI ? sp.nseg : 1;            // several moves per launch: the MULTI instantiation, cooperative launches only
+    for (int seg = 0; seg < nseg; ++seg) {
+    const int p_begin = !MULTI || seg == 0 ? 0 : sp.first2 + (seg - 1) * sp.period2;
+    const int p_end = !MULTI ? sp.phases : sp.first2 + seg * sp.period2;
     // ---- the phases ------------------------------------------------------------------------------------
-    for (int p = 0; p < sp.phases; ++p) {
+    for (int p = p_begin; p < p_end; ++p) {
         const int c = p & 1;
         const uint32_t sweep = sp.sweep0 + (uint32_t)(p >> 1);
         uint32_t* mine = s_spin + c * NW;
@@ -110,10 +120,13 @@ __global__ void __launch_bounds__(kSmallMaxThreads, 1) k_sweep_small(const View 
         __syncthreads();
     }
 
+    if (!MULTI || seg == nseg - 1) {
     // ---- store back ----------------------------------------------------------------------------------------
-    {
-        uint32_t* dst = reinterpret_cast<uint32_t*>(v.spins + ds * 2 * v.Nh);
-        for (int i = tid; i < 2 * NW; i += T) dst[i] = s_spin[i];
+        {
+            uint32_t* dst = reinterpret_cast<uint32_t*>(v.spins + ds * 2 * v.Nh);
+            for (int i = tid; i < 2 * NW; i += T) dst[i] = s_spin[i];
+        }
+
     }
 
     // ---- measurement (S5): every bond has exactly one colour-0 end -----------------------------------------
@@ -155,16 +168,51 @@ __global__ void __launch_bounds__(kSmallMaxThreads, 1) k_sweep_small(const View 
         }
     }
 
+    if (!MULTI || seg == nseg - 1) break;
+    // ---- an exchange step inside the launch: every CTA's sums are in View::acc once all have arrived; the last one runs the
+    // step and releases the flag word; then this replica's new rank, table, guard band and beta (the lattice keeps its slot)
+    {
+        __threadfence();
+        __syncthreads();
+        if (tid == 0) s_last = (atomicAdd(sp.ticket, 1u) == gridDim.x * (unsigned)(seg + 1) - 1u) ? 1 : 0;
+        __syncthreads();
+        const uint32_t xwant = (sp.epoch << 8) | (uint32_t)(seg + 1);
+        if (s_last) {
+            __threadfence();
+            for (int dd = 0; dd < v.D; ++dd) {
+                exchange_member(v, dd, sp.xstep + (uint32_t)seg, sp.xrow + seg, 1);
+                __syncthreads();
+            }
+            __threadfence();
+            if (tid == 0) st_release_gpu(sp.xflag, xwant);
+        } else if (tid == 0) {
+            int polls = 0;
+            while (ld_acquire_gpu(sp.xflag) != xwant) {
+                backoff();
+                if (++polls > (1 << 22)) { atomicOr(sp.diag, 1ull); break; }
+            }
+        }
+        __syncthreads();
+        tr = d * v.R + __ldcg(v.r2t + d * v.R + slot);
+        if (KIND == 0) { if (tid < 32) s_tab[tid] = v.etab[(long long)tr * 32 + tid]; }
+        else if (tid < 32) s_tab[tid] = reinterpret_cast<const uint32_t*>(v.gtab + (long long)tr * 16)[tid];
+        never = KIND == 0 ? v.never[tr] : 0u;
+        band = KIND == 0 ? 0.f : v.band[tr];
+        beta = v.beta[tr];
+        __syncthreads();
+    }
+    }
+
     // ---- exchange step by the CTA that arrives last -------------------------------------------------------------
     if (sp.exchange) {
         __threadfence();
         __syncthreads();
-        if (tid == 0) s_last = (atomicAdd(sp.ticket, 1u) == gridDim.x - 1) ? 1 : 0;
+        if (tid == 0) s_last = (atomicAdd(sp.ticket, 1u) == gridDim.x * (unsigned)nseg - 1u) ? 1 : 0;
         __syncthreads();
         if (s_last) {
             __threadfence();
             for (int dd = 0; dd < v.D; ++dd) {
-                exchange_member(v, dd, sp.xstep, sp.xrow, 1);
+                exchange_member(v, dd, sp.xstep + (uint32_t)(nseg - 1), sp.xrow + (nseg - 1), 1);
                 __syncthreads();
             }
             if (tid == 0) *sp.ticket = 0u;

@@ -289,6 +289,29 @@ def test_resident_kernel_several_moves_per_launch(L, R, grid, partition, kind, h
     g.close(); g1.close(); o.close()
 
 
+@pytest.mark.parametrize("L,R", [(8, 6), (16, 9), (24, 5)])
+@pytest.mark.parametrize("kind,h", [(BIMODAL, 1.0), (GAUSSIAN, 1.5)])
+def test_small_lattice_kernel_several_moves_per_launch(L, R, kind, h):
+    """The one-CTA-per-replica kernel also keeps the lattices in shared memory across exchange periods (a cooperative launch, the
+    exchange steps inside it): against the oracle and against one launch per move, with calls that start off a period boundary."""
+    T = np.geomspace(0.8, 5.0, R)
+    g, o = make_pair(L, R, 1.0, h, kind, 13 * L + R, T)
+    g1, _ = make_pair(L, R, 1.0, h, kind, 13 * L + R, T)
+    g.set_kernel_variant(5); g1.set_kernel_variant(5)
+    g1.set_tuning(3, 0)                                            # one launch per move
+    for chunk, k in [(2, 3), (13, 3), (20, 5), (9, 4), (133, 7)]:
+        l0 = g.diagnostics()["launches"]
+        g.sweep(chunk, k)
+        if (chunk, k) == (20, 5):
+            assert g.diagnostics()["launches"] - l0 == 1           # four exchange steps, one launch
+        g1.sweep(chunk, k); o.sweep(chunk, k)
+        assert_same_state(g, o, what=f"small kernel, several moves per launch, L={L} after chunk {chunk},{k}")
+        assert_same_state(g1, o, what=f"small kernel, one move per launch, L={L} after chunk {chunk},{k}")
+    assert_same_series(g, o)
+    assert_same_series(g1, o)
+    g.close(); g1.close(); o.close()
+
+
 @pytest.mark.parametrize("kind", [BIMODAL, GAUSSIAN])
 def test_resident_kernel_extreme_temperatures_and_long_launch(kind):
     T = np.array([1e-30, 0.05, 1.0, 1e3, 1e30])
