@@ -230,6 +230,28 @@ int rfim_pt_plan_launch(uint64_t sweep_index, int64_t n_sweeps, int exchange_eve
  * expected 0), [3] exchange decisions taken with a random number */
 int rfim_pt_get_diagnostics(rfim_pt* h, uint64_t diag[4]);
 
+/* ---- an entry point that allocates nothing ---------------------------------------------------- */
+
+/* The integer energy terms of Eq. 1 (the measurement of PAPER.md:220) for callers that may not call cudaMalloc
+ * (code under CUDA graph capture, tight serving loops): no handle, no cudaMalloc / cudaFree / allocating library call.  All
+ * three arrays are DEVICE memory owned by the caller:
+ *   spins_device  [R][L^3] int8 +1 / -1, site i = x + L (y + L z)            (the layout of rfim_pt_get_spins_all)
+ *   field_device  [L^3] int32, bimodal +-1 or Gaussian g_i in units of 2^-20 (the layout of rfim_pt_get_field)
+ *   terms_device  [R][3] int64: Eb = sum_bonds s_i s_j, Ef = sum_i h_i s_i (or sum_i g_i s_i), Msum = sum_i s_i, per replica
+ *                 (what rfim_pt_get_energy_terms reports by rank).
+ * The kernel is enqueued on cuda_stream (NULL: stream 0) and the call returns without synchronising.  Its scratch (per-CTA
+ * partial sums, one arrival counter per replica) is a static device array of RFIM_PT_NOALLOC_SCRATCH_BYTES bytes that every
+ * GPU loading the library holds until exit; L <= RFIM_PT_NOALLOC_MAX_L and R <= RFIM_PT_NOALLOC_MAX_R, larger sizes return
+ * RFIM_EINVAL.  All calls on a device share that array: calls that overlap on the GPU (different streams, or several host
+ * threads) race and give wrong sums -- serialise them on one stream.  RFIM_EINVAL: odd or < 2 L, R < 1, bad field_kind, a
+ * null pointer, a size beyond the limits; RFIM_ECUDA: a CUDA call failed.  The message is per host thread. */
+#define RFIM_PT_NOALLOC_MAX_R 256
+#define RFIM_PT_NOALLOC_MAX_L 128
+#define RFIM_PT_NOALLOC_SCRATCH_BYTES (256 * 16 * 3 * 8 + 256 * 4)
+int rfim_pt_energy_terms_noalloc(void* cuda_stream, int L, int R, int field_kind, const int8_t* spins_device,
+                                 const int32_t* field_device, int64_t* terms_device);
+const char* rfim_pt_noalloc_last_error(void);
+
 /* ---- roofline microbenchmarks (bench.py measures both bounds in the same run) ------------- */
 
 /* Philox4x32-10 only: calls_per_thread calls per thread, outputs folded; *ms = device time of one

@@ -85,6 +85,8 @@ SIGNATURES = {
     "rfim_pt_get_diagnostics": (ctypes.c_int, [_vp, _u64p]),
     "rfim_pt_plan_adaptation": (ctypes.c_int, [_dp, _dp, ctypes.c_int, ctypes.c_int, ctypes.c_int, _dp, ctypes.POINTER(ctypes.c_int)]),
     "rfim_pt_plan_launch": (ctypes.c_int, [ctypes.c_uint64, ctypes.c_int64, ctypes.c_int, ctypes.c_int, ctypes.POINTER(ctypes.c_int64), ctypes.POINTER(ctypes.c_int)]),
+    "rfim_pt_energy_terms_noalloc": (ctypes.c_int, [_vp, ctypes.c_int, ctypes.c_int, ctypes.c_int, _vp, _vp, _vp]),
+    "rfim_pt_noalloc_last_error": (ctypes.c_char_p, []),
     "rfim_pt_bench_philox": (ctypes.c_int, [_vp, ctypes.c_int, _dp, _dp]),
     "rfim_pt_bench_issue": (ctypes.c_int, [_vp, ctypes.c_int, ctypes.c_int, _dp, _dp]),
     "rfim_pt_bench_stream": (ctypes.c_int, [_vp, ctypes.c_size_t, _dp, _dp]),
@@ -436,6 +438,20 @@ def plan_launch(sweep_index, n_sweeps, exchange_every, several_moves):
     if rc:
         raise RfimPtError(rc, "rfim_pt_plan_launch")
     return int(sw.value), int(st.value)
+
+
+NOALLOC_MAX_R, NOALLOC_MAX_L = 256, 128      # RFIM_PT_NOALLOC_MAX_R / _MAX_L of include/rfim_pt.h
+
+
+def energy_terms_noalloc(L, R, field_kind, spins_device, field_device, terms_device, stream=None):
+    """rfim_pt_energy_terms_noalloc: (Eb, Ef, Msum) per replica from caller-owned DEVICE arrays, given as integer addresses
+    (e.g. tensor.data_ptr()): spins int8 [R][L^3], field int32 [L^3], terms int64 [R][3].  Enqueues on `stream` (a raw
+    cudaStream_t, default 0) and returns; the library allocates nothing (its scratch is a static device array)."""
+    lib = load()
+    rc = lib.rfim_pt_energy_terms_noalloc(_vp(stream or 0), int(L), int(R), int(field_kind), _vp(int(spins_device)),
+                                          _vp(int(field_device)), _vp(int(terms_device)))
+    if rc:
+        raise RfimPtError(rc, (lib.rfim_pt_noalloc_last_error() or b"").decode())
 
 
 def bench_philox(calls_per_thread=2000, stream=None):

@@ -9,6 +9,7 @@
 #include <cstdint>
 #include <cstdio>
 #include <cstring>
+#include <mutex>
 #include <string>
 #include <vector>
 
@@ -1753,6 +1754,136 @@ int rfim_pt_bench_stream(void* stream, size_t bytes, double* ms, double* bytes_m
     *bytes_moved = 2.0 * (double)n16 * 16.0;
     return rc;
 }
+
+}  // extern "C"
+
+// ---- an entry point that allocates nothing (include/rfim_pt.h: rfim_pt_energy_terms_noalloc) ----------------------
+// For callers that may not call cudaMalloc (CUDA graph capture, tight serving loops): the energy / magnetisation
+// reduction of k_reduce_site (S5; Eq. 1) over caller-owned DEVICE arrays in the boundary's
+// natural site order, with its scratch (per-CTA partial sums and one arrival counter per replica) in a file-scope
+// device array instead of a handle's cudaMalloc'ed accumulators.  Every GPU that loads the library holds the array until
+// exit.  In host code `g_noalloc_scratch` is a host-side stand-in, NOT a device address: the launch code below takes the
+// device address from cudaGetSymbolAddress, once per device, and passes that to the kernel.
+namespace {
+
+constexpr int kNoAllocMaxR = RFIM_PT_NOALLOC_MAX_R;      // replicas per call
+constexpr int kNoAllocMaxL = RFIM_PT_NOALLOC_MAX_L;      // lattice side per call
+constexpr int kNoAllocParts = 16;                        // CTAs (partial sums) per replica
+constexpr int kNoAllocThreads = 256;
+constexpr size_t kNoAllocPartWords = (size_t)kNoAllocMaxR * kNoAllocParts * 3;   // long long [R][part][Eb, Ef, Msum]
+constexpr size_t kNoAllocWords = kNoAllocPartWords + kNoAllocMaxR / 2;           // + uint32 arrival counters [R]
+constexpr int kNoAllocMaxDevices = 64;
+
+static __device__ __align__(256) long long g_noalloc_scratch[kNoAllocWords];     // 98 304 + 1 024 bytes
+static_assert(sizeof(long long) * kNoAllocWords == RFIM_PT_NOALLOC_SCRATCH_BYTES, "rfim_pt.h states the scratch size");
+
+// grid (kNoAllocParts, R).  Eb = sum_i s_i (s_{i+x} + s_{i+y} + s_{i+z}) with periodic wrap counts every bond of
+// k_reduce_site's colour-0 six-neighbour sum once (L = 2: twice, as there).  Pass 1: each CTA's partial sums go to
+// scratch; pass 2: the last CTA of a replica to arrive adds them in CTA order, writes terms[r][3] and re-arms the counter.
+__global__ void k_energy_terms_noalloc(int L, int kind, const int8_t* __restrict__ spins, const int32_t* __restrict__ field,
+                                       long long* __restrict__ terms, long long* scratch) {
+    const int r = blockIdx.y, parts = gridDim.x;
+    const long long N = (long long)L * L * L;
+    const int8_t* s = spins + (long long)r * N;
+    long long* part = scratch + ((long long)r * kNoAllocParts + blockIdx.x) * 3;
+    unsigned int* arrived = reinterpret_cast<unsigned int*>(scratch + kNoAllocPartWords) + r;
+    long long eb = 0, ef = 0, ms = 0;
+    for (long long i = (long long)blockIdx.x * blockDim.x + threadIdx.x; i < N; i += (long long)parts * blockDim.x) {
+        const int x = (int)(i % L), y = (int)((i / L) % L), z = (int)(i / ((long long)L * L));
+        const long long ix = i + (x + 1 == L ? 1 - L : 1);
+        const long long iy = i + (long long)L * (y + 1 == L ? 1 - L : 1);
+        const long long iz = i + (long long)L * L * (z + 1 == L ? 1 - L : 1);
+        const int si = s[i];
+        eb += si * ((int)s[ix] + (int)s[iy] + (int)s[iz]);
+        ms += si;
+        ef += kind == 0 ? (long long)(field[i] > 0 ? si : -si) : (long long)si * field[i];
+    }
+    __shared__ long long red[3][kNoAllocThreads / 32];
+    __shared__ bool last;
+    eb = warp_sum(eb); ef = warp_sum(ef); ms = warp_sum(ms);
+    if ((threadIdx.x & 31) == 0) { red[0][threadIdx.x >> 5] = eb; red[1][threadIdx.x >> 5] = ef; red[2][threadIdx.x >> 5] = ms; }
+    __syncthreads();
+    if (threadIdx.x == 0) {
+        for (int q = 0; q < 3; ++q) {
+            long long a = 0;
+            for (int w = 0; w < kNoAllocThreads / 32; ++w) a += red[q][w];
+            __stcg(part + q, a);
+        }
+        __threadfence();                                         // partial sums visible before the arrival is
+        last = atomicAdd(arrived, 1u) == (unsigned int)parts - 1;
+    }
+    __syncthreads();
+    if (!last) return;
+    if (threadIdx.x < 3) {
+        __threadfence();
+        long long a = 0;
+        for (int p = 0; p < parts; ++p) a += __ldcg(scratch + ((long long)r * kNoAllocParts + p) * 3 + threadIdx.x);
+        terms[(long long)r * 3 + threadIdx.x] = a;
+    }
+    if (threadIdx.x == 0) *arrived = 0;                          // the next call on this stream finds it at zero
+}
+
+thread_local char g_noalloc_err[256] = "";
+
+int noalloc_fail(int code, const char* what, const char* detail = "") {
+    std::snprintf(g_noalloc_err, sizeof g_noalloc_err, "%s%s", what, detail);
+    return code;
+}
+
+// device address of g_noalloc_scratch on the current device, looked up once per device
+int noalloc_scratch(long long** out) {
+    static long long* ptr[kNoAllocMaxDevices] = {};
+    static std::mutex mu;
+    int dev = -1;
+    cudaError_t e = cudaGetDevice(&dev);
+    if (e != cudaSuccess) return noalloc_fail(RFIM_ECUDA, "cudaGetDevice: ", cudaGetErrorString(e));
+    if (dev < 0 || dev >= kNoAllocMaxDevices) return noalloc_fail(RFIM_EINVAL, "device ordinal beyond the scratch table");
+    std::lock_guard<std::mutex> lock(mu);
+    if (!ptr[dev]) {
+        long long* p = nullptr;
+        e = cudaGetSymbolAddress((void**)&p, g_noalloc_scratch);
+        if (e != cudaSuccess || !p) return noalloc_fail(RFIM_ECUDA, "cudaGetSymbolAddress(g_noalloc_scratch): ", cudaGetErrorString(e));
+        ptr[dev] = p;
+    }
+    *out = ptr[dev];
+    return RFIM_OK;
+}
+
+}  // namespace
+
+extern "C" {
+
+int rfim_pt_energy_terms_noalloc(void* cuda_stream, int L, int R, int field_kind, const int8_t* spins_device,
+                                 const int32_t* field_device, int64_t* terms_device) {
+    char lim[96];
+    if (L < 2 || (L & 1)) return noalloc_fail(RFIM_EINVAL, "L must be even and >= 2");
+    if (L > kNoAllocMaxL) {
+        std::snprintf(lim, sizeof lim, "L = %d is beyond RFIM_PT_NOALLOC_MAX_L = %d", L, kNoAllocMaxL);
+        return noalloc_fail(RFIM_EINVAL, lim);
+    }
+    if (R < 1) return noalloc_fail(RFIM_EINVAL, "R must be >= 1");
+    if (R > kNoAllocMaxR) {
+        std::snprintf(lim, sizeof lim, "R = %d is beyond RFIM_PT_NOALLOC_MAX_R = %d (the static scratch holds that many replicas)", R, kNoAllocMaxR);
+        return noalloc_fail(RFIM_EINVAL, lim);
+    }
+    if (field_kind != RFIM_FIELD_BIMODAL && field_kind != RFIM_FIELD_GAUSSIAN) return noalloc_fail(RFIM_EINVAL, "bad field_kind");
+    if (!spins_device || !field_device || !terms_device) return noalloc_fail(RFIM_EINVAL, "null device pointer");
+    long long* scratch = nullptr;
+    int rc = noalloc_scratch(&scratch);
+    if (rc) return rc;
+    cudaStream_t s = reinterpret_cast<cudaStream_t>(cuda_stream);
+    // the arrival counters must start at zero whatever an earlier (possibly failed) call left behind
+    cudaError_t e = cudaMemsetAsync(scratch + kNoAllocPartWords, 0, sizeof(unsigned int) * kNoAllocMaxR, s);
+    if (e != cudaSuccess) return noalloc_fail(RFIM_ECUDA, "cudaMemsetAsync: ", cudaGetErrorString(e));
+    k_energy_terms_noalloc<<<dim3(kNoAllocParts, R), kNoAllocThreads, 0, s>>>(L, field_kind, spins_device, field_device,
+                                                                             reinterpret_cast<long long*>(terms_device), scratch);
+    e = cudaGetLastError();
+    if (e != cudaSuccess) return noalloc_fail(RFIM_ECUDA, "k_energy_terms_noalloc launch: ", cudaGetErrorString(e));
+    g_noalloc_err[0] = 0;
+    return RFIM_OK;
+}
+
+const char* rfim_pt_noalloc_last_error(void) { return g_noalloc_err; }
 
 }  // extern "C"
 
