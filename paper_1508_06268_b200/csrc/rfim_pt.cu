@@ -1855,7 +1855,7 @@ extern "C" {
 
 int rfim_pt_energy_terms_noalloc(void* cuda_stream, int L, int R, int field_kind, const int8_t* spins_device,
                                  const int32_t* field_device, int64_t* terms_device) {
-    char lim[96];
+    char lim[160];
     if (L < 2 || (L & 1)) return noalloc_fail(RFIM_EINVAL, "L must be even and >= 2");
     if (L > kNoAllocMaxL) {
         std::snprintf(lim, sizeof lim, "L = %d is beyond RFIM_PT_NOALLOC_MAX_L = %d", L, kNoAllocMaxL);
