@@ -292,12 +292,17 @@ int upload_tables(rfim_pt* h) {
                     e.y = (float)(c * sigma * h->v.hs);           // multiplies (float)g_i, which is exact
                     gtab[((size_t)d * R + t) * 16 + idx] = e;
                 }
-                // guard band: bound on |P~ - P| over the float path, in units of u
+                // guard band: bound on |P~ - P| over the float path, in units of u.  arg = fl(g*fl(y) + fl(x)):
+                // y's rounding moves it by <= |g y| 2^-24 <= aY 2^-24, x's by <= Xmax 2^-24, the fused multiply-add's one rounding by
+                // <= 33 * 2^-24 wherever the decision is open (0 <= arg <= 33: below, P~ < 1 + band; above, both rules accept);
+                // ex2.approx is taken at 2^-21 relative (twice its stated bound); float(u) is within 512 of u in either rounding
+                // mode and the binary64 threshold within 1 of P 2^32.  The float decision can differ from the exact one only when
+                // |float(u) - P~| <= 2^32 eta + 513: a quarter on top of that, and 1024 instead of 513.
                 const double aY = h->amax[d] * std::fabs(c);
                 const double Xmax = std::fabs(c) * std::fabs(h->J) * 6.0 + 32.0;
-                const double arg_err = std::ldexp(3.0 * aY + 2.0 * Xmax, -24);
-                const double eta = M_LN2 * arg_err + std::ldexp(1.0, -21) + std::ldexp(1.0, -22);   // ex2.approx, float(u) (rounded down by the resident kernel: < 2^-23)
-                const double bd = 1.5 * eta * kTwo32 + 512.0;
+                const double arg_err = std::ldexp(aY + Xmax + 33.0, -24);
+                const double eta = M_LN2 * arg_err + std::ldexp(1.0, -21);
+                const double bd = 1.25 * eta * kTwo32 + 1024.0;
                 band[(size_t)d * R + t] = (float)std::min(bd, 3.0e38);
             }
         CU(cudaMemcpyAsync(const_cast<GaussEntry*>(h->v.gtab), gtab.data(), gtab.size() * sizeof(GaussEntry), cudaMemcpyHostToDevice, h->stream));
